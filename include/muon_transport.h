@@ -1,0 +1,163 @@
+/* muon_transport.h — C ABI of the B200-native muon transport library (libmuon_transport.so).
+ *
+ * The library implements the per-muon transport step loop of "Ultra-Fast Muon Transport via Histogram
+ * Sampling on GPUs" (arxiv 2512.10520): Algorithm 1 (§4) with the sampling of §2-§3
+ * (L51-53, L73-77), the rotation of §4.2 (L124-129, Eq. 3) and the RK4 Lorentz push of §4.3 (L133-137,
+ * Eq. 4).  The exact arithmetic is DESIGN.md §3.  Call order follows the paper's statement of the problem
+ * (Alg. 1 "Input", L144-146; static data resident in GPU global memory, L174):
+ *
+ *     mt_create -> mt_load_histograms -> mt_build_alias -> mt_set_geometry -> mt_transport (any number)
+ *
+ * Conventions.  Units: metres, GeV/c, tesla.  Every function returns an int status: MT_OK (0) or a
+ * negative MT_ERR_* code; nothing throws or aborts across this boundary; mt_last_error() gives a text for
+ * the last failure on a context.  A context belongs to one CUDA device and is not thread-safe.  "HOST"
+ * pointers are ordinary host memory, read during the call and never retained.  "DEVICE" pointers are
+ * CUDA device memory on the context's device; the caller owns them (the library never frees them), and
+ * those marked "borrowed" must stay valid and unchanged until the context is destroyed or the geometry is
+ * replaced.  There is no CPU implementation behind these calls: without a CUDA device they fail.
+ */
+#ifndef MUON_TRANSPORT_H_
+#define MUON_TRANSPORT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mt_ctx mt_ctx;
+
+enum {
+  MT_OK = 0,
+  MT_ERR_INVALID_ARG = -1, /* null pointer, non-positive size, unsorted regions, ...                      */
+  MT_ERR_STATE = -2,       /* call order violated (e.g. mt_transport before mt_set_geometry)               */
+  MT_ERR_EMPTY_HIST = -3,  /* a (material, bin) histogram sums to 0 or holds a negative / non-finite count */
+  MT_ERR_UNSUPPORTED = -4, /* a size beyond what the kernels support (see each call)                       */
+  MT_ERR_CUDA = -5,        /* a CUDA runtime call failed; mt_last_error() has the CUDA message             */
+  MT_ERR_NOMEM = -6
+};
+
+/* termination flags written to the outputs (Alg. 1 l.2-4, L148-151) */
+enum { MT_FLAG_STOPPED = 1, MT_FLAG_EXITED = 2, MT_FLAG_ESCAPED = 3, MT_FLAG_MAXSTEPS = 4 };
+
+enum { MT_GEOM_REGIONS = 0, MT_GEOM_VOXEL = 1 };
+
+/* alias-table placement (north_star subsystem 1) */
+enum { MT_PLACE_AUTO = 0, MT_PLACE_SMEM = 1, MT_PLACE_L2 = 2 };
+
+/* scheduling of muons onto lanes (north_star subsystem 4); results never depend on it */
+enum {
+  MT_SCHED_AUTO = 0,
+  MT_SCHED_STATIC = 1,     /* one lane per muon for its whole life (the paper's mapping, L59, L174)        */
+  MT_SCHED_REFILL = 2,     /* persistent warps; idle lanes refill from a global work counter               */
+  MT_SCHED_WAVEFRONT = 3   /* z-slab passes over a compacted live list (field working set stays in L2/L1)  */
+};
+
+/* integer options for mt_set_option */
+enum {
+  MT_OPT_SCHEDULE = 1,       /* MT_SCHED_*                                                                 */
+  MT_OPT_BLOCK_THREADS = 2,  /* 0 = library default; else a multiple of 32 in [32, 1024]                   */
+  MT_OPT_BLOCKS_PER_SM = 3,  /* 0 = library default (persistent kernels)                                   */
+  MT_OPT_SLAB_CELLS = 4,     /* wavefront: slab thickness along z, in units of 1 cm; 0 = default           */
+  MT_OPT_REFILL_MIN_IDLE = 5 /* refill: lanes of a warp that must be idle before it refills; 0 = default   */
+};
+
+const char* mt_strerror(int code);
+const char* mt_last_error(const mt_ctx* ctx);
+
+/* Create / destroy a context on CUDA device `cuda_device`.  MT_ERR_CUDA if there is no such device. */
+int mt_create(mt_ctx** out, int cuda_device);
+int mt_destroy(mt_ctx* ctx);
+int mt_set_option(mt_ctx* ctx, int option, int64_t value);
+
+/* Histograms H_{M,i} (BASELINE.json configs[0]: one Dp/p and one polar-angle
+ * histogram per material and momentum bin, on log2 axes).  All arrays HOST, row-major, copied. */
+typedef struct {
+  int32_t n_materials;     /* material ids 1..n_materials; id 0 = vacuum, never sampled (L155); <= 255     */
+  int32_t n_pbins;         /* log-spaced momentum bins over [p_lo, p_hi] GeV/c (L99); 1..4096              */
+  float p_lo, p_hi;
+  int32_t n_dp, n_th;      /* cells per Dp/p and per theta histogram; 1..65536                             */
+  const float* counts_dp;  /* [n_materials][n_pbins][n_dp] non-negative weights                            */
+  const float* counts_th;  /* [n_materials][n_pbins][n_th]                                                 */
+  const float* axis_dp;    /* [n_materials][n_pbins][2] = {log2 of the lower edge, log2 width of a cell}   */
+  const float* axis_th;    /* same for theta (radians)                                                     */
+  const float* step_m;     /* [n_materials + 1] path length per step in material id (index 0 = vacuum)     */
+} mt_hist_desc;
+int mt_load_histograms(mt_ctx* ctx, const mt_hist_desc* desc);
+
+/* Build the alias tables (Walker/Vose; construction order DESIGN.md §3.9), pack them
+ * and upload them.  MT_ERR_EMPTY_HIST names the offending table in mt_last_error(). */
+int mt_build_alias(mt_ctx* ctx, int placement);
+
+/* Test export of the tables as built: HOST outputs shaped like counts_dp / counts_th. */
+int mt_get_alias(const mt_ctx* ctx, float* prob_dp, uint32_t* alias_dp, float* prob_th, uint32_t* alias_th);
+
+/* Geometry G and field map (Alg. 1 "Input", L144-146; L61-63; §4.3).  Regions: axis-aligned boxes,
+ * half-open on every axis, sorted by z_lo and disjoint in z.  Voxel: cell (ix,iy,iz) spans
+ * [o + i*cell, o + (i+1)*cell); field values sit at cell centres and are interpolated trilinearly. */
+typedef struct {
+  float z_lo, z_hi, x_lo, x_hi, y_lo, y_hi;
+  int32_t material;
+  float bx, by, bz;        /* uniform field inside the box                                                 */
+} mt_region;
+
+typedef struct {
+  int32_t mode;            /* MT_GEOM_REGIONS | MT_GEOM_VOXEL                                              */
+  float x_min, x_max, y_min, y_max, z_min, z_exit; /* world box; z >= z_exit -> EXITED                    */
+  float p_min;             /* |p| < p_min -> STOPPED                                                       */
+  int32_t max_steps;       /* step cap -> MAXSTEPS                                                         */
+  int32_t world_material;  /* material outside every region / outside the voxel grid                       */
+  int32_t n_regions;       /* REGIONS mode: 0..1024                                                        */
+  const mt_region* regions;/* HOST, copied                                                                 */
+  int32_t nx, ny, nz;      /* VOXEL mode                                                                   */
+  float ox, oy, oz, cell;
+  const uint8_t* d_material; /* DEVICE [nz][ny][nx], read during the call only                            */
+  const float* d_field;      /* DEVICE [nz][ny][nx][3], read during the call only                         */
+} mt_geometry;
+/* VOXEL mode repacks both grids into one library-owned 16-byte-per-cell grid {Bx,By,Bz,material}
+ * (DESIGN.md §6), so the caller may free d_material / d_field after the call returns. */
+int mt_set_geometry(mt_ctx* ctx, const mt_geometry* geom);
+
+/* Muon state, SoA of 16-byte records (north_star subsystem 3). */
+typedef struct {
+  const float* pos_q;      /* [n][4] = x, y, z, charge (+1.f / -1.f)                                       */
+  const float* mom;        /* [n][4] = px, py, pz, unused                                                  */
+} mt_muons_in;
+
+typedef struct {
+  float* pos_flag;         /* [n][4] = final x, y, z, flag (int32 bits in the 4th float)                   */
+  float* mom_steps;        /* [n][4] = final px, py, pz, step count (int32 bits)                           */
+  float* exit_rec;         /* optional [exit_capacity][8]: x,y,z,index(uint32 bits),px,py,pz,steps(int32)  */
+  uint32_t* exit_count;    /* optional, one counter; ADDED to (caller zeroes it); may exceed the capacity  */
+  uint32_t exit_capacity;
+  uint64_t* counters;      /* optional [8], ADDED to: [0] total steps, [1..4] muons per flag               */
+} mt_muons_out;
+
+/* Transport n muons (ids id_base .. id_base+n-1) until each meets a break condition.  All buffers DEVICE.
+ * Asynchronous: kernels are enqueued on `cuda_stream` (a cudaStream_t; NULL = default stream) and the call
+ * returns; outputs are complete when the stream reaches that point.  Outputs are a function of (inputs,
+ * seed, id) only — not of launch shape, schedule, batch split or refill order. */
+int mt_transport(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                 const mt_muons_out* out, void* cuda_stream);
+
+/* Same with HOST buffers: copies in, transports, copies out on `cuda_stream`, then synchronises it.
+ * exit_rec / exit_count / counters (if non-NULL) are HOST too; exit_count and counters are overwritten. */
+int mt_transport_host(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                      const mt_muons_out* out, void* cuda_stream);
+
+/* Number of kernel launches made by this context so far (bench.py's gpu_launches). */
+int64_t mt_launch_count(const mt_ctx* ctx);
+
+/* Test hooks (DEVICE buffers, asynchronous on the stream).
+ * mt_debug_sample: cell_out[i] = alias draw from table `which` (0 = Dp/p, 1 = theta) of
+ * (material, pbin) with word d_words[i].
+ * mt_debug_philox: out[i][0..3] = Philox4x32-10 block for (seed, id_base + i, step). */
+int mt_debug_sample(mt_ctx* ctx, int material, int pbin, int which, const uint32_t* d_words, uint64_t n,
+                    uint32_t* d_cell_out, void* cuda_stream);
+int mt_debug_philox(mt_ctx* ctx, uint64_t seed, uint64_t id_base, uint32_t step, uint64_t n,
+                    uint32_t* d_out, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MUON_TRANSPORT_H_ */

@@ -1,0 +1,29 @@
+// mt_launch.h — launcher interface between mt_lib.cu (host logic) and mt_kernels.cu (kernels).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "mt_params.h"
+
+#ifndef MT_MAX_THREADS
+#define MT_MAX_THREADS 256      // largest block the transport kernel is compiled for
+#endif
+#ifndef MT_MIN_BLOCKS
+#define MT_MIN_BLOCKS 3         // -> at most 85 registers per thread
+#endif
+
+struct MtLaunchCfg {
+  unsigned grid, block;
+  size_t smem_bytes;
+  int pack;        // 32 or 64 (bits per packed alias cell)
+  bool tab_smem;   // tables staged in shared memory
+  int sched;       // MT_SCHED_STATIC / _REFILL / _WAVEFRONT
+};
+
+cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream);
+cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm);
+cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, float4* out, size_t n_cells, int* d_max_material,
+                             cudaStream_t stream);
+cudaError_t mt_launch_debug_sample(int pack, const void* tab, uint32_t N, const uint32_t* words, uint64_t n,
+                                   uint32_t* out, cudaStream_t stream);
+cudaError_t mt_launch_debug_philox(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,
+                                   uint32_t* out, cudaStream_t stream);

@@ -1,0 +1,560 @@
+// mt_lib.cu — host side of the C ABI in include/muon_transport.h: context, alias-table construction and
+// packing, geometry upload, schedule selection and the transport launch sequences.
+// No transport arithmetic runs on the host; there is no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/muon_transport.h"
+#include "mt_launch.h"
+
+namespace {
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t bytes = 0;
+  cudaError_t reserve(size_t want) {
+    if (want <= bytes) return cudaSuccess;
+    if (p) cudaFree(p);
+    p = nullptr; bytes = 0;
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e == cudaSuccess) bytes = want;
+    return e;
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+};
+
+}  // namespace
+
+struct mt_ctx {
+  int device = 0;
+  int sm_count = 0;
+  size_t smem_optin = 0;
+  std::string last_error;
+  // options
+  int opt_sched = MT_SCHED_AUTO, opt_block = 0, opt_blocks_per_sm = 0, opt_slab_cells = 0, opt_min_idle = 0;
+  // histograms (host copies)
+  bool have_hist = false, have_tables = false, have_geom = false;
+  int32_t n_materials = 0, n_pbins = 0, n_dp = 0, n_th = 0;
+  float p_lo = 0, p_hi = 0;
+  std::vector<float> counts_dp, counts_th, axis_dp, axis_th, step_m;
+  // built tables (host, for mt_get_alias) and packed device copies
+  std::vector<float> prob_dp, prob_th;
+  std::vector<uint32_t> alias_dp, alias_th;
+  int pack = 32;
+  int placement = MT_PLACE_AUTO;
+  size_t table_bytes = 0;
+  DevBuf d_tab, d_axes, d_blob, d_grid, d_scratch, d_live[2], d_stage_in, d_stage_out, d_stage_misc;
+  // geometry
+  mt_geometry geom{};
+  std::vector<mt_region> regions;
+  MtBlobLayout bl{};
+  int64_t launches = 0;
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int fail(mt_ctx* c, int code, const char* fmt, ...) {
+  if (c) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    c->last_error = buf;
+  }
+  return code;
+}
+
+#define MT_CUDA(c, expr)                                                                             \
+  do {                                                                                               \
+    cudaError_t e_ = (expr);                                                                         \
+    if (e_ != cudaSuccess)                                                                           \
+      return fail((c), e_ == cudaErrorMemoryAllocation ? MT_ERR_NOMEM : MT_ERR_CUDA, "%s: %s", #expr, \
+                  cudaGetErrorString(e_));                                                           \
+  } while (0)
+
+// Walker/Vose construction with a pinned pairing order.  Returns false on an empty or
+// invalid histogram.
+bool build_one_alias(const float* counts, int N, float* prob, uint32_t* alias) {
+  double total = 0.0;
+  for (int j = 0; j < N; ++j) {
+    const float v = counts[j];
+    if (!(v >= 0.0f) || isinf(v)) return false;
+    total += (double)v;
+  }
+  if (!(total > 0.0)) return false;
+  std::vector<double> scaled(N);
+  std::vector<int> below, above;           // stacks of cells with scaled mass < 1 and >= 1
+  below.reserve(N); above.reserve(N);
+  for (int j = 0; j < N; ++j) {
+    scaled[j] = ((double)counts[j] * (double)N) / total;
+    (scaled[j] < 1.0 ? below : above).push_back(j);
+  }
+  while (!below.empty() && !above.empty()) {
+    const int s = below.back(), l = above.back();
+    below.pop_back(); above.pop_back();
+    prob[s] = (float)scaled[s];
+    alias[s] = (uint32_t)l;
+    scaled[l] = (scaled[l] + scaled[s]) - 1.0;
+    (scaled[l] < 1.0 ? below : above).push_back(l);
+  }
+  for (int j : above) { prob[j] = 1.0f; alias[j] = (uint32_t)j; }
+  for (int j : below) { prob[j] = 1.0f; alias[j] = (uint32_t)j; }
+  return true;
+}
+
+// integer acceptance threshold: a24 < T  <=>  (float)a24 * 2^-24 < prob
+uint32_t threshold24(float prob) {
+  const double t = ceil((double)prob * 16777216.0);
+  return t <= 0.0 ? 0u : (t >= 16777216.0 ? 16777216u : (uint32_t)t);
+}
+
+size_t blob_bytes(const mt_ctx* c) { return (size_t)c->bl.n_words * sizeof(float); }
+
+int rebuild_blob(mt_ctx* c) {
+  // [edges][steps x4][z_lo][regions]; see mt_params.h
+  const int n_edges = c->n_pbins + 1;
+  const int n_reg = c->have_geom ? (int)c->regions.size() : 0;
+  MtBlobLayout bl;
+  bl.off_steps = (n_edges + 3) & ~3;
+  bl.off_zlo = bl.off_steps + 4 * (c->n_materials + 1);
+  bl.off_regions = (bl.off_zlo + n_reg + 3) & ~3;
+  bl.n_words = bl.off_regions + 10 * n_reg;
+  std::vector<float> blob((size_t)bl.n_words + 4, 0.0f);
+  const double lo = (double)c->p_lo, hi = (double)c->p_hi;
+  for (int j = 0; j <= c->n_pbins; ++j)
+    blob[j] = (float)(lo * pow(hi / lo, (double)j / (double)c->n_pbins));                 // §3.4
+  for (int m = 0; m <= c->n_materials; ++m) {
+    const float h = c->step_m[m];
+    blob[bl.off_steps + 4 * m + 0] = h;
+    blob[bl.off_steps + 4 * m + 1] = h * 0.5f;
+    blob[bl.off_steps + 4 * m + 2] = (float)((double)h / 6.0);                           // §3.2
+  }
+  for (int j = 0; j < n_reg; ++j) {
+    blob[bl.off_zlo + j] = c->regions[j].z_lo;
+    static_assert(sizeof(mt_region) == 40 && sizeof(MtRegionDev) == 40, "region layout");
+    memcpy(&blob[bl.off_regions + 10 * j], &c->regions[j], sizeof(mt_region));
+  }
+  c->bl = bl;
+  MT_CUDA(c, c->d_blob.reserve(blob.size() * sizeof(float)));
+  MT_CUDA(c, cudaMemcpy(c->d_blob.p, blob.data(), blob.size() * sizeof(float), cudaMemcpyHostToDevice));
+  return MT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mt_strerror(int code) {
+  switch (code) {
+    case MT_OK: return "ok";
+    case MT_ERR_INVALID_ARG: return "invalid argument";
+    case MT_ERR_STATE: return "call order violated";
+    case MT_ERR_EMPTY_HIST: return "empty or invalid histogram";
+    case MT_ERR_UNSUPPORTED: return "unsupported size or mode";
+    case MT_ERR_CUDA: return "CUDA error";
+    case MT_ERR_NOMEM: return "out of memory";
+    default: return "unknown error";
+  }
+}
+
+const char* mt_last_error(const mt_ctx* ctx) { return ctx ? ctx->last_error.c_str() : "null context"; }
+
+int mt_create(mt_ctx** out, int cuda_device) {
+  if (!out) return MT_ERR_INVALID_ARG;
+  *out = nullptr;
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cuda_device < 0 || cuda_device >= n_dev) {
+    cudaGetLastError();
+    return MT_ERR_CUDA;
+  }
+  mt_ctx* c = new (std::nothrow) mt_ctx;
+  if (!c) return MT_ERR_NOMEM;
+  c->device = cuda_device;
+  DeviceGuard g(cuda_device);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { delete c; return MT_ERR_CUDA; }
+  c->sm_count = prop.multiProcessorCount;
+  c->smem_optin = prop.sharedMemPerBlockOptin;
+  *out = c;
+  return MT_OK;
+}
+
+int mt_destroy(mt_ctx* c) {
+  if (!c) return MT_OK;
+  DeviceGuard g(c->device);
+  DevBuf* bufs[] = {&c->d_tab, &c->d_axes, &c->d_blob, &c->d_grid, &c->d_scratch, &c->d_live[0], &c->d_live[1],
+                    &c->d_stage_in, &c->d_stage_out, &c->d_stage_misc};
+  for (DevBuf* b : bufs) b->release();
+  delete c;
+  return MT_OK;
+}
+
+int mt_set_option(mt_ctx* c, int option, int64_t value) {
+  if (!c) return MT_ERR_INVALID_ARG;
+  switch (option) {
+    case MT_OPT_SCHEDULE:
+      if (value < MT_SCHED_AUTO || value > MT_SCHED_WAVEFRONT) return fail(c, MT_ERR_INVALID_ARG, "bad schedule %lld", (long long)value);
+      c->opt_sched = (int)value; return MT_OK;
+    case MT_OPT_BLOCK_THREADS:
+      if (value != 0 && (value < 32 || value > MT_MAX_THREADS || value % 32))
+        return fail(c, MT_ERR_INVALID_ARG, "block threads must be a multiple of 32 in [32, %d]", MT_MAX_THREADS);
+      c->opt_block = (int)value; return MT_OK;
+    case MT_OPT_BLOCKS_PER_SM:
+      if (value < 0 || value > 32) return fail(c, MT_ERR_INVALID_ARG, "bad blocks per SM");
+      c->opt_blocks_per_sm = (int)value; return MT_OK;
+    case MT_OPT_SLAB_CELLS:
+      if (value < 0 || value > 1000000) return fail(c, MT_ERR_INVALID_ARG, "bad slab thickness");
+      c->opt_slab_cells = (int)value; return MT_OK;
+    case MT_OPT_REFILL_MIN_IDLE:
+      if (value < 0 || value > 32) return fail(c, MT_ERR_INVALID_ARG, "bad refill threshold");
+      c->opt_min_idle = (int)value; return MT_OK;
+    default: return fail(c, MT_ERR_INVALID_ARG, "unknown option %d", option);
+  }
+}
+
+int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) {
+  if (!c || !d) return MT_ERR_INVALID_ARG;
+  if (!d->counts_dp || !d->counts_th || !d->axis_dp || !d->axis_th || !d->step_m)
+    return fail(c, MT_ERR_INVALID_ARG, "null histogram array");
+  if (d->n_materials < 1 || d->n_materials > 255 || d->n_pbins < 1 || d->n_pbins > 4096 || d->n_dp < 1 ||
+      d->n_dp > 65536 || d->n_th < 1 || d->n_th > 65536)
+    return fail(c, MT_ERR_UNSUPPORTED, "histogram shape out of range");
+  if (!(d->p_lo > 0.0f) || !(d->p_hi > d->p_lo) || isinf(d->p_hi))
+    return fail(c, MT_ERR_INVALID_ARG, "need 0 < p_lo < p_hi");
+  for (int m = 0; m <= d->n_materials; ++m)
+    if (!(d->step_m[m] > 0.0f) || isinf(d->step_m[m])) return fail(c, MT_ERR_INVALID_ARG, "step_m[%d] must be positive", m);
+  const size_t nt = (size_t)d->n_materials * d->n_pbins;
+  c->n_materials = d->n_materials; c->n_pbins = d->n_pbins; c->n_dp = d->n_dp; c->n_th = d->n_th;
+  c->p_lo = d->p_lo; c->p_hi = d->p_hi;
+  c->counts_dp.assign(d->counts_dp, d->counts_dp + nt * d->n_dp);
+  c->counts_th.assign(d->counts_th, d->counts_th + nt * d->n_th);
+  c->axis_dp.assign(d->axis_dp, d->axis_dp + nt * 2);
+  c->axis_th.assign(d->axis_th, d->axis_th + nt * 2);
+  c->step_m.assign(d->step_m, d->step_m + d->n_materials + 1);
+  c->have_hist = true;
+  c->have_tables = false;
+  return MT_OK;
+}
+
+int mt_build_alias(mt_ctx* c, int placement) {
+  if (!c) return MT_ERR_INVALID_ARG;
+  if (!c->have_hist) return fail(c, MT_ERR_STATE, "mt_build_alias before mt_load_histograms");
+  if (placement < MT_PLACE_AUTO || placement > MT_PLACE_L2) return fail(c, MT_ERR_INVALID_ARG, "bad placement");
+  DeviceGuard g(c->device);
+  const size_t nt = (size_t)c->n_materials * c->n_pbins;
+  const int n_dp = c->n_dp, n_th = c->n_th, n_cells = n_dp + n_th;
+  c->prob_dp.assign(nt * n_dp, 0.0f); c->alias_dp.assign(nt * n_dp, 0u);
+  c->prob_th.assign(nt * n_th, 0.0f); c->alias_th.assign(nt * n_th, 0u);
+  for (size_t t = 0; t < nt; ++t) {
+    if (!build_one_alias(&c->counts_dp[t * n_dp], n_dp, &c->prob_dp[t * n_dp], &c->alias_dp[t * n_dp]))
+      return fail(c, MT_ERR_EMPTY_HIST, "Dp/p histogram of material %d, momentum bin %d is empty or invalid",
+                  (int)(t / c->n_pbins) + 1, (int)(t % c->n_pbins));
+    if (!build_one_alias(&c->counts_th[t * n_th], n_th, &c->prob_th[t * n_th], &c->alias_th[t * n_th]))
+      return fail(c, MT_ERR_EMPTY_HIST, "theta histogram of material %d, momentum bin %d is empty or invalid",
+                  (int)(t / c->n_pbins) + 1, (int)(t % c->n_pbins));
+  }
+  // pack: per (material, pbin) the Dp/p cells followed by the theta cells
+  c->pack = (std::max(n_dp, n_th) <= 256) ? 32 : 64;
+  std::vector<uint32_t> packed(nt * n_cells * (c->pack == 32 ? 1 : 2));
+  for (size_t t = 0; t < nt; ++t) {
+    for (int k = 0; k < n_cells; ++k) {
+      const bool is_dp = k < n_dp;
+      const float pr = is_dp ? c->prob_dp[t * n_dp + k] : c->prob_th[t * n_th + (k - n_dp)];
+      uint32_t al = is_dp ? c->alias_dp[t * n_dp + k] : c->alias_th[t * n_th + (k - n_dp)];
+      uint32_t T = threshold24(pr);
+      const uint32_t self = (uint32_t)(is_dp ? k : k - n_dp);
+      if (c->pack == 32) {
+        if (T >= 16777216u) { T = 16777215u; al = self; }     // prob == 1: the alias is never taken
+        packed[t * n_cells + k] = (T << 8) | al;
+      } else {
+        packed[2 * (t * n_cells + k)] = T;
+        packed[2 * (t * n_cells + k) + 1] = al;
+      }
+    }
+  }
+  c->table_bytes = packed.size() * sizeof(uint32_t);
+  MT_CUDA(c, c->d_tab.reserve(c->table_bytes));
+  MT_CUDA(c, cudaMemcpy(c->d_tab.p, packed.data(), c->table_bytes, cudaMemcpyHostToDevice));
+  std::vector<float> axes(nt * 4);
+  for (size_t t = 0; t < nt; ++t) {
+    axes[4 * t + 0] = c->axis_dp[2 * t]; axes[4 * t + 1] = c->axis_dp[2 * t + 1];
+    axes[4 * t + 2] = c->axis_th[2 * t]; axes[4 * t + 3] = c->axis_th[2 * t + 1];
+  }
+  MT_CUDA(c, c->d_axes.reserve(axes.size() * sizeof(float)));
+  MT_CUDA(c, cudaMemcpy(c->d_axes.p, axes.data(), axes.size() * sizeof(float), cudaMemcpyHostToDevice));
+  c->placement = placement;
+  c->have_tables = true;
+  return rebuild_blob(c);
+}
+
+int mt_get_alias(const mt_ctx* c, float* prob_dp, uint32_t* alias_dp, float* prob_th, uint32_t* alias_th) {
+  if (!c || !prob_dp || !alias_dp || !prob_th || !alias_th) return MT_ERR_INVALID_ARG;
+  if (!c->have_tables) return MT_ERR_STATE;
+  memcpy(prob_dp, c->prob_dp.data(), c->prob_dp.size() * sizeof(float));
+  memcpy(alias_dp, c->alias_dp.data(), c->alias_dp.size() * sizeof(uint32_t));
+  memcpy(prob_th, c->prob_th.data(), c->prob_th.size() * sizeof(float));
+  memcpy(alias_th, c->alias_th.data(), c->alias_th.size() * sizeof(uint32_t));
+  return MT_OK;
+}
+
+int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
+  if (!c || !gm) return MT_ERR_INVALID_ARG;
+  if (!c->have_tables) return fail(c, MT_ERR_STATE, "mt_set_geometry before mt_build_alias");
+  if (gm->mode != MT_GEOM_REGIONS && gm->mode != MT_GEOM_VOXEL) return fail(c, MT_ERR_INVALID_ARG, "bad geometry mode");
+  if (!(gm->x_min < gm->x_max) || !(gm->y_min < gm->y_max) || !(gm->z_min < gm->z_exit))
+    return fail(c, MT_ERR_INVALID_ARG, "empty world box");
+  if (gm->max_steps < 0 || gm->world_material < 0 || gm->world_material > c->n_materials)
+    return fail(c, MT_ERR_INVALID_ARG, "bad max_steps or world_material");
+  DeviceGuard g(c->device);
+  std::vector<mt_region> regs;
+  if (gm->mode == MT_GEOM_REGIONS) {
+    if (gm->n_regions < 0 || gm->n_regions > 1024) return fail(c, MT_ERR_UNSUPPORTED, "0..1024 regions supported");
+    if (gm->n_regions > 0 && !gm->regions) return fail(c, MT_ERR_INVALID_ARG, "null region array");
+    regs.assign(gm->regions, gm->regions + gm->n_regions);
+    for (size_t j = 0; j < regs.size(); ++j) {
+      const mt_region& r = regs[j];
+      if (!(r.z_lo < r.z_hi) || !(r.x_lo < r.x_hi) || !(r.y_lo < r.y_hi))
+        return fail(c, MT_ERR_INVALID_ARG, "region %zu is empty", j);
+      if (r.material < 0 || r.material > c->n_materials) return fail(c, MT_ERR_INVALID_ARG, "region %zu: bad material", j);
+      if (j > 0 && !(regs[j - 1].z_hi <= r.z_lo))
+        return fail(c, MT_ERR_INVALID_ARG, "regions must be sorted by z_lo and disjoint in z (region %zu)", j);
+    }
+  } else {
+    if (gm->nx < 1 || gm->ny < 1 || gm->nz < 1 || !(gm->cell > 0.0f) || !gm->d_material || !gm->d_field)
+      return fail(c, MT_ERR_INVALID_ARG, "bad voxel grid");
+    const size_t n_cells = (size_t)gm->nx * gm->ny * gm->nz;
+    if (n_cells > ((size_t)1 << 31)) return fail(c, MT_ERR_UNSUPPORTED, "voxel grid above 2^31 cells");
+    MT_CUDA(c, c->d_grid.reserve(n_cells * sizeof(float4)));
+    MT_CUDA(c, c->d_scratch.reserve(4096));
+    MT_CUDA(c, cudaMemset(c->d_scratch.p, 0, sizeof(int)));
+    MT_CUDA(c, mt_launch_repack(gm->d_material, gm->d_field, (float4*)c->d_grid.p, n_cells, (int*)c->d_scratch.p, 0));
+    c->launches += 1;
+    int max_mat = 0;
+    MT_CUDA(c, cudaMemcpy(&max_mat, c->d_scratch.p, sizeof(int), cudaMemcpyDeviceToHost));
+    if (max_mat > c->n_materials) return fail(c, MT_ERR_INVALID_ARG, "voxel grid holds material %d > n_materials", max_mat);
+  }
+  c->geom = *gm;
+  c->geom.regions = nullptr; c->geom.d_material = nullptr; c->geom.d_field = nullptr;
+  c->regions.swap(regs);
+  c->geom.n_regions = (int32_t)c->regions.size();
+  c->have_geom = true;
+  return rebuild_blob(c);
+}
+
+int64_t mt_launch_count(const mt_ctx* c) { return c ? c->launches : 0; }
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// transport
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+void fill_params(const mt_ctx* c, MtParams& P) {
+  memset(&P, 0, sizeof P);
+  const mt_geometry& g = c->geom;
+  P.mode = g.mode;
+  P.x_min = g.x_min; P.x_max = g.x_max; P.y_min = g.y_min; P.y_max = g.y_max; P.z_min = g.z_min; P.z_exit = g.z_exit;
+  P.p_min = g.p_min; P.max_steps = g.max_steps; P.world_material = g.world_material;
+  P.n_regions = g.n_regions;
+  P.nx = g.nx; P.ny = g.ny; P.nz = g.nz; P.ox = g.ox; P.oy = g.oy; P.oz = g.oz;
+  P.inv_cell = (g.mode == MT_GEOM_VOXEL) ? 1.0f / g.cell : 0.0f;          // IEEE float32 division (§3.2)
+  P.grid = (const float4*)c->d_grid.p;
+  P.n_materials = c->n_materials; P.n_pbins = c->n_pbins; P.n_dp = c->n_dp; P.n_th = c->n_th;
+  P.inv_p_lo = 1.0f / c->p_lo;
+  P.bin_scale = (float)((double)c->n_pbins / log2((double)c->p_hi / (double)c->p_lo));
+  P.tab32 = (c->pack == 32) ? (const uint32_t*)c->d_tab.p : nullptr;
+  P.tab64 = (c->pack == 64) ? (const uint2*)c->d_tab.p : nullptr;
+  P.axes = (const float4*)c->d_axes.p;
+  P.blob = (const float*)c->d_blob.p;
+  P.bl = c->bl;
+  P.table_words = (int32_t)(c->table_bytes / 4);
+}
+
+int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                  const mt_muons_out* out, cudaStream_t stream) {
+  if (!c->have_geom) return fail(c, MT_ERR_STATE, "mt_transport before mt_set_geometry");
+  if (n == 0) return MT_OK;
+  if (!in->pos_q || !in->mom || !out->pos_flag || !out->mom_steps) return fail(c, MT_ERR_INVALID_ARG, "null muon buffer");
+  if (n >= ((uint64_t)1 << 32)) return fail(c, MT_ERR_UNSUPPORTED, "at most 2^32 - 1 muons per call");
+  if (out->exit_rec && !out->exit_count) return fail(c, MT_ERR_INVALID_ARG, "exit_rec without exit_count");
+
+  MtParams P;
+  fill_params(c, P);
+  P.n = n; P.id_base = id_base;
+  P.key0 = (uint32_t)seed; P.key1 = (uint32_t)(seed >> 32);
+  P.in_pos_q = (const float4*)in->pos_q; P.in_mom = (const float4*)in->mom;
+  P.out_pos_flag = (float4*)out->pos_flag; P.out_mom_steps = (float4*)out->mom_steps;
+  P.exit_rec = (float4*)out->exit_rec; P.exit_count = out->exit_count; P.exit_capacity = out->exit_capacity;
+  P.counters = (unsigned long long*)out->counters;
+
+  MtLaunchCfg cfg;
+  cfg.pack = c->pack;
+  cfg.block = c->opt_block ? (unsigned)c->opt_block : 256u;
+  const size_t blob_b = ((blob_bytes(c) + 15) & ~(size_t)15);
+  // table placement (north_star subsystem 1): shared memory when blob + tables leave room for >= 2 CTAs/SM
+  const size_t smem_budget = c->smem_optin;
+  bool tab_smem = false;
+  if (c->placement == MT_PLACE_SMEM) {
+    if (blob_b + c->table_bytes > smem_budget) return fail(c, MT_ERR_UNSUPPORTED, "tables (%zu B) do not fit in shared memory", c->table_bytes);
+    tab_smem = true;
+  } else if (c->placement == MT_PLACE_AUTO) {
+    tab_smem = (blob_b + c->table_bytes) * 2 <= smem_budget;
+  }
+  cfg.tab_smem = tab_smem;
+  cfg.smem_bytes = blob_b + (tab_smem ? c->table_bytes : 0) + 16;
+  if (cfg.smem_bytes > smem_budget) return fail(c, MT_ERR_UNSUPPORTED, "region table too large for shared memory");
+
+  int sched = c->opt_sched;
+  if (sched == MT_SCHED_AUTO) sched = (c->geom.mode == MT_GEOM_VOXEL) ? MT_SCHED_WAVEFRONT : MT_SCHED_REFILL;
+  cfg.sched = sched;
+  P.refill_min_idle = c->opt_min_idle ? c->opt_min_idle : 1;
+
+  int occ = 0;
+  MT_CUDA(c, mt_occupancy(P, cfg, &occ));
+  if (occ < 1) return fail(c, MT_ERR_UNSUPPORTED, "kernel does not fit on an SM with %zu B shared memory", cfg.smem_bytes);
+  if (c->opt_blocks_per_sm) occ = std::min(occ, c->opt_blocks_per_sm);
+  const unsigned persistent_grid = (unsigned)(c->sm_count * occ);
+
+  if (sched == MT_SCHED_STATIC) {
+    cfg.grid = (unsigned)((n + cfg.block - 1) / cfg.block);
+    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
+    c->launches += 1;
+    return MT_OK;
+  }
+
+  if (sched == MT_SCHED_REFILL) {
+    MT_CUDA(c, c->d_scratch.reserve(4096));
+    MT_CUDA(c, cudaMemsetAsync(c->d_scratch.p, 0, 8, stream));
+    P.work_counter = (unsigned long long*)c->d_scratch.p;
+    cfg.grid = (unsigned)std::min<uint64_t>(persistent_grid, (n + cfg.block - 1) / cfg.block);
+    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
+    c->launches += 1;
+    return MT_OK;
+  }
+
+  // WAVEFRONT: one pass per z-slab over the compacted list of live muons.  In-flight state lives in the
+  // output arrays (4th component: charge instead of flag until the muon terminates).
+  const float slab = (c->opt_slab_cells ? (float)c->opt_slab_cells : 32.0f) * 0.01f;
+  const double span = (double)c->geom.z_exit - (double)c->geom.z_min;
+  int n_pass = (int)ceil(span / (double)slab);
+  n_pass = std::max(1, std::min(n_pass, 4096));
+  // scratch: [n_pass + 1] work counters (u64) then [n_pass + 1] live counts (u32)
+  const size_t scratch_b = (size_t)(n_pass + 1) * 12 + 64;
+  MT_CUDA(c, c->d_scratch.reserve(std::max<size_t>(scratch_b, 4096)));
+  MT_CUDA(c, cudaMemsetAsync(c->d_scratch.p, 0, scratch_b, stream));
+  unsigned long long* work = (unsigned long long*)c->d_scratch.p;
+  uint32_t* counts = (uint32_t*)(work + n_pass + 1);
+  MT_CUDA(c, c->d_live[0].reserve(n * sizeof(uint32_t)));
+  MT_CUDA(c, c->d_live[1].reserve(n * sizeof(uint32_t)));
+  cfg.grid = (unsigned)std::min<uint64_t>(persistent_grid, (n + cfg.block - 1) / cfg.block);
+  for (int s = 0; s < n_pass; ++s) {
+    P.first_pass = (s == 0);
+    P.live_in = (s == 0) ? nullptr : (const uint32_t*)c->d_live[(s + 1) & 1].p;
+    P.live_in_count = (s == 0) ? nullptr : counts + s;
+    P.live_out = (uint32_t*)c->d_live[s & 1].p;
+    P.live_out_count = counts + s + 1;
+    P.work_counter = work + s;
+    P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * (double)slab);
+    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
+    c->launches += 1;
+  }
+  return MT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mt_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                 const mt_muons_out* out, void* cuda_stream) {
+  if (!c || !in || !out) return MT_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  return run_transport(c, in, n, id_base, seed, out, (cudaStream_t)cuda_stream);
+}
+
+int mt_transport_host(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                      const mt_muons_out* out, void* cuda_stream) {
+  if (!c || !in || !out) return MT_ERR_INVALID_ARG;
+  if (n == 0) return MT_OK;
+  if (!in->pos_q || !in->mom || !out->pos_flag || !out->mom_steps) return fail(c, MT_ERR_INVALID_ARG, "null muon buffer");
+  DeviceGuard g(c->device);
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  const size_t rec = n * 4 * sizeof(float);
+  MT_CUDA(c, c->d_stage_in.reserve(2 * rec));
+  MT_CUDA(c, c->d_stage_out.reserve(2 * rec));
+  const size_t exit_b = out->exit_rec ? (size_t)out->exit_capacity * 8 * sizeof(float) : 0;
+  MT_CUDA(c, c->d_stage_misc.reserve(exit_b + 128));
+  char* d_in = (char*)c->d_stage_in.p;
+  char* d_out = (char*)c->d_stage_out.p;
+  char* d_misc = (char*)c->d_stage_misc.p;
+  MT_CUDA(c, cudaMemcpyAsync(d_in, in->pos_q, rec, cudaMemcpyHostToDevice, stream));
+  MT_CUDA(c, cudaMemcpyAsync(d_in + rec, in->mom, rec, cudaMemcpyHostToDevice, stream));
+  MT_CUDA(c, cudaMemsetAsync(d_misc, 0, 128, stream));
+  mt_muons_in din = {(const float*)d_in, (const float*)(d_in + rec)};
+  mt_muons_out dout;
+  memset(&dout, 0, sizeof dout);
+  dout.pos_flag = (float*)d_out;
+  dout.mom_steps = (float*)(d_out + rec);
+  dout.counters = out->counters ? (uint64_t*)d_misc : nullptr;            // 8 x u64 at offset 0
+  if (out->exit_rec) {
+    if (!out->exit_count) return fail(c, MT_ERR_INVALID_ARG, "exit_rec without exit_count");
+    dout.exit_count = (uint32_t*)(d_misc + 64);
+    dout.exit_rec = (float*)(d_misc + 128);
+    dout.exit_capacity = out->exit_capacity;
+  }
+  const int rc = run_transport(c, &din, n, id_base, seed, &dout, stream);
+  if (rc != MT_OK) return rc;
+  MT_CUDA(c, cudaMemcpyAsync(out->pos_flag, d_out, rec, cudaMemcpyDeviceToHost, stream));
+  MT_CUDA(c, cudaMemcpyAsync(out->mom_steps, d_out + rec, rec, cudaMemcpyDeviceToHost, stream));
+  if (out->counters) MT_CUDA(c, cudaMemcpyAsync(out->counters, d_misc, 64, cudaMemcpyDeviceToHost, stream));
+  if (out->exit_rec) {
+    MT_CUDA(c, cudaMemcpyAsync(out->exit_count, d_misc + 64, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
+    MT_CUDA(c, cudaMemcpyAsync(out->exit_rec, d_misc + 128, exit_b, cudaMemcpyDeviceToHost, stream));
+  }
+  MT_CUDA(c, cudaStreamSynchronize(stream));
+  return MT_OK;
+}
+
+int mt_debug_sample(mt_ctx* c, int material, int pbin, int which, const uint32_t* d_words, uint64_t n,
+                    uint32_t* d_cell_out, void* cuda_stream) {
+  if (!c || !d_words || !d_cell_out) return MT_ERR_INVALID_ARG;
+  if (!c->have_tables) return fail(c, MT_ERR_STATE, "mt_debug_sample before mt_build_alias");
+  if (material < 1 || material > c->n_materials || pbin < 0 || pbin >= c->n_pbins || which < 0 || which > 1)
+    return fail(c, MT_ERR_INVALID_ARG, "bad table selector");
+  DeviceGuard g(c->device);
+  const size_t t = (size_t)(material - 1) * c->n_pbins + pbin;
+  const size_t cell = t * (c->n_dp + c->n_th) + (which ? c->n_dp : 0);
+  const char* tab = (const char*)c->d_tab.p + cell * (c->pack == 32 ? 4 : 8);
+  MT_CUDA(c, mt_launch_debug_sample(c->pack, tab, (uint32_t)(which ? c->n_th : c->n_dp), d_words, n, d_cell_out,
+                                    (cudaStream_t)cuda_stream));
+  c->launches += 1;
+  return MT_OK;
+}
+
+int mt_debug_philox(mt_ctx* c, uint64_t seed, uint64_t id_base, uint32_t step, uint64_t n, uint32_t* d_out,
+                    void* cuda_stream) {
+  if (!c || !d_out) return MT_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  MT_CUDA(c, mt_launch_debug_philox((uint32_t)seed, (uint32_t)(seed >> 32), id_base, step, n, d_out,
+                                    (cudaStream_t)cuda_stream));
+  c->launches += 1;
+  return MT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,61 @@
+// mt_params.h — plain structs shared by the host side (mt_lib.cu) and the kernels (mt_kernels.cu).
+// Part of the CUDA path; shares nothing with oracle/.
+#pragma once
+#include <stdint.h>
+
+// Region record as staged in shared memory.  Same field order as mt_region.
+struct MtRegionDev {
+  float z_lo, z_hi, x_lo, x_hi, y_lo, y_hi;
+  int32_t material;
+  float bx, by, bz;
+};
+
+// The "const blob": small read-only arrays every CTA stages into shared memory at start.
+//   [0, n_pbins]                         momentum-bin edges, float32
+//   [off_steps + 4*m .. +2]              h, h/2, h/6 of material m, m = 0..n_materials
+//   [off_zlo  + j]                       z_lo of region j (search array)
+//   [off_regions + 10*j ..]              MtRegionDev j
+struct MtBlobLayout {
+  int32_t off_steps, off_zlo, off_regions, n_words;
+};
+
+struct MtParams {
+  // ---- geometry
+  int32_t mode;
+  float x_min, x_max, y_min, y_max, z_min, z_exit, p_min;
+  int32_t max_steps, world_material, n_regions;
+  int32_t nx, ny, nz;
+  float ox, oy, oz, inv_cell;
+  const float4* grid;            // [nz][ny][nx] {Bx, By, Bz, material as int bits}, library-owned
+  // ---- tables
+  int32_t n_materials, n_pbins, n_dp, n_th;
+  float inv_p_lo, bin_scale;     // bin guess: floor(log2(P * inv_p_lo) * bin_scale), then fixed on the edges
+  const uint32_t* tab32;         // pack32: [material-1][pbin][n_dp + n_th] = threshold24 << 8 | alias8
+  const uint2* tab64;            // pack64: same shape, {threshold (<= 2^24), alias}
+  const float4* axes;            // [material-1][pbin] = {lo_dp, d_dp, lo_th, d_th} (log2)
+  const float* blob;             // const blob (global copy)
+  MtBlobLayout bl;
+  int32_t table_words;           // 32-bit words of the packed tables (for staging into shared memory)
+  // ---- this call
+  uint64_t n, id_base;
+  uint32_t key0, key1;           // Philox key = seed lo, hi
+  const float4* in_pos_q;
+  const float4* in_mom;
+  float4* out_pos_flag;
+  float4* out_mom_steps;
+  float4* exit_rec;
+  uint32_t* exit_count;
+  uint32_t exit_capacity;
+  unsigned long long* counters;  // optional [8]
+  unsigned long long* work_counter;   // refill scheduler
+  int32_t refill_min_idle;
+  // ---- wavefront scheduler (mt_kernels.cu)
+  const uint32_t* live_in;       // indices of live muons entering this pass (nullptr: 0..n-1)
+  uint32_t* live_out;            // indices still alive after this pass
+  const uint32_t* live_in_count; // device count of live_in
+  uint32_t* live_out_count;
+  float4* st_pos_q;              // in-flight state between passes: x, y, z, q
+  float4* st_mom_step;           // px, py, pz, step (int bits)
+  float slab_z_end;              // a pass advances each muon until z >= slab_z_end (or it terminates)
+  int32_t first_pass;            // read from in_pos_q/in_mom instead of st_*
+};

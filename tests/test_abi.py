@@ -1,0 +1,60 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads, and exports every symbol the header
+declares; the binding's structs have the header's layout; without a GPU the product path fails loudly."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "muon_transport.h")
+
+
+def declared_functions():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(mt_[a-z_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(mt):
+    names = declared_functions()
+    assert {"mt_load_histograms", "mt_build_alias", "mt_set_geometry", "mt_transport"} <= set(names)
+    L = ctypes.CDLL(mt.binding.LIB_PATH)
+    for n in names:
+        assert hasattr(L, n), n
+    assert sorted(mt.binding.SYMBOLS) == names
+
+
+def test_struct_layouts_match_the_header(mt):
+    b = mt.binding
+    assert ctypes.sizeof(b.mt_region) == 40
+    assert ctypes.sizeof(b.mt_hist_desc) == 24 + 5 * 8
+    assert b.mt_geometry.regions.offset == 48 and b.mt_geometry.d_material.offset == 88
+    assert ctypes.sizeof(b.mt_geometry) == 104
+    assert ctypes.sizeof(b.mt_muons_in) == 16 and ctypes.sizeof(b.mt_muons_out) == 48
+    assert b.lib().mt_strerror(b.MT_ERR_EMPTY_HIST).decode().startswith("empty")
+
+
+def test_no_cpu_fallback(mt):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("this check is for the CPU box")
+    with pytest.raises(mt.binding.MtError):
+        mt.binding.mt_create(0)
+    with pytest.raises(RuntimeError):
+        mt.binding.MuonTransport(0)
+
+
+def test_product_path_never_touches_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2512_10520_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
+                assert "muon_oracle" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(from|import)\s+paper_2512_10520_b200", text, flags=re.M), f
+            assert "csrc/" not in text.replace("paper_2512_10520_b200/csrc/.", "") or f.endswith(".cpp")
