@@ -1,0 +1,344 @@
+"""bench.py — throughput of the muon-transport hot path (BASELINE.json metric: muon-steps/s and muons/s).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--muons M]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one mt_transport call: the whole hot path over one batch of synthetic
+muons of BASELINE.json configs[3] (10^7 muons, 200x200x3000 voxel field map) — the config north_star's
+roofline target is quoted on.  Rank r transports its own 10^7 muons (ids r*M ..), no collective on the data
+path (weak scaling).  One JSON line on stdout (rank 0); everything else goes to stderr.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# algorithmic thread-operations and gathered bytes per muon-step (contract operations of
+# DESIGN.md §3 counted one each; loads not counted as operations)
+ALG_OPS_PER_STEP = {"voxel": 383, "regions": 308}
+ALG_GATHER_BYTES_PER_STEP = {"voxel": 168, "regions": 40}
+SM_COUNT, LANES_PER_SM = 148, 128          # B200: 4 SMSPs x 32 lanes issue one warp instruction per clock
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu, self.rows, self.proc, self.thread = gpu_index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return self
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) >= 9:
+                self.rows.append(parts)
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"], samples=0)
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=5)
+        sm, mx, reasons, power = [], [], set(), []
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2])); power.append(float(r[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm), power_w_max=max(power) if power else None)
+
+
+# ------------------------------------------------------------------------------------------ workload
+def make_workload(config, n_muons, device, rank):
+    """BASELINE.json configs[config] with this rank's batch of muons (generator batch = rank)."""
+    from paper_2512_10520_b200 import workloads as w
+    t0 = time.time()
+    if config == 3:
+        wl = w.config3(n=8, device=device)                       # histograms + voxel grids (made on the GPU)
+        wl.muons = w.spectrum_muons(3, n_muons, "square", batch=rank)
+    elif config == 2:
+        wl = w.config2(n=8)
+        wl.muons = w.spectrum_muons(2, n_muons, "square", batch=rank)
+    elif config == 1:
+        wl = w.config1(n=8)
+        wl.muons = w.spectrum_muons(1, n_muons, "gauss", batch=rank)
+    else:
+        raise SystemExit("bench.py times configs 1, 2 and 3 (config 0 is the oracle-sized parity case)")
+    log("[bench] rank %d: %s, %d muons generated in %.1f s" % (rank, wl.name, n_muons, time.time() - t0))
+    return wl
+
+
+def oracle_sample(wl, n_muons, id_base, target_seconds, threads=None):
+    """Time the CPU oracle (as it stands) on an id-strided sample of this workload sized to ~target_seconds.
+    Returns (muon-steps/s, muons/s, cores, description, runner) where runner() repeats the sized sample."""
+    import oracle
+    threads = threads or oracle.max_threads()
+    T, G = oracle.OracleTables(wl.hist), oracle.OracleGeometry(wl.geom)
+
+    def run(sel):
+        t0 = time.perf_counter()
+        r = oracle.transport(T, G, wl.muons.pos_q[sel], wl.muons.mom[sel], wl.seed, ids=(id_base + sel).astype(np.uint64),
+                             threads=threads)
+        return time.perf_counter() - t0, int(r["steps"].sum()), len(sel)
+
+    pilot = np.arange(0, n_muons, max(1, n_muons // 2048), dtype=np.int64)[:2048]
+    dt, steps, _ = run(pilot)
+    rate = steps / max(dt, 1e-9)
+    per_muon = steps / max(len(pilot), 1)
+    n_sample = int(min(n_muons, max(len(pilot), target_seconds * rate / max(per_muon, 1.0))))
+    sel = np.arange(0, n_muons, max(1, n_muons // n_sample), dtype=np.int64)[:n_sample]
+    desc = "every %dth muon of the batch (%d muons), float32 contract mode, OpenMP over muons" % (max(1, n_muons // n_sample), len(sel))
+    return threads, desc, (lambda: run(sel))
+
+
+# --------------------------------------------------------------------------------------- reference arm
+def run_reference(args, rank, world):
+    """The CPU oracle on host cores, same config / metric / unit; rank 0 only."""
+    if rank != 0:
+        return
+    import torch
+    dev = "cuda" if torch.cuda.is_available() else "cpu"          # the grid generator may use the GPU; the timed code never does
+    wl = make_workload(args.config, args.muons, dev, 0)
+    cores, desc, runner = oracle_sample(wl, args.muons, 0, args.ref_seconds)
+    for _ in range(args.warmup):
+        runner()
+    t_tot, s_tot, m_tot = 0.0, 0, 0
+    for _ in range(args.steps):
+        dt, s, m = runner()
+        t_tot += dt; s_tot += s; m_tot += m
+    value = s_tot / t_tot
+    line = {
+        "impl": "reference", "metric": "muon_steps_per_s", "value": value, "unit": "muon-steps/s",
+        "muons_per_s": m_tot / t_tot, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": wl.name, "muons_per_step": m_tot // max(args.steps, 1), "sample": desc},
+        "cpu_baseline": {"value": value, "unit": "muon-steps/s", "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": "muon-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------- our arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2512_10520_b200 import binding as b, build as lib_build
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the transport path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if rank == 0:
+        lib_build.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+        dist.barrier()
+    b.lib()
+
+    n = args.muons
+    id_base = rank * n
+    wl = make_workload(args.config, n, dev, rank)
+    mode = "voxel" if wl.geom.mode == 1 else "regions"
+    h = b.MuonTransport(local_rank).setup(wl.hist, wl.geom, args.placement)
+    h.set_option(b.MT_OPT_SCHEDULE, args.sched).set_option(b.MT_OPT_BLOCK_THREADS, args.block)
+    h.set_option(b.MT_OPT_SLAB_CELLS, args.slab).set_option(b.MT_OPT_REFILL_MIN_IDLE, args.min_idle)
+    h.set_option(b.MT_OPT_BLOCKS_PER_SM, args.blocks_per_sm)
+    host_geom = None
+    if rank == 0 and not args.no_cpu_baseline:
+        import copy
+        host_geom = copy.copy(wl.geom)                       # host copies for the oracle, made before the grids are freed
+        if mode == "voxel":
+            host_geom.material, host_geom.field = wl.geom.material.cpu().numpy(), wl.geom.field.cpu().numpy()
+    wl.geom.material = wl.geom.field = None                   # the library repacked them; free 1.5 GB
+    torch.cuda.empty_cache()
+
+    stream = torch.cuda.Stream(device=dev)
+    d_pos, d_mom = torch.from_numpy(wl.muons.pos_q).to(dev), torch.from_numpy(wl.muons.mom).to(dev)
+    out = {"pos_flag": torch.empty((n, 4), dtype=torch.float32, device=dev),
+           "mom_steps": torch.empty((n, 4), dtype=torch.float32, device=dev)}
+    torch.cuda.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident leg: inputs already in HBM; CUDA events on the launching stream around every step
+    def one_step():
+        return h.transport(d_pos, d_mom, wl.seed, id_base=id_base, out=out, stream=stream)
+
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            res = one_step()
+        stream.synchronize()
+        steps_per_call = int(res["counters"][0].item())
+        barrier()
+        sampler = ClockSampler(local_rank).start() if rank == 0 else None
+        launches0 = b.mt_launch_count(h.ctx)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        wall0 = time.perf_counter()
+        for e0, e1 in evs:
+            e0.record(stream)
+            one_step()
+            e1.record(stream)
+        stream.synchronize()
+        barrier()
+        wall = time.perf_counter() - wall0
+        clocks = sampler.stop() if sampler else None
+        launches = b.mt_launch_count(h.ctx) - launches0
+    dev_ms = [e0.elapsed_time(e1) for e0, e1 in evs]
+    t_dev = sum(dev_ms) * 1e-3
+    flags = np.bincount(out["pos_flag"][:, 3].view(torch.int32).cpu().numpy(), minlength=5)[1:5]
+
+    # ---- end-to-end leg: HOST (pinned) buffers through mt_transport_host, copies inside the timed region
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    h_pos, h_mom = pin(wl.muons.pos_q), pin(wl.muons.mom)
+    h_out = {"pos_flag": torch.empty((n, 4), dtype=torch.float32).pin_memory(),
+             "mom_steps": torch.empty((n, 4), dtype=torch.float32).pin_memory()}
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    h.transport_host(h_pos, h_mom, wl.seed, id_base=id_base, out=h_out, stream=stream)      # warm-up: staging buffers
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        r = h.transport_host(h_pos, h_mom, wl.seed, id_base=id_base, out=h_out, stream=stream)
+    barrier()
+    t_e2e = time.perf_counter() - t0
+    assert int(r["counters"][0]) == steps_per_call
+    h2d = h_pos.numel() * 4 + h_mom.numel() * 4
+    d2h = h_out["pos_flag"].numel() * 4 + h_out["mom_steps"].numel() * 4 + 64
+
+    # ---- max over ranks, totals over ranks
+    t = torch.tensor([t_dev, t_e2e, wall], dtype=torch.float64, device=dev)
+    tot = torch.tensor([steps_per_call, n], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    t_dev_max, t_e2e_max, wall_max = t.tolist()
+    steps_all, muons_all = tot.tolist()
+    h.close()
+    if rank != 0:
+        return
+
+    peaks = load_peaks()
+    value = steps_all * args.steps / t_dev_max
+    e2e_value = steps_all * e2e_steps / t_e2e_max
+    # roofline of the dominant kernel (transport_kernel), this rank: algorithmic thread-operations per launch /
+    # CUDA-event duration per launch, against the FP32 issue peak 148 SMs x 128 lanes x max SM clock
+    launches_per_step = max(1, launches // args.steps)
+    alu_peak = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12                  # T thread-ops/s
+    achieved = steps_per_call * ALG_OPS_PER_STEP[mode] * args.steps / t_dev / 1e12
+    gather_tbs = steps_per_call * ALG_GATHER_BYTES_PER_STEP[mode] * args.steps / t_dev / 1e12
+    line = {
+        "metric": "muon_steps_per_s", "value": value, "unit": "muon-steps/s",
+        "muons_per_s": muons_all * args.steps / t_dev_max,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_dev_max / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": wl.name, "muons_per_gpu": n, "muon_steps_per_gpu_step": steps_per_call,
+                   "schedule": args.sched, "placement": args.placement, "block": args.block, "slab_cells": args.slab,
+                   "parallelism": "id-range sharding x%d, replicated tables and grids, no collective" % world,
+                   "l2": "inputs larger than L2 (320 MB muon state, 1.9 GB field grid per step)",
+                   "flags_rank0": {"stopped": int(flags[0]), "exited": int(flags[1]), "escaped": int(flags[2]),
+                                   "maxsteps": int(flags[3])}},
+        "e2e": {"value": e2e_value, "unit": "muon-steps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "ms_per_step": 1e3 * t_e2e_max / e2e_steps},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "T thread-ops/s",
+                     "frac": achieved / alu_peak, "traffic": None,
+                     "kernel": "transport_kernel (%d launches per step)" % launches_per_step,
+                     "ops_per_muon_step": ALG_OPS_PER_STEP[mode], "peak_source": "148 SM x 128 lanes x %s sm_max_mhz"
+                     % peaks["source"], "gather_tb_per_s": gather_tbs,
+                     "gather_bytes_per_muon_step": ALG_GATHER_BYTES_PER_STEP[mode],
+                     "hbm_gbs_%s" % peaks["source"]: peaks["hbm_gbs"]},
+        "wall_ms_per_step": 1e3 * wall_max / args.steps,
+        "dev_ms_steps": [round(x, 3) for x in dev_ms],
+    }
+    if host_geom is not None:
+        wl.geom = host_geom
+        cores, desc, runner = oracle_sample(wl, n, id_base, args.ref_seconds)
+        dt, s, m = runner()
+        line["cpu_baseline"] = {"value": s / dt, "unit": "muon-steps/s", "cores": cores, "kind": "oracle",
+                                "sample": desc, "muons_per_s": m / dt, "seconds": dt}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--muons", type=int, default=10_000_000, help="muons per GPU per step")
+    ap.add_argument("--sched", type=int, default=0, help="MT_SCHED_* (0 = library default)")
+    ap.add_argument("--placement", type=int, default=0, help="MT_PLACE_* (0 = auto)")
+    ap.add_argument("--block", type=int, default=0)
+    ap.add_argument("--blocks-per-sm", type=int, default=0)
+    ap.add_argument("--slab", type=int, default=0)
+    ap.add_argument("--min-idle", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--ref-seconds", type=float, default=15.0, help="CPU work per oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 1:
+        args.warmup = 1
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
