@@ -1,12 +1,13 @@
 // mt_kernels.cu — the transport kernels and their launchers (sm_100a).
 //
-// One kernel template runs Algorithm 1 under three schedules:
+// Algorithm 1 runs under three schedules; the per-step arithmetic is
+// mt_step.cuh and results do not depend on the schedule:
 //   STATIC     one lane per muon for its whole life (the paper's own mapping, L59, L174);
 //   REFILL     persistent warps; lanes whose muon has terminated take new muons from a global counter;
-//   WAVEFRONT  like REFILL, but over a compacted list of live muons and only until each muon leaves the
-//              current z-slab; the caller launches one pass per slab, so every resident muon reads the same
-//              few z-layers of the field grid (L2/L1-resident) instead of the whole 1.9 GB grid.
-// The per-step arithmetic is mt_step.cuh; results do not depend on the schedule.
+//   WAVEFRONT  one pass per z-slab over the live muons, which are re-sorted by xy cell between passes
+//              (counting sort: wave_bin / wave_scan / wave_scatter).  A warp then holds 32 muons of the same
+//              cell column at the same z, so its eight field-corner gathers fall into one or two cache lines
+//              instead of 32, and the slab's few z-layers of the 1.9 GB grid stay L1/L2-resident.
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "mt_launch.h"
@@ -17,7 +18,7 @@ namespace {
 using namespace mt;
 
 enum { SCHED_STATIC = 1, SCHED_REFILL = 2, SCHED_WAVEFRONT = 3 };
-constexpr int kInnerSteps = 8;        // steps between two refill checks
+constexpr int kInnerSteps = 8;        // REFILL: steps between two refill checks
 constexpr unsigned kFull = 0xFFFFFFFFu;
 
 extern __shared__ __align__(16) unsigned char mt_smem[];
@@ -44,16 +45,63 @@ MT_DEV View<PACK> stage_view(const MtParams& P) {
   return V;
 }
 
+// per-lane tallies of a call, reduced per warp and added to the caller's counters at kernel end
+struct Tally {
+  unsigned long long steps = 0;
+  unsigned f1 = 0, f2 = 0, f3 = 0, f4 = 0;
+  MT_DEV void count(int flag) { f1 += (flag == 1); f2 += (flag == 2); f3 += (flag == 3); f4 += (flag == 4); }
+  MT_DEV void flush(unsigned long long* counters, unsigned lane) {
+    if (!counters) return;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) steps += __shfl_xor_sync(kFull, steps, o);
+    f1 = __reduce_add_sync(kFull, f1); f2 = __reduce_add_sync(kFull, f2);
+    f3 = __reduce_add_sync(kFull, f3); f4 = __reduce_add_sync(kFull, f4);
+    if (lane == 0) {
+      if (steps) atomicAdd(counters + 0, steps);
+      if (f1) atomicAdd(counters + 1, (unsigned long long)f1);
+      if (f2) atomicAdd(counters + 2, (unsigned long long)f2);
+      if (f3) atomicAdd(counters + 3, (unsigned long long)f3);
+      if (f4) atomicAdd(counters + 4, (unsigned long long)f4);
+    }
+  }
+};
+
+// final state of a terminated muon -> dense outputs; exit-plane hits also go to the compact list through one
+// atomic per warp (north_star subsystem 6).  Called by all 32 lanes; `flag` is 0 on lanes with nothing to write.
+MT_DEV void write_final(const MtParams& P, const Muon& m, uint32_t idx, int flag, unsigned lane) {
+  if (flag) {
+    P.out_pos_flag[idx] = make_float4(m.x, m.y, m.z, __int_as_float(flag));
+    P.out_mom_steps[idx] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
+  }
+  if (P.exit_rec) {
+    const bool ex = (flag == 2);
+    const unsigned em = __ballot_sync(kFull, ex);
+    if (em) {
+      const int leader = __ffs(em) - 1;
+      unsigned base = 0;
+      if ((int)lane == leader) base = atomicAdd(P.exit_count, (unsigned)__popc(em));
+      base = __shfl_sync(kFull, base, leader);
+      if (ex) {
+        const unsigned slot = base + (unsigned)__popc(em & ((1u << lane) - 1u));
+        if (slot < P.exit_capacity) {
+          P.exit_rec[2 * (size_t)slot] = make_float4(m.x, m.y, m.z, __uint_as_float(idx));
+          P.exit_rec[2 * (size_t)slot + 1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// STATIC and REFILL
+// ------------------------------------------------------------------------------------------------
 template <int GEOM, int PACK, bool TAB_SMEM, int SCHED>
 __global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
 transport_kernel(const __grid_constant__ MtParams P) {
   const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt_mask = (1u << lane) - 1u;
-
-  // number of work items: muons (STATIC/REFILL) or live-list entries (WAVEFRONT)
-  uint64_t n_items = P.n;
-  if (SCHED == SCHED_WAVEFRONT && P.live_in_count) n_items = *P.live_in_count;
+  const uint64_t n_items = P.n;
 
   Muon m;
   m.x = m.y = m.z = m.q = m.px = m.py = m.pz = 0.0f;
@@ -61,25 +109,12 @@ transport_kernel(const __grid_constant__ MtParams P) {
   uint32_t idx = 0;              // muon index within this call
   bool active = false;
   bool exhausted = false;        // warp-uniform: the work counter has run past n_items
-  unsigned long long acc_steps = 0;
-  unsigned acc_f1 = 0, acc_f2 = 0, acc_f3 = 0, acc_f4 = 0;     // muons terminated per flag by this lane
+  Tally tally;
 
   auto load = [&](uint64_t item) {
-    if (SCHED == SCHED_WAVEFRONT) {
-      idx = P.live_in ? P.live_in[item] : (uint32_t)item;
-      if (P.first_pass) {
-        const float4 a = __ldg(P.in_pos_q + idx), b = __ldg(P.in_mom + idx);
-        m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z; m.step = 0;
-      } else {
-        const float4 a = P.out_pos_flag[idx], b = P.out_mom_steps[idx];
-        m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z;
-        m.step = __float_as_int(b.w);
-      }
-    } else {
-      idx = (uint32_t)item;
-      const float4 a = __ldg(P.in_pos_q + idx), b = __ldg(P.in_mom + idx);
-      m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z; m.step = 0;
-    }
+    idx = (uint32_t)item;
+    const float4 a = __ldg(P.in_pos_q + idx), b = __ldg(P.in_mom + idx);
+    m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z; m.step = 0;
     active = true;
   };
 
@@ -114,80 +149,180 @@ transport_kernel(const __grid_constant__ MtParams P) {
 #pragma unroll 1
     for (int k = 0; k < kInnerSteps; ++k) {
       int flag = 0;
-      // WAVEFRONT: a live muon at or beyond the end of the slab waits for the next pass
-      const bool parked = (SCHED == SCHED_WAVEFRONT) && active && m.z >= P.slab_z_end;
-      if (active && !parked) {
+      if (active) {
         const uint64_t id = P.id_base + idx;
-        flag = step_once<GEOM, PACK, !TAB_SMEM>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
-        if (flag == 0) acc_steps += 1;
+        flag = step_once<GEOM, PACK, !TAB_SMEM, false>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
+        if (flag == 0) tally.steps += 1;
       }
-      // exit-plane records through one atomic per warp (north_star subsystem 6)
-      if (P.exit_rec) {
-        const bool ex = (flag == 2);
-        const unsigned em = __ballot_sync(kFull, ex);
-        if (em) {
-          const int leader = __ffs(em) - 1;
-          unsigned base = 0;
-          if ((int)lane == leader) base = atomicAdd(P.exit_count, (unsigned)__popc(em));
-          base = __shfl_sync(kFull, base, leader);
-          if (ex) {
-            const unsigned slot = base + (unsigned)__popc(em & lt_mask);
-            if (slot < P.exit_capacity) {
-              P.exit_rec[2 * (size_t)slot] = make_float4(m.x, m.y, m.z, __uint_as_float(idx));
-              P.exit_rec[2 * (size_t)slot + 1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
-            }
-          }
-        }
-      }
+      write_final(P, m, idx, flag, lane);
       if (flag) {
-        P.out_pos_flag[idx] = make_float4(m.x, m.y, m.z, __int_as_float(flag));
-        P.out_mom_steps[idx] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
-        acc_f1 += (flag == 1); acc_f2 += (flag == 2); acc_f3 += (flag == 3); acc_f4 += (flag == 4);
+        tally.count(flag);
         active = false;
-      }
-      if (SCHED == SCHED_WAVEFRONT) {
-        const unsigned pm = __ballot_sync(kFull, parked);
-        if (pm) {
-          const int leader = __ffs(pm) - 1;
-          unsigned base = 0;
-          if ((int)lane == leader) base = atomicAdd(P.live_out_count, (unsigned)__popc(pm));
-          base = __shfl_sync(kFull, base, leader);
-          if (parked) {
-            P.live_out[base + (unsigned)__popc(pm & lt_mask)] = idx;
-            P.out_pos_flag[idx] = make_float4(m.x, m.y, m.z, m.q);
-            P.out_mom_steps[idx] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
-            active = false;
-          }
-        }
       }
       if (!__any_sync(kFull, active)) break;
     }
     if (SCHED == SCHED_STATIC && !__any_sync(kFull, active)) break;
   }
+  tally.flush(P.counters, lane);
+}
 
-  // ---- per-call counters: total steps and muons per flag
-  if (P.counters) {
+// ------------------------------------------------------------------------------------------------
+// WAVEFRONT: sorted z-slab passes
+// ------------------------------------------------------------------------------------------------
+MT_DEV uint32_t sort_key(const MtParams& P, float x, float y) {
+  // any mapping works (the order never changes results); NaN and far-away positions land in a border cell
+  const float fx = fminf(fmaxf((x - P.key_x0) * P.key_inv, 0.0f), (float)(P.key_nx - 1));
+  const float fy = fminf(fmaxf((y - P.key_y0) * P.key_inv, 0.0f), (float)(P.key_ny - 1));
+  return (uint32_t)((int)fy * P.key_nx + (int)fx);
+}
+
+// pass "-1": key and rank of every input muon (the state itself is read by wave_scatter from the caller's arrays)
+__global__ void __launch_bounds__(256) wave_bin_kernel(const __grid_constant__ MtParams P) {
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += stride) {
+    const float4 a = __ldg(P.in_pos_q + i);
+    const uint32_t key = sort_key(P, a.x, a.y);
+    const uint32_t rank = atomicAdd(P.hist + key, 1u);
+    P.u_key[i] = make_uint4((uint32_t)i, key, rank, 0u);
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) *P.live_out_count = (uint32_t)P.n;
+}
+
+// exclusive scan of the key histogram (one CTA; n_keys <= 2^20), which it zeroes for the next pass
+__global__ void __launch_bounds__(1024) wave_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ offset,
+                                                         int n_keys) {
+  __shared__ uint32_t warp_sum[32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int per = (n_keys + 1023) / 1024;
+  const int k0 = min(tid * per, n_keys), k1 = min(k0 + per, n_keys);
+  uint32_t sum = 0;
+  for (int k = k0; k < k1; ++k) sum += hist[k];
+  uint32_t inc = sum;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc_steps += __shfl_xor_sync(kFull, acc_steps, o);
-    acc_f1 = __reduce_add_sync(kFull, acc_f1); acc_f2 = __reduce_add_sync(kFull, acc_f2);
-    acc_f3 = __reduce_add_sync(kFull, acc_f3); acc_f4 = __reduce_add_sync(kFull, acc_f4);
-    if (lane == 0) {
-      if (acc_steps) atomicAdd(P.counters + 0, acc_steps);
-      if (acc_f1) atomicAdd(P.counters + 1, (unsigned long long)acc_f1);
-      if (acc_f2) atomicAdd(P.counters + 2, (unsigned long long)acc_f2);
-      if (acc_f3) atomicAdd(P.counters + 3, (unsigned long long)acc_f3);
-      if (acc_f4) atomicAdd(P.counters + 4, (unsigned long long)acc_f4);
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t v = __shfl_up_sync(kFull, inc, o);
+    if (lane >= o) inc += v;
+  }
+  if (lane == 31) warp_sum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t w = warp_sum[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t v = __shfl_up_sync(kFull, w, o);
+      if (lane >= o) w += v;
     }
+    warp_sum[lane] = w;
+  }
+  __syncthreads();
+  uint32_t run = inc - sum + (wid ? warp_sum[wid - 1] : 0u);
+  for (int k = k0; k < k1; ++k) {
+    const uint32_t v = hist[k];
+    offset[k] = run;
+    run += v;
+    hist[k] = 0u;
   }
 }
 
-// ---- voxel repack: {material u8, field f32x3} -> one float4 per cell; also reports the largest material id
+// parked list (arrival order) -> sorted list; `first` reads the caller's input arrays (whose mom.w is unused)
+__global__ void __launch_bounds__(256) wave_scatter_kernel(const __grid_constant__ MtParams P, const float4* __restrict__ src_a,
+                                                           const float4* __restrict__ src_b, int first) {
+  const uint32_t n = *P.live_out_count;
+  const uint32_t stride = gridDim.x * blockDim.x;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const uint4 k = P.u_key[i];
+    const uint32_t dst = P.key_offset[k.y] + k.z;
+    const float4 a = src_a[i];
+    float4 b = src_b[i];
+    if (first) b.w = __int_as_float(0);
+    P.s_pos_q[dst] = a;
+    P.s_mom_step[dst] = b;
+    P.s_idx[dst] = k.x;
+  }
+}
+
+template <int GEOM, int PACK, bool TAB_SMEM>
+__global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
+wave_transport_kernel(const __grid_constant__ MtParams P) {
+  const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const uint32_t n_items = *P.live_in_count;
+  Tally tally;
+
+  for (;;) {
+    // ---- the warp takes the next 32 muons of the sorted list
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(P.work_counter, 32ull);
+    base = __shfl_sync(kFull, base, 0);
+    if (base >= n_items) break;
+    const uint32_t item = (uint32_t)base + lane;
+    Muon m;
+    uint32_t idx = 0;
+    int flag = -1;                                    // -1: no muon on this lane
+    m.x = m.y = m.z = m.q = m.px = m.py = m.pz = 0.0f;
+    m.step = 0;
+    if (item < n_items) {
+      const float4 a = P.s_pos_q[item], b = P.s_mom_step[item];
+      idx = P.s_idx[item];
+      m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z;
+      m.step = __float_as_int(b.w);
+      flag = 0;
+    }
+    const uint64_t id = P.id_base + idx;
+    const uint32_t id_lo = (uint32_t)id, id_hi = (uint32_t)(id >> 32);
+
+    // ---- step until every lane has terminated or reached the end of the slab
+    for (;;) {
+      if (flag == 0) {
+        flag = step_once<GEOM, PACK, !TAB_SMEM, true>(P, V, m, id_lo, id_hi, P.slab_z_end);
+        if (flag == 0) tally.steps += 1;
+      }
+      if (!__any_sync(kFull, flag == 0)) break;
+    }
+
+    // ---- terminated muons: final state; parked muons: state, sort key and rank for the next pass
+    const int fin = (flag >= 1 && flag <= 4) ? flag : 0;
+    write_final(P, m, idx, fin, lane);
+    tally.count(fin);
+    const bool parked = (flag == MT_PARK);
+    const unsigned pm = __ballot_sync(kFull, parked);
+    if (pm) {
+      const int leader = __ffs(pm) - 1;
+      unsigned slot0 = 0;
+      if ((int)lane == leader) slot0 = atomicAdd(P.live_out_count, (unsigned)__popc(pm));
+      slot0 = __shfl_sync(kFull, slot0, leader);
+      if (parked) {
+        const uint32_t key = sort_key(P, m.x, m.y);
+        const unsigned peers = __match_any_sync(pm, key);
+        const int pl = __ffs(peers) - 1;
+        unsigned r0 = 0;
+        if ((int)lane == pl) r0 = atomicAdd(P.hist + key, (unsigned)__popc(peers));
+        r0 = __shfl_sync(peers, r0, pl);
+        const unsigned slot = slot0 + (unsigned)__popc(pm & lt_mask);
+        P.u_pos_q[slot] = make_float4(m.x, m.y, m.z, m.q);
+        P.u_mom_step[slot] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
+        P.u_key[slot] = make_uint4(idx, key, r0 + (unsigned)__popc(peers & lt_mask), 0u);
+      }
+    }
+  }
+  tally.flush(P.counters, lane);
+}
+
+// ---- voxel repack: {material u8, field f32x3} -> one float4 per cell of a grid with a one-cell border that
+// replicates the faces (so the clamped corner indices of DESIGN.md §3.3 need no clamps in the step loop);
+// also reports the largest material id
 __global__ void repack_kernel(const uint8_t* __restrict__ mat, const float* __restrict__ fld, float4* __restrict__ out,
-                              size_t n_cells, int* __restrict__ max_material) {
+                              int nx, int ny, int nz, int* __restrict__ max_material) {
   int local_max = 0;
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_cells; i += (size_t)gridDim.x * blockDim.x) {
-    const int mval = mat[i];
-    out[i] = make_float4(fld[3 * i], fld[3 * i + 1], fld[3 * i + 2], __int_as_float(mval));
+  const int px = nx + 2, py = ny + 2;
+  const size_t n_padded = (size_t)px * py * (nz + 2);
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_padded; i += (size_t)gridDim.x * blockDim.x) {
+    const int x = (int)(i % px), y = (int)((i / px) % py), z = (int)(i / ((size_t)px * py));
+    const int sx = min(max(x - 1, 0), nx - 1), sy = min(max(y - 1, 0), ny - 1), sz = min(max(z - 1, 0), nz - 1);
+    const size_t src = ((size_t)sz * ny + sy) * nx + sx;
+    const int mval = mat[src];
+    out[i] = make_float4(fld[3 * src], fld[3 * src + 1], fld[3 * src + 2], __int_as_float(mval));
     local_max = max(local_max, mval);
   }
   for (int o = 16; o > 0; o >>= 1) local_max = max(local_max, __shfl_xor_sync(kFull, local_max, o));
@@ -218,7 +353,7 @@ kernel_fn pick_sched(int sched) {
   switch (sched) {
     case SCHED_STATIC: return transport_kernel<GEOM, PACK, TAB_SMEM, SCHED_STATIC>;
     case SCHED_REFILL: return transport_kernel<GEOM, PACK, TAB_SMEM, SCHED_REFILL>;
-    default: return transport_kernel<GEOM, PACK, TAB_SMEM, SCHED_WAVEFRONT>;
+    default: return wave_transport_kernel<GEOM, PACK, TAB_SMEM>;
   }
 }
 template <int GEOM>
@@ -249,9 +384,23 @@ cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, (const void*)fn, cfg.block, cfg.smem_bytes);
 }
 
-cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, float4* out, size_t n_cells, int* d_max_material,
-                             cudaStream_t stream) {
-  repack_kernel<<<148 * 8, 256, 0, stream>>>(mat, fld, out, n_cells, d_max_material);
+cudaError_t mt_launch_wave_bin(const MtParams& P, unsigned grid, cudaStream_t stream) {
+  wave_bin_kernel<<<grid, 256, 0, stream>>>(P);
+  return cudaGetLastError();
+}
+
+cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src_a, const float4* src_b, int first,
+                                unsigned grid, cudaStream_t stream) {
+  wave_scan_kernel<<<1, 1024, 0, stream>>>(P.hist, P.key_offset, n_keys);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  wave_scatter_kernel<<<grid, 256, 0, stream>>>(P, src_a, src_b, first);
+  return cudaGetLastError();
+}
+
+cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, float4* out, int nx, int ny, int nz,
+                             int* d_max_material, cudaStream_t stream) {
+  repack_kernel<<<148 * 8, 256, 0, stream>>>(mat, fld, out, nx, ny, nz, d_max_material);
   return cudaGetLastError();
 }
 

@@ -21,8 +21,13 @@ struct MtLaunchCfg {
 
 cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream);
 cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm);
-cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, float4* out, size_t n_cells, int* d_max_material,
-                             cudaStream_t stream);
+// WAVEFRONT helpers: key + rank of the input muons; scan of the key histogram followed by the scatter of the
+// parked list (src_a / src_b) into the sorted list
+cudaError_t mt_launch_wave_bin(const MtParams& P, unsigned grid, cudaStream_t stream);
+cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src_a, const float4* src_b, int first,
+                                unsigned grid, cudaStream_t stream);
+cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, float4* out, int nx, int ny, int nz,
+                             int* d_max_material, cudaStream_t stream);
 cudaError_t mt_launch_debug_sample(int pack, const void* tab, uint32_t N, const uint32_t* words, uint64_t n,
                                    uint32_t* out, cudaStream_t stream);
 cudaError_t mt_launch_debug_philox(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,

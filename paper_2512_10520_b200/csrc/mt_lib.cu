@@ -51,7 +51,7 @@ struct mt_ctx {
   int pack = 32;
   int placement = MT_PLACE_AUTO;
   size_t table_bytes = 0;
-  DevBuf d_tab, d_axes, d_blob, d_grid, d_scratch, d_live[2], d_stage_in, d_stage_out, d_stage_misc;
+  DevBuf d_tab, d_axes, d_blob, d_grid, d_scratch, d_wave, d_stage_in, d_stage_out, d_stage_misc;
   // geometry
   mt_geometry geom{};
   std::vector<mt_region> regions;
@@ -197,7 +197,7 @@ int mt_create(mt_ctx** out, int cuda_device) {
 int mt_destroy(mt_ctx* c) {
   if (!c) return MT_OK;
   DeviceGuard g(c->device);
-  DevBuf* bufs[] = {&c->d_tab, &c->d_axes, &c->d_blob, &c->d_grid, &c->d_scratch, &c->d_live[0], &c->d_live[1],
+  DevBuf* bufs[] = {&c->d_tab, &c->d_axes, &c->d_blob, &c->d_grid, &c->d_scratch, &c->d_wave,
                     &c->d_stage_in, &c->d_stage_out, &c->d_stage_misc};
   for (DevBuf* b : bufs) b->release();
   delete c;
@@ -236,6 +236,16 @@ int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) {
     return fail(c, MT_ERR_UNSUPPORTED, "histogram shape out of range");
   if (!(d->p_lo > 0.0f) || !(d->p_hi > d->p_lo) || isinf(d->p_hi))
     return fail(c, MT_ERR_INVALID_ARG, "need 0 < p_lo < p_hi");
+  // the momentum-bin guess of the kernel (a logarithm, then one comparison against the float32 edges) needs bins
+  // wider than 2^-16 in log2(p); the jitter scale 2^-16 is folded into the axis steps, which must stay normal
+  if ((double)d->n_pbins / log2((double)d->p_hi / (double)d->p_lo) > 65536.0)
+    return fail(c, MT_ERR_UNSUPPORTED, "momentum bins narrower than 2^-16 in log2(p)");
+  for (size_t t = 0; t < (size_t)d->n_materials * d->n_pbins; ++t)
+    for (const float* ax : {d->axis_dp, d->axis_th}) {
+      const float w = ax[2 * t + 1];
+      if (!isfinite(ax[2 * t]) || !isfinite(w) || (w != 0.0f && fabsf(w) < 0x1p-100f))
+        return fail(c, MT_ERR_INVALID_ARG, "axis of table %zu is not finite or its cell width is below 2^-100", t);
+    }
   for (int m = 0; m <= d->n_materials; ++m)
     if (!(d->step_m[m] > 0.0f) || isinf(d->step_m[m])) return fail(c, MT_ERR_INVALID_ARG, "step_m[%d] must be positive", m);
   const size_t nt = (size_t)d->n_materials * d->n_pbins;
@@ -292,8 +302,9 @@ int mt_build_alias(mt_ctx* c, int placement) {
   MT_CUDA(c, cudaMemcpy(c->d_tab.p, packed.data(), c->table_bytes, cudaMemcpyHostToDevice));
   std::vector<float> axes(nt * 4);
   for (size_t t = 0; t < nt; ++t) {
-    axes[4 * t + 0] = c->axis_dp[2 * t]; axes[4 * t + 1] = c->axis_dp[2 * t + 1];
-    axes[4 * t + 2] = c->axis_th[2 * t]; axes[4 * t + 3] = c->axis_th[2 * t + 1];
+    // cell widths carry the jitter's 2^-16 (exact: a power of two; mt_step.cuh decode)
+    axes[4 * t + 0] = c->axis_dp[2 * t]; axes[4 * t + 1] = c->axis_dp[2 * t + 1] * 0x1p-16f;
+    axes[4 * t + 2] = c->axis_th[2 * t]; axes[4 * t + 3] = c->axis_th[2 * t + 1] * 0x1p-16f;
   }
   MT_CUDA(c, c->d_axes.reserve(axes.size() * sizeof(float)));
   MT_CUDA(c, cudaMemcpy(c->d_axes.p, axes.data(), axes.size() * sizeof(float), cudaMemcpyHostToDevice));
@@ -337,12 +348,15 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
   } else {
     if (gm->nx < 1 || gm->ny < 1 || gm->nz < 1 || !(gm->cell > 0.0f) || !gm->d_material || !gm->d_field)
       return fail(c, MT_ERR_INVALID_ARG, "bad voxel grid");
-    const size_t n_cells = (size_t)gm->nx * gm->ny * gm->nz;
-    if (n_cells > ((size_t)1 << 31)) return fail(c, MT_ERR_UNSUPPORTED, "voxel grid above 2^31 cells");
+    if (gm->nx > (1 << 20) || gm->ny > (1 << 20) || gm->nz > (1 << 20))
+      return fail(c, MT_ERR_UNSUPPORTED, "voxel grid above 2^20 cells along an axis");
+    const size_t n_cells = (size_t)(gm->nx + 2) * (gm->ny + 2) * (gm->nz + 2);       // with the replicated border
+    if (n_cells >= ((size_t)1 << 31)) return fail(c, MT_ERR_UNSUPPORTED, "voxel grid above 2^31 cells");
     MT_CUDA(c, c->d_grid.reserve(n_cells * sizeof(float4)));
     MT_CUDA(c, c->d_scratch.reserve(4096));
     MT_CUDA(c, cudaMemset(c->d_scratch.p, 0, sizeof(int)));
-    MT_CUDA(c, mt_launch_repack(gm->d_material, gm->d_field, (float4*)c->d_grid.p, n_cells, (int*)c->d_scratch.p, 0));
+    MT_CUDA(c, mt_launch_repack(gm->d_material, gm->d_field, (float4*)c->d_grid.p, gm->nx, gm->ny, gm->nz,
+                                (int*)c->d_scratch.p, 0));
     c->launches += 1;
     int max_mat = 0;
     MT_CUDA(c, cudaMemcpy(&max_mat, c->d_scratch.p, sizeof(int), cudaMemcpyDeviceToHost));
@@ -375,6 +389,8 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.nx = g.nx; P.ny = g.ny; P.nz = g.nz; P.ox = g.ox; P.oy = g.oy; P.oz = g.oz;
   P.inv_cell = (g.mode == MT_GEOM_VOXEL) ? 1.0f / g.cell : 0.0f;          // IEEE float32 division (§3.2)
   P.grid = (const float4*)c->d_grid.p;
+  P.gsy = g.nx + 2; P.gsz = (g.nx + 2) * (g.ny + 2);
+  P.fnx = (float)g.nx; P.fny = (float)g.ny; P.fnz = (float)g.nz;
   P.n_materials = c->n_materials; P.n_pbins = c->n_pbins; P.n_dp = c->n_dp; P.n_th = c->n_th;
   P.inv_p_lo = 1.0f / c->p_lo;
   P.bin_scale = (float)((double)c->n_pbins / log2((double)c->p_hi / (double)c->p_lo));
@@ -398,6 +414,10 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   fill_params(c, P);
   P.n = n; P.id_base = id_base;
   P.key0 = (uint32_t)seed; P.key1 = (uint32_t)(seed >> 32);
+  for (uint32_t r = 0; r < 10; ++r) {                       // Philox round keys
+    P.rk[2 * r] = P.key0 + r * 0x9E3779B9u;
+    P.rk[2 * r + 1] = P.key1 + r * 0xBB67AE85u;
+  }
   P.in_pos_q = (const float4*)in->pos_q; P.in_mom = (const float4*)in->mom;
   P.out_pos_flag = (float4*)out->pos_flag; P.out_mom_steps = (float4*)out->mom_steps;
   P.exit_rec = (float4*)out->exit_rec; P.exit_count = out->exit_count; P.exit_capacity = out->exit_capacity;
@@ -448,31 +468,59 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
     return MT_OK;
   }
 
-  // WAVEFRONT: one pass per z-slab over the compacted list of live muons.  In-flight state lives in the
-  // output arrays (4th component: charge instead of flag until the muon terminates).
-  const float slab = (c->opt_slab_cells ? (float)c->opt_slab_cells : 32.0f) * 0.01f;
+  // WAVEFRONT: one pass per z-slab; between passes the live muons are counting-sorted by xy cell.
+  const bool voxel = (c->geom.mode == MT_GEOM_VOXEL);
+  const double unit = voxel ? (double)c->geom.cell : 0.01;
+  const double slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : 32.0) * unit;
   const double span = (double)c->geom.z_exit - (double)c->geom.z_min;
-  int n_pass = (int)ceil(span / (double)slab);
-  n_pass = std::max(1, std::min(n_pass, 4096));
-  // scratch: [n_pass + 1] work counters (u64) then [n_pass + 1] live counts (u32)
-  const size_t scratch_b = (size_t)(n_pass + 1) * 12 + 64;
+  const int n_pass = (int)std::max(1.0, std::min(ceil(span / slab), 4096.0));
+  // sort key: the voxel column (coarsened until there are at most 2^18 keys), or a 128 x 128 grid over the world box
+  int key_nx, key_ny;
+  if (voxel) {
+    int coarse = 1;
+    while ((size_t)((c->geom.nx + coarse - 1) / coarse) * ((c->geom.ny + coarse - 1) / coarse) > ((size_t)1 << 18)) coarse *= 2;
+    key_nx = (c->geom.nx + coarse - 1) / coarse; key_ny = (c->geom.ny + coarse - 1) / coarse;
+    P.key_x0 = c->geom.ox; P.key_y0 = c->geom.oy; P.key_inv = 1.0f / (c->geom.cell * (float)coarse);
+  } else {
+    key_nx = key_ny = 128;
+    const float ext = std::max(c->geom.x_max - c->geom.x_min, c->geom.y_max - c->geom.y_min);
+    P.key_x0 = c->geom.x_min; P.key_y0 = c->geom.y_min; P.key_inv = 128.0f / ext;
+  }
+  P.key_nx = key_nx; P.key_ny = key_ny;
+  const int n_keys = key_nx * key_ny;
+  // scratch: [n_pass + 1] work counters (u64), [n_pass + 1] live counts (u32), histogram and offsets [n_keys] (u32)
+  const size_t off_counts = (size_t)(n_pass + 1) * 8, off_hist = (off_counts + (size_t)(n_pass + 1) * 4 + 255) & ~(size_t)255;
+  const size_t zero_b = off_hist + (size_t)n_keys * 4, scratch_b = zero_b + (size_t)n_keys * 4;
   MT_CUDA(c, c->d_scratch.reserve(std::max<size_t>(scratch_b, 4096)));
-  MT_CUDA(c, cudaMemsetAsync(c->d_scratch.p, 0, scratch_b, stream));
+  MT_CUDA(c, cudaMemsetAsync(c->d_scratch.p, 0, zero_b, stream));
   unsigned long long* work = (unsigned long long*)c->d_scratch.p;
-  uint32_t* counts = (uint32_t*)(work + n_pass + 1);
-  MT_CUDA(c, c->d_live[0].reserve(n * sizeof(uint32_t)));
-  MT_CUDA(c, c->d_live[1].reserve(n * sizeof(uint32_t)));
+  uint32_t* counts = (uint32_t*)((char*)c->d_scratch.p + off_counts);
+  P.hist = (uint32_t*)((char*)c->d_scratch.p + off_hist);
+  P.key_offset = P.hist + n_keys;
+  // in-flight state: S (sorted) 36 B and U (parked) 48 B per muon
+  const size_t n16 = ((size_t)n * 16 + 255) & ~(size_t)255, n4 = ((size_t)n * 4 + 255) & ~(size_t)255;
+  MT_CUDA(c, c->d_wave.reserve(5 * n16 + n4));
+  char* w = (char*)c->d_wave.p;
+  P.s_pos_q = (float4*)w; P.s_mom_step = (float4*)(w + n16); P.u_pos_q = (float4*)(w + 2 * n16);
+  P.u_mom_step = (float4*)(w + 3 * n16); P.u_key = (uint4*)(w + 4 * n16); P.s_idx = (uint32_t*)(w + 5 * n16);
+  const unsigned aux_grid = (unsigned)std::min<uint64_t>((uint64_t)c->sm_count * 8, (n + 255) / 256);
   cfg.grid = (unsigned)std::min<uint64_t>(persistent_grid, (n + cfg.block - 1) / cfg.block);
+
+  P.live_out_count = counts;                                   // counts[s] = muons entering pass s
+  MT_CUDA(c, mt_launch_wave_bin(P, aux_grid, stream));
+  MT_CUDA(c, mt_launch_wave_sort(P, n_keys, P.in_pos_q, P.in_mom, 1, aux_grid, stream));
+  c->launches += 3;
   for (int s = 0; s < n_pass; ++s) {
-    P.first_pass = (s == 0);
-    P.live_in = (s == 0) ? nullptr : (const uint32_t*)c->d_live[(s + 1) & 1].p;
-    P.live_in_count = (s == 0) ? nullptr : counts + s;
-    P.live_out = (uint32_t*)c->d_live[s & 1].p;
+    P.live_in_count = counts + s;
     P.live_out_count = counts + s + 1;
     P.work_counter = work + s;
-    P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * (double)slab);
+    P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * slab);
     MT_CUDA(c, mt_launch_transport(P, cfg, stream));
     c->launches += 1;
+    if (s < n_pass - 1) {
+      MT_CUDA(c, mt_launch_wave_sort(P, n_keys, P.u_pos_q, P.u_mom_step, 0, aux_grid, stream));
+      c->launches += 2;
+    }
   }
   return MT_OK;
 }

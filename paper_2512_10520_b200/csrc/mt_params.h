@@ -26,7 +26,10 @@ struct MtParams {
   int32_t max_steps, world_material, n_regions;
   int32_t nx, ny, nz;
   float ox, oy, oz, inv_cell;
-  const float4* grid;            // [nz][ny][nx] {Bx, By, Bz, material as int bits}, library-owned
+  const float4* grid;            // [nz+2][ny+2][nx+2] {Bx, By, Bz, material as int bits}: the caller's grids with a
+                                 // one-cell clamp-replicated border, library-owned
+  int32_t gsy, gsz;              // grid strides in cells: nx+2 and (nx+2)(ny+2)
+  float fnx, fny, fnz;           // (float)nx, ny, nz for the inside test
   // ---- tables
   int32_t n_materials, n_pbins, n_dp, n_th;
   float inv_p_lo, bin_scale;     // bin guess: floor(log2(P * inv_p_lo) * bin_scale), then fixed on the edges
@@ -39,6 +42,7 @@ struct MtParams {
   // ---- this call
   uint64_t n, id_base;
   uint32_t key0, key1;           // Philox key = seed lo, hi
+  uint32_t rk[20];               // the ten round keys (key + r * Weyl), precomputed on the host
   const float4* in_pos_q;
   const float4* in_mom;
   float4* out_pos_flag;
@@ -49,13 +53,19 @@ struct MtParams {
   unsigned long long* counters;  // optional [8]
   unsigned long long* work_counter;   // refill scheduler
   int32_t refill_min_idle;
-  // ---- wavefront scheduler (mt_kernels.cu)
-  const uint32_t* live_in;       // indices of live muons entering this pass (nullptr: 0..n-1)
-  uint32_t* live_out;            // indices still alive after this pass
-  const uint32_t* live_in_count; // device count of live_in
-  uint32_t* live_out_count;
-  float4* st_pos_q;              // in-flight state between passes: x, y, z, q
-  float4* st_mom_step;           // px, py, pz, step (int bits)
+  // ---- wavefront scheduler (mt_kernels.cu): one pass per z-slab.  In-flight muons live in
+  //      library scratch: S = sorted by xy cell (read by a pass), U = parked in arrival order (written by it).
+  const uint32_t* live_in_count; // device count of S
+  uint32_t* live_out_count;      // device count of U (zero on entry)
   float slab_z_end;              // a pass advances each muon until z >= slab_z_end (or it terminates)
-  int32_t first_pass;            // read from in_pos_q/in_mom instead of st_*
+  float4* s_pos_q;               // [live] x, y, z, q
+  float4* s_mom_step;            // [live] px, py, pz, step (int bits)
+  uint32_t* s_idx;               // [live] muon index within the call
+  float4* u_pos_q;
+  float4* u_mom_step;
+  uint4* u_key;                  // [parked] {muon index, sort key, rank within key, -}
+  uint32_t* hist;                // [n_keys] muons parked per sort key (zero on entry; the scan zeroes it again)
+  uint32_t* key_offset;          // [n_keys] exclusive scan of hist
+  float key_x0, key_y0, key_inv; // sort key = iy * key_nx + ix, ix = clamp((int)((x - key_x0) * key_inv), 0, key_nx-1)
+  int32_t key_nx, key_ny;
 };
