@@ -27,12 +27,13 @@ def _nvcc():
     return "nvcc"
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, defines=()) -> str:
+    """`defines`: extra -D macros (e.g. MT_MIN_BLOCKS=4, MT_MAX_THREADS=128) for tuning experiments."""
     deps = [os.path.join(CSRC, d) for d in DEPS] + [os.path.join(INCLUDE, "muon_transport.h"), __file__]
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [_nvcc(), *NVCC_FLAGS, *["-D" + d for d in defines], "-I", INCLUDE, "-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout)
@@ -47,4 +48,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv or any(a.startswith("-D") for a in sys.argv), verbose="--quiet" not in sys.argv,
+                defines=[a[2:] for a in sys.argv if a.startswith("-D")]))

@@ -188,15 +188,25 @@ __global__ void __launch_bounds__(256) wave_bin_kernel(const __grid_constant__ M
   if (blockIdx.x == 0 && threadIdx.x == 0) *P.live_out_count = (uint32_t)P.n;
 }
 
-// exclusive scan of the key histogram (one CTA; n_keys <= 2^20), which it zeroes for the next pass
+// exclusive scan of the key histogram (one CTA; n_keys <= 2^18), which it zeroes for the next pass.  STAGE: the
+// histogram passes through shared memory so that global traffic is coalesced (thread t owns `per` consecutive
+// keys, `per` odd -> conflict-free); otherwise (histograms above the shared-memory size) each thread walks its
+// keys in global memory.
+template <bool STAGE>
 __global__ void __launch_bounds__(1024) wave_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ offset,
                                                          int n_keys) {
   __shared__ uint32_t warp_sum[32];
+  uint32_t* sh = reinterpret_cast<uint32_t*>(mt_smem);
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int per = (n_keys + 1023) / 1024;
+  const int per = ((n_keys + 1023) / 1024) | 1;
   const int k0 = min(tid * per, n_keys), k1 = min(k0 + per, n_keys);
+  if (STAGE) {
+    for (int k = tid; k < n_keys; k += 1024) { sh[k] = hist[k]; hist[k] = 0u; }
+    __syncthreads();
+  }
+  const uint32_t* src = STAGE ? sh : hist;
   uint32_t sum = 0;
-  for (int k = k0; k < k1; ++k) sum += hist[k];
+  for (int k = k0; k < k1; ++k) sum += src[k];
   uint32_t inc = sum;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
@@ -216,11 +226,12 @@ __global__ void __launch_bounds__(1024) wave_scan_kernel(uint32_t* __restrict__ 
   }
   __syncthreads();
   uint32_t run = inc - sum + (wid ? warp_sum[wid - 1] : 0u);
-  for (int k = k0; k < k1; ++k) {
-    const uint32_t v = hist[k];
-    offset[k] = run;
-    run += v;
-    hist[k] = 0u;
+  if (STAGE) {
+    for (int k = k0; k < k1; ++k) { const uint32_t v = sh[k]; sh[k] = run; run += v; }
+    __syncthreads();
+    for (int k = tid; k < n_keys; k += 1024) offset[k] = sh[k];
+  } else {
+    for (int k = k0; k < k1; ++k) { const uint32_t v = hist[k]; offset[k] = run; run += v; hist[k] = 0u; }
   }
 }
 
@@ -271,15 +282,14 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
     }
     const uint64_t id = P.id_base + idx;
     const uint32_t id_lo = (uint32_t)id, id_hi = (uint32_t)(id >> 32);
+    const int step_in = m.step;
 
     // ---- step until every lane has terminated or reached the end of the slab
     for (;;) {
-      if (flag == 0) {
-        flag = step_once<GEOM, PACK, !TAB_SMEM, true>(P, V, m, id_lo, id_hi, P.slab_z_end);
-        if (flag == 0) tally.steps += 1;
-      }
+      if (flag == 0) flag = step_once<GEOM, PACK, !TAB_SMEM, true>(P, V, m, id_lo, id_hi, P.slab_z_end);
       if (!__any_sync(kFull, flag == 0)) break;
     }
+    tally.steps += (unsigned)(m.step - step_in);
 
     // ---- terminated muons: final state; parked muons: state, sort key and rank for the next pass
     const int fin = (flag >= 1 && flag <= 4) ? flag : 0;
@@ -333,7 +343,7 @@ template <int PACK>
 __global__ void debug_sample_kernel(const typename Tab<PACK>::cell_t* tab, uint32_t N, const uint32_t* words,
                                     uint64_t n, uint32_t* out) {
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = Tab<PACK>::template draw<true>(tab, N, words[i]);
+  if (i < n) out[i] = Tab<PACK>::template draw<true>(tab, 0u, N, words[i]);
 }
 
 __global__ void debug_philox_kernel(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,
@@ -391,8 +401,16 @@ cudaError_t mt_launch_wave_bin(const MtParams& P, unsigned grid, cudaStream_t st
 
 cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src_a, const float4* src_b, int first,
                                 unsigned grid, cudaStream_t stream) {
-  wave_scan_kernel<<<1, 1024, 0, stream>>>(P.hist, P.key_offset, n_keys);
-  cudaError_t e = cudaGetLastError();
+  const size_t stage_b = (size_t)n_keys * sizeof(uint32_t);
+  cudaError_t e;
+  if (stage_b <= 200 * 1024) {
+    e = cudaFuncSetAttribute((const void*)wave_scan_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage_b);
+    if (e != cudaSuccess) return e;
+    wave_scan_kernel<true><<<1, 1024, stage_b, stream>>>(P.hist, P.key_offset, n_keys);
+  } else {
+    wave_scan_kernel<false><<<1, 1024, 0, stream>>>(P.hist, P.key_offset, n_keys);
+  }
+  e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   wave_scatter_kernel<<<grid, 256, 0, stream>>>(P, src_a, src_b, first);
   return cudaGetLastError();

@@ -234,6 +234,8 @@ int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) {
   if (d->n_materials < 1 || d->n_materials > 255 || d->n_pbins < 1 || d->n_pbins > 4096 || d->n_dp < 1 ||
       d->n_dp > 65536 || d->n_th < 1 || d->n_th > 65536)
     return fail(c, MT_ERR_UNSUPPORTED, "histogram shape out of range");
+  if ((uint64_t)d->n_materials * d->n_pbins * ((uint64_t)d->n_dp + d->n_th) >= ((uint64_t)1 << 31))
+    return fail(c, MT_ERR_UNSUPPORTED, "more than 2^31 table cells");
   if (!(d->p_lo > 0.0f) || !(d->p_hi > d->p_lo) || isinf(d->p_hi))
     return fail(c, MT_ERR_INVALID_ARG, "need 0 < p_lo < p_hi");
   // the momentum-bin guess of the kernel (a logarithm, then one comparison against the float32 edges) needs bins
