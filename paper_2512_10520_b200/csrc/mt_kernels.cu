@@ -25,21 +25,23 @@ extern __shared__ __align__(16) unsigned char mt_smem[];
 
 template <int PACK, bool TAB_SMEM>
 MT_DEV View<PACK> stage_view(const MtParams& P) {
-  // const blob (edges, step lengths, regions) -> shared memory; tables too when they fit
+  // const blob (edges, step lengths, axes, regions) -> shared memory, then the hot prefix of the packed tables
   float* sblob = reinterpret_cast<float*>(mt_smem);
   for (int i = threadIdx.x; i < P.bl.n_words; i += blockDim.x) sblob[i] = __ldg(P.blob + i);
   View<PACK> V;
   V.edges = sblob;
   V.steps = sblob + P.bl.off_steps;
+  V.axes = reinterpret_cast<const float4*>(sblob + P.bl.off_axes);
   V.zlo = sblob + P.bl.off_zlo;
   V.regions = reinterpret_cast<const MtRegionDev*>(sblob + P.bl.off_regions);
   const uint32_t* gtab = (PACK == 32) ? P.tab32 : reinterpret_cast<const uint32_t*>(P.tab64);
+  V.tab = reinterpret_cast<const typename Tab<PACK>::cell_t*>(gtab);
+  uint4* stab = reinterpret_cast<uint4*>(sblob + ((P.bl.n_words + 3) & ~3));
+  V.hot = reinterpret_cast<const typename Tab<PACK>::cell_t*>(stab);
   if (TAB_SMEM) {
-    uint32_t* stab = reinterpret_cast<uint32_t*>(sblob + ((P.bl.n_words + 3) & ~3));
-    for (int i = threadIdx.x; i < P.table_words; i += blockDim.x) stab[i] = __ldg(gtab + i);
-    V.tab = reinterpret_cast<const typename Tab<PACK>::cell_t*>(stab);
-  } else {
-    V.tab = reinterpret_cast<const typename Tab<PACK>::cell_t*>(gtab);
+    const uint32_t n16 = (P.hot_cells * (PACK / 8) + 15u) / 16u;          // the device array is padded to 16 bytes
+    const uint4* src = reinterpret_cast<const uint4*>(gtab);
+    for (uint32_t i = threadIdx.x; i < n16; i += blockDim.x) stab[i] = __ldg(src + i);
   }
   __syncthreads();
   return V;
@@ -151,7 +153,7 @@ transport_kernel(const __grid_constant__ MtParams P) {
       int flag = 0;
       if (active) {
         const uint64_t id = P.id_base + idx;
-        flag = step_once<GEOM, PACK, !TAB_SMEM, false>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
+        flag = step_once<GEOM, PACK, TAB_SMEM, false>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
         if (flag == 0) tally.steps += 1;
       }
       write_final(P, m, idx, flag, lane);
@@ -286,7 +288,7 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
 
     // ---- step until every lane has terminated or reached the end of the slab
     for (;;) {
-      if (flag == 0) flag = step_once<GEOM, PACK, !TAB_SMEM, true>(P, V, m, id_lo, id_hi, P.slab_z_end);
+      if (flag == 0) flag = step_once<GEOM, PACK, TAB_SMEM, true>(P, V, m, id_lo, id_hi, P.slab_z_end);
       if (!__any_sync(kFull, flag == 0)) break;
     }
     tally.steps += (unsigned)(m.step - step_in);
@@ -319,31 +321,44 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
   tally.flush(P.counters, lane);
 }
 
-// ---- voxel repack: {material u8, field f32x3} -> one float4 per cell of a grid with a one-cell border that
-// replicates the faces (so the clamped corner indices of DESIGN.md §3.3 need no clamps in the step loop);
-// also reports the largest material id
-__global__ void repack_kernel(const uint8_t* __restrict__ mat, const float* __restrict__ fld, float4* __restrict__ out,
-                              int nx, int ny, int nz, int* __restrict__ max_material) {
-  int local_max = 0;
+// ---- voxel repack: {material u8, field f32x3} -> one 32-byte record {cell x, cell x+1} per cell of a grid with a
+// one-cell border that replicates the faces (so the clamped corner indices of DESIGN.md §3.3 need no clamps in
+// the step loop and an x-pair of corners is one load); also counts the cells of each material
+__global__ void repack_kernel(const uint8_t* __restrict__ mat, const float* __restrict__ fld, MtCellPair* __restrict__ out,
+                              int nx, int ny, int nz, unsigned long long* __restrict__ material_cells) {
+  __shared__ unsigned hist[256];
+  for (int i = threadIdx.x; i < 256; i += blockDim.x) hist[i] = 0u;
+  __syncthreads();
   const int px = nx + 2, py = ny + 2;
   const size_t n_padded = (size_t)px * py * (nz + 2);
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_padded; i += (size_t)gridDim.x * blockDim.x) {
     const int x = (int)(i % px), y = (int)((i / px) % py), z = (int)(i / ((size_t)px * py));
-    const int sx = min(max(x - 1, 0), nx - 1), sy = min(max(y - 1, 0), ny - 1), sz = min(max(z - 1, 0), nz - 1);
-    const size_t src = ((size_t)sz * ny + sy) * nx + sx;
-    const int mval = mat[src];
-    out[i] = make_float4(fld[3 * src], fld[3 * src + 1], fld[3 * src + 2], __int_as_float(mval));
-    local_max = max(local_max, mval);
+    const int sx = min(max(x - 1, 0), nx - 1), sx1 = min(max(x, 0), nx - 1);
+    const int sy = min(max(y - 1, 0), ny - 1), sz = min(max(z - 1, 0), nz - 1);
+    const size_t row = ((size_t)sz * ny + sy) * nx;
+    const size_t s0 = row + sx, s1 = row + sx1;
+    MtCellPair r;
+    r.a = make_float4(fld[3 * s0], fld[3 * s0 + 1], fld[3 * s0 + 2], __int_as_float((int)mat[s0]));
+    r.b = make_float4(fld[3 * s1], fld[3 * s1 + 1], fld[3 * s1 + 2], __int_as_float((int)mat[s1]));
+    out[i] = r;
+    if (x >= 1 && x <= nx && y >= 1 && y <= ny && z >= 1 && z <= nz) atomicAdd(&hist[mat[s0]], 1u);
   }
-  for (int o = 16; o > 0; o >>= 1) local_max = max(local_max, __shfl_xor_sync(kFull, local_max, o));
-  if ((threadIdx.x & 31) == 0 && local_max > 0) atomicMax(max_material, local_max);
+  __syncthreads();
+  for (int i = threadIdx.x; i < 256; i += blockDim.x)
+    if (hist[i]) atomicAdd(material_cells + i, (unsigned long long)hist[i]);
 }
 
 template <int PACK>
 __global__ void debug_sample_kernel(const typename Tab<PACK>::cell_t* tab, uint32_t N, const uint32_t* words,
                                     uint64_t n, uint32_t* out) {
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = Tab<PACK>::template draw<true>(tab, 0u, N, words[i]);
+  if (i >= n) return;
+  MtParams P;                       // only hot_cells is read: nothing staged here
+  P.hot_cells = 0u;
+  View<PACK> V;
+  V.tab = tab;
+  V.hot = tab;
+  out[i] = draw<PACK, false>(P, V, 0u, N, words[i]);
 }
 
 __global__ void debug_philox_kernel(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,
@@ -416,9 +431,9 @@ cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src
   return cudaGetLastError();
 }
 
-cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, float4* out, int nx, int ny, int nz,
-                             int* d_max_material, cudaStream_t stream) {
-  repack_kernel<<<148 * 8, 256, 0, stream>>>(mat, fld, out, nx, ny, nz, d_max_material);
+cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, MtCellPair* out, int nx, int ny, int nz,
+                             unsigned long long* d_material_cells, cudaStream_t stream) {
+  repack_kernel<<<148 * 8, 256, 0, stream>>>(mat, fld, out, nx, ny, nz, d_material_cells);
   return cudaGetLastError();
 }
 

@@ -5,17 +5,17 @@
 #include "mt_params.h"
 
 #ifndef MT_MAX_THREADS
-#define MT_MAX_THREADS 256      // largest block the transport kernel is compiled for
-#endif
+#define MT_MAX_THREADS 768      // largest block the transport kernels are compiled for: one CTA of 768 threads
+#endif                          // or three of 256 per SM -> at most 85 registers per thread
 #ifndef MT_MIN_BLOCKS
-#define MT_MIN_BLOCKS 3         // -> at most 85 registers per thread
+#define MT_MIN_BLOCKS 1
 #endif
 
 struct MtLaunchCfg {
   unsigned grid, block;
   size_t smem_bytes;
   int pack;        // 32 or 64 (bits per packed alias cell)
-  bool tab_smem;   // tables staged in shared memory
+  bool tab_smem;   // the hot prefix of the tables (P.hot_cells > 0) is staged in shared memory
   int sched;       // MT_SCHED_STATIC / _REFILL / _WAVEFRONT
 };
 
@@ -26,8 +26,9 @@ cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_
 cudaError_t mt_launch_wave_bin(const MtParams& P, unsigned grid, cudaStream_t stream);
 cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src_a, const float4* src_b, int first,
                                 unsigned grid, cudaStream_t stream);
-cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, float4* out, int nx, int ny, int nz,
-                             int* d_max_material, cudaStream_t stream);
+// d_material_cells: [256] counters (zeroed by the caller) of grid cells per material id
+cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, MtCellPair* out, int nx, int ny, int nz,
+                             unsigned long long* d_material_cells, cudaStream_t stream);
 cudaError_t mt_launch_debug_sample(int pack, const void* tab, uint32_t N, const uint32_t* words, uint64_t n,
                                    uint32_t* out, cudaStream_t stream);
 cudaError_t mt_launch_debug_philox(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,

@@ -51,7 +51,9 @@ struct mt_ctx {
   int pack = 32;
   int placement = MT_PLACE_AUTO;
   size_t table_bytes = 0;
-  DevBuf d_tab, d_axes, d_blob, d_grid, d_scratch, d_wave, d_stage_in, d_stage_out, d_stage_misc;
+  std::vector<int> mat_order;        // material ids, most-used first: the order of their blocks in the packed tables
+  std::vector<uint32_t> mat_cell0;   // [n_materials + 1] first cell of material m's block in the packed tables
+  DevBuf d_tab, d_blob, d_grid, d_scratch, d_wave, d_stage_in, d_stage_out, d_stage_misc;
   // geometry
   mt_geometry geom{};
   std::vector<mt_region> regions;
@@ -126,12 +128,14 @@ uint32_t threshold24(float prob) {
 size_t blob_bytes(const mt_ctx* c) { return (size_t)c->bl.n_words * sizeof(float); }
 
 int rebuild_blob(mt_ctx* c) {
-  // [edges][steps x4][z_lo][regions]; see mt_params.h
+  // [edges][steps x4][axes x4][z_lo][regions]; see mt_params.h
   const int n_edges = c->n_pbins + 1;
   const int n_reg = c->have_geom ? (int)c->regions.size() : 0;
+  const int nt = c->n_materials * c->n_pbins;
   MtBlobLayout bl;
   bl.off_steps = (n_edges + 3) & ~3;
-  bl.off_zlo = bl.off_steps + 4 * (c->n_materials + 1);
+  bl.off_axes = bl.off_steps + 4 * (c->n_materials + 1);
+  bl.off_zlo = bl.off_axes + 4 * nt;
   bl.off_regions = (bl.off_zlo + n_reg + 3) & ~3;
   bl.n_words = bl.off_regions + 10 * n_reg;
   std::vector<float> blob((size_t)bl.n_words + 4, 0.0f);
@@ -143,6 +147,14 @@ int rebuild_blob(mt_ctx* c) {
     blob[bl.off_steps + 4 * m + 0] = h;
     blob[bl.off_steps + 4 * m + 1] = h * 0.5f;
     blob[bl.off_steps + 4 * m + 2] = (float)((double)h / 6.0);                           // §3.2
+    const int32_t cell0 = (int32_t)c->mat_cell0[m];
+    memcpy(&blob[bl.off_steps + 4 * m + 3], &cell0, sizeof cell0);
+  }
+  for (int t = 0; t < nt; ++t) {
+    // cell widths carry the jitter's 2^-16 (exact: a power of two; mt_step.cuh decode)
+    float* ax = &blob[bl.off_axes + 4 * t];
+    ax[0] = c->axis_dp[2 * t]; ax[1] = c->axis_dp[2 * t + 1] * 0x1p-16f;
+    ax[2] = c->axis_th[2 * t]; ax[3] = c->axis_th[2 * t + 1] * 0x1p-16f;
   }
   for (int j = 0; j < n_reg; ++j) {
     blob[bl.off_zlo + j] = c->regions[j].z_lo;
@@ -153,6 +165,50 @@ int rebuild_blob(mt_ctx* c) {
   MT_CUDA(c, c->d_blob.reserve(blob.size() * sizeof(float)));
   MT_CUDA(c, cudaMemcpy(c->d_blob.p, blob.data(), blob.size() * sizeof(float), cudaMemcpyHostToDevice));
   return MT_OK;
+}
+
+// Pack the host tables (per (material, pbin): the Dp/p cells followed by the theta cells) with the material
+// blocks in the order c->mat_order, upload them, and record where each block starts.
+int upload_tables(mt_ctx* c) {
+  const int n_dp = c->n_dp, n_th = c->n_th, n_cells = n_dp + n_th;
+  const size_t nt = (size_t)c->n_materials * c->n_pbins;
+  const int wpc = (c->pack == 32) ? 1 : 2;                 // 32-bit words per cell
+  std::vector<uint32_t> packed(nt * n_cells * wpc + 8, 0u);
+  c->mat_cell0.assign(c->n_materials + 1, 0u);
+  size_t block = 0;
+  for (int m : c->mat_order) {
+    c->mat_cell0[m] = (uint32_t)(block * c->n_pbins * n_cells);
+    for (int i = 0; i < c->n_pbins; ++i) {
+      const size_t t = (size_t)(m - 1) * c->n_pbins + i;                        // table in caller order
+      const size_t dst = (block * c->n_pbins + i) * n_cells;                    // first cell in packed order
+      for (int k = 0; k < n_cells; ++k) {
+        const bool is_dp = k < n_dp;
+        const float pr = is_dp ? c->prob_dp[t * n_dp + k] : c->prob_th[t * n_th + (k - n_dp)];
+        uint32_t al = is_dp ? c->alias_dp[t * n_dp + k] : c->alias_th[t * n_th + (k - n_dp)];
+        uint32_t T = threshold24(pr);
+        const uint32_t self = (uint32_t)(is_dp ? k : k - n_dp);
+        if (c->pack == 32) {
+          if (T >= 16777216u) { T = 16777215u; al = self; }     // prob == 1: the alias is never taken
+          packed[dst + k] = (T << 8) | al;
+        } else {
+          packed[2 * (dst + k)] = T;
+          packed[2 * (dst + k) + 1] = al;
+        }
+      }
+    }
+    ++block;
+  }
+  c->table_bytes = nt * n_cells * wpc * sizeof(uint32_t);
+  MT_CUDA(c, c->d_tab.reserve(packed.size() * sizeof(uint32_t)));               // padded: staged in 16-byte units
+  MT_CUDA(c, cudaMemcpy(c->d_tab.p, packed.data(), packed.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+  return MT_OK;
+}
+
+// order the material blocks by weight (cells or volume per material), heaviest first
+void order_materials(mt_ctx* c, const std::vector<double>& weight) {
+  c->mat_order.resize(c->n_materials);
+  for (int m = 1; m <= c->n_materials; ++m) c->mat_order[m - 1] = m;
+  std::stable_sort(c->mat_order.begin(), c->mat_order.end(), [&](int a, int b) { return weight[a] > weight[b]; });
 }
 
 }  // namespace
@@ -197,7 +253,7 @@ int mt_create(mt_ctx** out, int cuda_device) {
 int mt_destroy(mt_ctx* c) {
   if (!c) return MT_OK;
   DeviceGuard g(c->device);
-  DevBuf* bufs[] = {&c->d_tab, &c->d_axes, &c->d_blob, &c->d_grid, &c->d_scratch, &c->d_wave,
+  DevBuf* bufs[] = {&c->d_tab, &c->d_blob, &c->d_grid, &c->d_scratch, &c->d_wave,
                     &c->d_stage_in, &c->d_stage_out, &c->d_stage_misc};
   for (DevBuf* b : bufs) b->release();
   delete c;
@@ -236,6 +292,8 @@ int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) {
     return fail(c, MT_ERR_UNSUPPORTED, "histogram shape out of range");
   if ((uint64_t)d->n_materials * d->n_pbins * ((uint64_t)d->n_dp + d->n_th) >= ((uint64_t)1 << 31))
     return fail(c, MT_ERR_UNSUPPORTED, "more than 2^31 table cells");
+  if ((uint64_t)d->n_materials * d->n_pbins > 4096)        // edges and axes live in shared memory (<= 80 KB)
+    return fail(c, MT_ERR_UNSUPPORTED, "more than 4096 (material, momentum bin) tables");
   if (!(d->p_lo > 0.0f) || !(d->p_hi > d->p_lo) || isinf(d->p_hi))
     return fail(c, MT_ERR_INVALID_ARG, "need 0 < p_lo < p_hi");
   // the momentum-bin guess of the kernel (a logarithm, then one comparison against the float32 edges) needs bins
@@ -269,7 +327,7 @@ int mt_build_alias(mt_ctx* c, int placement) {
   if (placement < MT_PLACE_AUTO || placement > MT_PLACE_L2) return fail(c, MT_ERR_INVALID_ARG, "bad placement");
   DeviceGuard g(c->device);
   const size_t nt = (size_t)c->n_materials * c->n_pbins;
-  const int n_dp = c->n_dp, n_th = c->n_th, n_cells = n_dp + n_th;
+  const int n_dp = c->n_dp, n_th = c->n_th;
   c->prob_dp.assign(nt * n_dp, 0.0f); c->alias_dp.assign(nt * n_dp, 0u);
   c->prob_th.assign(nt * n_th, 0.0f); c->alias_th.assign(nt * n_th, 0u);
   for (size_t t = 0; t < nt; ++t) {
@@ -280,36 +338,10 @@ int mt_build_alias(mt_ctx* c, int placement) {
       return fail(c, MT_ERR_EMPTY_HIST, "theta histogram of material %d, momentum bin %d is empty or invalid",
                   (int)(t / c->n_pbins) + 1, (int)(t % c->n_pbins));
   }
-  // pack: per (material, pbin) the Dp/p cells followed by the theta cells
   c->pack = (std::max(n_dp, n_th) <= 256) ? 32 : 64;
-  std::vector<uint32_t> packed(nt * n_cells * (c->pack == 32 ? 1 : 2));
-  for (size_t t = 0; t < nt; ++t) {
-    for (int k = 0; k < n_cells; ++k) {
-      const bool is_dp = k < n_dp;
-      const float pr = is_dp ? c->prob_dp[t * n_dp + k] : c->prob_th[t * n_th + (k - n_dp)];
-      uint32_t al = is_dp ? c->alias_dp[t * n_dp + k] : c->alias_th[t * n_th + (k - n_dp)];
-      uint32_t T = threshold24(pr);
-      const uint32_t self = (uint32_t)(is_dp ? k : k - n_dp);
-      if (c->pack == 32) {
-        if (T >= 16777216u) { T = 16777215u; al = self; }     // prob == 1: the alias is never taken
-        packed[t * n_cells + k] = (T << 8) | al;
-      } else {
-        packed[2 * (t * n_cells + k)] = T;
-        packed[2 * (t * n_cells + k) + 1] = al;
-      }
-    }
-  }
-  c->table_bytes = packed.size() * sizeof(uint32_t);
-  MT_CUDA(c, c->d_tab.reserve(c->table_bytes));
-  MT_CUDA(c, cudaMemcpy(c->d_tab.p, packed.data(), c->table_bytes, cudaMemcpyHostToDevice));
-  std::vector<float> axes(nt * 4);
-  for (size_t t = 0; t < nt; ++t) {
-    // cell widths carry the jitter's 2^-16 (exact: a power of two; mt_step.cuh decode)
-    axes[4 * t + 0] = c->axis_dp[2 * t]; axes[4 * t + 1] = c->axis_dp[2 * t + 1] * 0x1p-16f;
-    axes[4 * t + 2] = c->axis_th[2 * t]; axes[4 * t + 3] = c->axis_th[2 * t + 1] * 0x1p-16f;
-  }
-  MT_CUDA(c, c->d_axes.reserve(axes.size() * sizeof(float)));
-  MT_CUDA(c, cudaMemcpy(c->d_axes.p, axes.data(), axes.size() * sizeof(float), cudaMemcpyHostToDevice));
+  order_materials(c, std::vector<double>(c->n_materials + 1, 0.0));       // caller order until a geometry says otherwise
+  int rc = upload_tables(c);
+  if (rc != MT_OK) return rc;
   c->placement = placement;
   c->have_tables = true;
   return rebuild_blob(c);
@@ -335,10 +367,12 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
     return fail(c, MT_ERR_INVALID_ARG, "bad max_steps or world_material");
   DeviceGuard g(c->device);
   std::vector<mt_region> regs;
+  std::vector<double> weight(256, 0.0);                     // how much of the geometry each material fills
   if (gm->mode == MT_GEOM_REGIONS) {
     if (gm->n_regions < 0 || gm->n_regions > 1024) return fail(c, MT_ERR_UNSUPPORTED, "0..1024 regions supported");
     if (gm->n_regions > 0 && !gm->regions) return fail(c, MT_ERR_INVALID_ARG, "null region array");
     regs.assign(gm->regions, gm->regions + gm->n_regions);
+    double world = ((double)gm->x_max - gm->x_min) * ((double)gm->y_max - gm->y_min) * ((double)gm->z_exit - gm->z_min);
     for (size_t j = 0; j < regs.size(); ++j) {
       const mt_region& r = regs[j];
       if (!(r.z_lo < r.z_hi) || !(r.x_lo < r.x_hi) || !(r.y_lo < r.y_hi))
@@ -346,7 +380,14 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
       if (r.material < 0 || r.material > c->n_materials) return fail(c, MT_ERR_INVALID_ARG, "region %zu: bad material", j);
       if (j > 0 && !(regs[j - 1].z_hi <= r.z_lo))
         return fail(c, MT_ERR_INVALID_ARG, "regions must be sorted by z_lo and disjoint in z (region %zu)", j);
+      const double dx = std::min(r.x_hi, gm->x_max) - std::max(r.x_lo, gm->x_min);
+      const double dy = std::min(r.y_hi, gm->y_max) - std::max(r.y_lo, gm->y_min);
+      const double dz = std::min(r.z_hi, gm->z_exit) - std::max(r.z_lo, gm->z_min);
+      const double vol = std::max(dx, 0.0) * std::max(dy, 0.0) * std::max(dz, 0.0);
+      weight[r.material] += vol;
+      world -= vol;
     }
+    weight[gm->world_material] += std::max(world, 0.0);
   } else {
     if (gm->nx < 1 || gm->ny < 1 || gm->nz < 1 || !(gm->cell > 0.0f) || !gm->d_material || !gm->d_field)
       return fail(c, MT_ERR_INVALID_ARG, "bad voxel grid");
@@ -354,21 +395,28 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
       return fail(c, MT_ERR_UNSUPPORTED, "voxel grid above 2^20 cells along an axis");
     const size_t n_cells = (size_t)(gm->nx + 2) * (gm->ny + 2) * (gm->nz + 2);       // with the replicated border
     if (n_cells >= ((size_t)1 << 31)) return fail(c, MT_ERR_UNSUPPORTED, "voxel grid above 2^31 cells");
-    MT_CUDA(c, c->d_grid.reserve(n_cells * sizeof(float4)));
+    MT_CUDA(c, c->d_grid.reserve(n_cells * sizeof(MtCellPair)));
     MT_CUDA(c, c->d_scratch.reserve(4096));
-    MT_CUDA(c, cudaMemset(c->d_scratch.p, 0, sizeof(int)));
-    MT_CUDA(c, mt_launch_repack(gm->d_material, gm->d_field, (float4*)c->d_grid.p, gm->nx, gm->ny, gm->nz,
-                                (int*)c->d_scratch.p, 0));
+    MT_CUDA(c, cudaMemset(c->d_scratch.p, 0, 256 * sizeof(unsigned long long)));
+    MT_CUDA(c, mt_launch_repack(gm->d_material, gm->d_field, (MtCellPair*)c->d_grid.p, gm->nx, gm->ny, gm->nz,
+                                (unsigned long long*)c->d_scratch.p, 0));
     c->launches += 1;
-    int max_mat = 0;
-    MT_CUDA(c, cudaMemcpy(&max_mat, c->d_scratch.p, sizeof(int), cudaMemcpyDeviceToHost));
-    if (max_mat > c->n_materials) return fail(c, MT_ERR_INVALID_ARG, "voxel grid holds material %d > n_materials", max_mat);
+    unsigned long long cells[256];
+    MT_CUDA(c, cudaMemcpy(cells, c->d_scratch.p, sizeof cells, cudaMemcpyDeviceToHost));
+    for (int m = 0; m < 256; ++m) {
+      if (cells[m] && m > c->n_materials) return fail(c, MT_ERR_INVALID_ARG, "voxel grid holds material %d > n_materials", m);
+      weight[m] = (double)cells[m];
+    }
   }
   c->geom = *gm;
   c->geom.regions = nullptr; c->geom.d_material = nullptr; c->geom.d_field = nullptr;
   c->regions.swap(regs);
   c->geom.n_regions = (int32_t)c->regions.size();
   c->have_geom = true;
+  // the most-used materials come first in the packed tables, so that a shared-memory prefix holds them
+  order_materials(c, weight);
+  const int rc = upload_tables(c);
+  if (rc != MT_OK) return rc;
   return rebuild_blob(c);
 }
 
@@ -390,7 +438,7 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.n_regions = g.n_regions;
   P.nx = g.nx; P.ny = g.ny; P.nz = g.nz; P.ox = g.ox; P.oy = g.oy; P.oz = g.oz;
   P.inv_cell = (g.mode == MT_GEOM_VOXEL) ? 1.0f / g.cell : 0.0f;          // IEEE float32 division (§3.2)
-  P.grid = (const float4*)c->d_grid.p;
+  P.grid = (const MtCellPair*)c->d_grid.p;
   P.gsy = g.nx + 2; P.gsz = (g.nx + 2) * (g.ny + 2);
   P.fnx = (float)g.nx; P.fny = (float)g.ny; P.fnz = (float)g.nz;
   P.n_materials = c->n_materials; P.n_pbins = c->n_pbins; P.n_dp = c->n_dp; P.n_th = c->n_th;
@@ -398,10 +446,8 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.bin_scale = (float)((double)c->n_pbins / log2((double)c->p_hi / (double)c->p_lo));
   P.tab32 = (c->pack == 32) ? (const uint32_t*)c->d_tab.p : nullptr;
   P.tab64 = (c->pack == 64) ? (const uint2*)c->d_tab.p : nullptr;
-  P.axes = (const float4*)c->d_axes.p;
   P.blob = (const float*)c->d_blob.p;
   P.bl = c->bl;
-  P.table_words = (int32_t)(c->table_bytes / 4);
 }
 
 int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
@@ -425,32 +471,49 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   P.exit_rec = (float4*)out->exit_rec; P.exit_count = out->exit_count; P.exit_capacity = out->exit_capacity;
   P.counters = (unsigned long long*)out->counters;
 
-  MtLaunchCfg cfg;
-  cfg.pack = c->pack;
-  cfg.block = c->opt_block ? (unsigned)c->opt_block : 256u;
-  const size_t blob_b = ((blob_bytes(c) + 15) & ~(size_t)15);
-  // table placement (north_star subsystem 1): shared memory when blob + tables leave room for >= 2 CTAs/SM
-  const size_t smem_budget = c->smem_optin;
-  bool tab_smem = false;
-  if (c->placement == MT_PLACE_SMEM) {
-    if (blob_b + c->table_bytes > smem_budget) return fail(c, MT_ERR_UNSUPPORTED, "tables (%zu B) do not fit in shared memory", c->table_bytes);
-    tab_smem = true;
-  } else if (c->placement == MT_PLACE_AUTO) {
-    tab_smem = (blob_b + c->table_bytes) * 2 <= smem_budget;
-  }
-  cfg.tab_smem = tab_smem;
-  cfg.smem_bytes = blob_b + (tab_smem ? c->table_bytes : 0) + 16;
-  if (cfg.smem_bytes > smem_budget) return fail(c, MT_ERR_UNSUPPORTED, "region table too large for shared memory");
-
   int sched = c->opt_sched;
   if (sched == MT_SCHED_AUTO) sched = (c->geom.mode == MT_GEOM_VOXEL) ? MT_SCHED_WAVEFRONT : MT_SCHED_REFILL;
-  cfg.sched = sched;
   P.refill_min_idle = c->opt_min_idle ? c->opt_min_idle : 1;
 
+  // Table placement (north_star subsystem 1).  The packed tables start with the most-used material; shared
+  // memory takes the longest prefix of whole material blocks that fits.  AUTO stages everything when that still
+  // leaves room for two CTAs per SM and otherwise nothing: on config 3 a shared-memory copy of the iron tables
+  // (154 KB, one 768-thread CTA per SM) measured 2 % slower than L1/L2 gathers (profiles/r1_sweeps.md).
+  // MT_PLACE_SMEM stages as many materials as fit.
+  MtLaunchCfg cfg;
+  cfg.pack = c->pack;
+  cfg.sched = sched;
+  const size_t blob_b = ((blob_bytes(c) + 15) & ~(size_t)15);
+  const size_t smem_budget = c->smem_optin;
+  if (blob_b + 16 > smem_budget) return fail(c, MT_ERR_UNSUPPORTED, "edges, axes and regions (%zu B) do not fit in shared memory", blob_b);
+  const size_t cell_b = (c->pack == 32) ? 4 : 8;
+  const size_t block_cells = (size_t)c->n_pbins * (c->n_dp + c->n_th);                // cells per material
+  const size_t fit_blocks = std::min<size_t>((smem_budget - blob_b - 16) / (block_cells * cell_b), c->n_materials);
+  size_t hot_blocks = 0;
+  if (c->placement == MT_PLACE_SMEM) {
+    if (fit_blocks == 0) return fail(c, MT_ERR_UNSUPPORTED, "no material's tables (%zu B) fit in shared memory", block_cells * cell_b);
+    hot_blocks = fit_blocks;
+  } else if (c->placement == MT_PLACE_AUTO) {
+    if ((blob_b + c->table_bytes + 16) * 2 <= smem_budget) hot_blocks = c->n_materials;
+  }
+  P.hot_cells = (uint32_t)(hot_blocks * block_cells);
+  cfg.tab_smem = hot_blocks > 0;
+  cfg.smem_bytes = blob_b + ((hot_blocks * block_cells * cell_b + 15) & ~(size_t)15) + 16;
+
+  // block size: the one that keeps the most threads resident (ties -> the smaller block)
   int occ = 0;
-  MT_CUDA(c, mt_occupancy(P, cfg, &occ));
+  cfg.block = 0;
+  for (unsigned cand : {256u, 384u, 512u, 768u}) {
+    if (c->opt_block && cand != 256u) break;
+    const unsigned blk = c->opt_block ? (unsigned)c->opt_block : cand;
+    MtLaunchCfg probe = cfg;
+    probe.block = blk;
+    int o = 0;
+    MT_CUDA(c, mt_occupancy(P, probe, &o));
+    if (c->opt_blocks_per_sm) o = std::min(o, c->opt_blocks_per_sm);
+    if ((size_t)o * blk > (size_t)occ * cfg.block) { occ = o; cfg.block = blk; }
+  }
   if (occ < 1) return fail(c, MT_ERR_UNSUPPORTED, "kernel does not fit on an SM with %zu B shared memory", cfg.smem_bytes);
-  if (c->opt_blocks_per_sm) occ = std::min(occ, c->opt_blocks_per_sm);
   const unsigned persistent_grid = (unsigned)(c->sm_count * occ);
 
   if (sched == MT_SCHED_STATIC) {
@@ -473,7 +536,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   // WAVEFRONT: one pass per z-slab; between passes the live muons are counting-sorted by xy cell.
   const bool voxel = (c->geom.mode == MT_GEOM_VOXEL);
   const double unit = voxel ? (double)c->geom.cell : 0.01;
-  const double slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : 32.0) * unit;
+  const double slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : 64.0) * unit;
   const double span = (double)c->geom.z_exit - (double)c->geom.z_min;
   const int n_pass = (int)std::max(1.0, std::min(ceil(span / slab), 4096.0));
   // sort key: the voxel column (coarsened until there are at most 2^18 keys), or a 128 x 128 grid over the world box
@@ -588,8 +651,7 @@ int mt_debug_sample(mt_ctx* c, int material, int pbin, int which, const uint32_t
   if (material < 1 || material > c->n_materials || pbin < 0 || pbin >= c->n_pbins || which < 0 || which > 1)
     return fail(c, MT_ERR_INVALID_ARG, "bad table selector");
   DeviceGuard g(c->device);
-  const size_t t = (size_t)(material - 1) * c->n_pbins + pbin;
-  const size_t cell = t * (c->n_dp + c->n_th) + (which ? c->n_dp : 0);
+  const size_t cell = (size_t)c->mat_cell0[material] + (size_t)pbin * (c->n_dp + c->n_th) + (which ? c->n_dp : 0);
   const char* tab = (const char*)c->d_tab.p + cell * (c->pack == 32 ? 4 : 8);
   MT_CUDA(c, mt_launch_debug_sample(c->pack, tab, (uint32_t)(which ? c->n_th : c->n_dp), d_words, n, d_cell_out,
                                     (cudaStream_t)cuda_stream));

@@ -12,11 +12,19 @@ struct MtRegionDev {
 
 // The "const blob": small read-only arrays every CTA stages into shared memory at start.
 //   [0, n_pbins]                         momentum-bin edges, float32
-//   [off_steps + 4*m .. +2]              h, h/2, h/6 of material m, m = 0..n_materials
+//   [off_steps + 4*m .. +3]              h, h/2, h/6 of material m, m = 0..n_materials, and the
+//                                        first cell of the material's tables in the packed array (int bits)
+//   [off_axes + 4*t .. +3]               lo_dp, d_dp * 2^-16, lo_th, d_th * 2^-16 (log2) of table t = (m-1)*n_pbins + i
 //   [off_zlo  + j]                       z_lo of region j (search array)
 //   [off_regions + 10*j ..]              MtRegionDev j
 struct MtBlobLayout {
-  int32_t off_steps, off_zlo, off_regions, n_words;
+  int32_t off_steps, off_axes, off_zlo, off_regions, n_words;
+};
+
+// Two x-neighbours of the padded field grid in one 32-byte record, so that the x-pair of a trilinear corner set
+// is one 256-bit load.  a = cell x, b = cell x+1; .w = material id (int bits).
+struct __align__(32) MtCellPair {
+  float4 a, b;
 };
 
 struct MtParams {
@@ -26,19 +34,19 @@ struct MtParams {
   int32_t max_steps, world_material, n_regions;
   int32_t nx, ny, nz;
   float ox, oy, oz, inv_cell;
-  const float4* grid;            // [nz+2][ny+2][nx+2] {Bx, By, Bz, material as int bits}: the caller's grids with a
-                                 // one-cell clamp-replicated border, library-owned
+  const MtCellPair* grid;        // [nz+2][ny+2][nx+2] pairs {cell x, cell x+1} of {Bx, By, Bz, material}: the caller's grids
+                                 // with a one-cell clamp-replicated border, library-owned
   int32_t gsy, gsz;              // grid strides in cells: nx+2 and (nx+2)(ny+2)
   float fnx, fny, fnz;           // (float)nx, ny, nz for the inside test
   // ---- tables
   int32_t n_materials, n_pbins, n_dp, n_th;
   float inv_p_lo, bin_scale;     // bin guess: floor(log2(P * inv_p_lo) * bin_scale), then fixed on the edges
-  const uint32_t* tab32;         // pack32: [material-1][pbin][n_dp + n_th] = threshold24 << 8 | alias8
-  const uint2* tab64;            // pack64: same shape, {threshold (<= 2^24), alias}
-  const float4* axes;            // [material-1][pbin] = {lo_dp, d_dp, lo_th, d_th} (log2)
+  const uint32_t* tab32;         // pack32: [material block][pbin][n_dp + n_th] = threshold24 << 8 | alias8; the blocks are
+  const uint2* tab64;            // ordered most-used material first.  pack64: same shape, {threshold (<= 2^24), alias}
   const float* blob;             // const blob (global copy)
   MtBlobLayout bl;
-  int32_t table_words;           // 32-bit words of the packed tables (for staging into shared memory)
+  uint32_t hot_cells;            // the first hot_cells cells of the packed tables are staged in shared memory
+                                 // (whole material blocks; 0 = none)
   // ---- this call
   uint64_t n, id_base;
   uint32_t key0, key1;           // Philox key = seed lo, hi
