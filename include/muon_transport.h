@@ -59,7 +59,9 @@ enum {
   MT_OPT_BLOCK_THREADS = 2,  /* 0 = library default; else a multiple of 32 in [32, 1024]                   */
   MT_OPT_BLOCKS_PER_SM = 3,  /* 0 = library default (persistent kernels)                                   */
   MT_OPT_SLAB_CELLS = 4,     /* wavefront: slab thickness along z, in units of 1 cm; 0 = default           */
-  MT_OPT_REFILL_MIN_IDLE = 5 /* refill: lanes of a warp that must be idle before it refills; 0 = default   */
+  MT_OPT_REFILL_MIN_IDLE = 5,/* refill: lanes of a warp that must be idle before it refills; 0 = default   */
+  MT_OPT_KEY_LOOKAHEAD = 6   /* wavefront: the sort key is the xy cell a muon reaches after this many percent */
+                             /* of a slab on a straight line; -1 = default (50), 0 = its current cell         */
 };
 
 const char* mt_strerror(int code);

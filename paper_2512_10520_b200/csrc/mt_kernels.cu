@@ -171,8 +171,13 @@ transport_kernel(const __grid_constant__ MtParams P) {
 // ------------------------------------------------------------------------------------------------
 // WAVEFRONT: sorted z-slab passes
 // ------------------------------------------------------------------------------------------------
-MT_DEV uint32_t sort_key(const MtParams& P, float x, float y) {
-  // any mapping works (the order never changes results); NaN and far-away positions land in a border cell
+MT_DEV uint32_t sort_key(const MtParams& P, float x, float y, float px, float py, float pz) {
+  // any mapping works (the order never changes results); NaN and far-away positions land in a border cell.
+  // The key is the xy cell the muon will be in after key_look metres of z on a straight line (about mid-slab), so
+  // that the muons of a warp fan out around a common cell instead of away from it.
+  const float t = __fdividef(P.key_look, fmaxf(pz, 0.05f));
+  x = fmaf(px, t, x);
+  y = fmaf(py, t, y);
   const float fx = fminf(fmaxf((x - P.key_x0) * P.key_inv, 0.0f), (float)(P.key_nx - 1));
   const float fy = fminf(fmaxf((y - P.key_y0) * P.key_inv, 0.0f), (float)(P.key_ny - 1));
   return (uint32_t)((int)fy * P.key_nx + (int)fx);
@@ -182,8 +187,8 @@ MT_DEV uint32_t sort_key(const MtParams& P, float x, float y) {
 __global__ void __launch_bounds__(256) wave_bin_kernel(const __grid_constant__ MtParams P) {
   const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += stride) {
-    const float4 a = __ldg(P.in_pos_q + i);
-    const uint32_t key = sort_key(P, a.x, a.y);
+    const float4 a = __ldg(P.in_pos_q + i), b = __ldg(P.in_mom + i);
+    const uint32_t key = sort_key(P, a.x, a.y, b.x, b.y, b.z);
     const uint32_t rank = atomicAdd(P.hist + key, 1u);
     P.u_key[i] = make_uint4((uint32_t)i, key, rank, 0u);
   }
@@ -305,7 +310,7 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
       if ((int)lane == leader) slot0 = atomicAdd(P.live_out_count, (unsigned)__popc(pm));
       slot0 = __shfl_sync(kFull, slot0, leader);
       if (parked) {
-        const uint32_t key = sort_key(P, m.x, m.y);
+        const uint32_t key = sort_key(P, m.x, m.y, m.px, m.py, m.pz);
         const unsigned peers = __match_any_sync(pm, key);
         const int pl = __ffs(peers) - 1;
         unsigned r0 = 0;

@@ -39,7 +39,7 @@ struct mt_ctx {
   size_t smem_optin = 0;
   std::string last_error;
   // options
-  int opt_sched = MT_SCHED_AUTO, opt_block = 0, opt_blocks_per_sm = 0, opt_slab_cells = 0, opt_min_idle = 0;
+  int opt_sched = MT_SCHED_AUTO, opt_block = 0, opt_blocks_per_sm = 0, opt_slab_cells = 0, opt_min_idle = 0, opt_key_look = -1;
   // histograms (host copies)
   bool have_hist = false, have_tables = false, have_geom = false;
   int32_t n_materials = 0, n_pbins = 0, n_dp = 0, n_th = 0;
@@ -276,6 +276,9 @@ int mt_set_option(mt_ctx* c, int option, int64_t value) {
     case MT_OPT_SLAB_CELLS:
       if (value < 0 || value > 1000000) return fail(c, MT_ERR_INVALID_ARG, "bad slab thickness");
       c->opt_slab_cells = (int)value; return MT_OK;
+    case MT_OPT_KEY_LOOKAHEAD:
+      if (value < -1 || value > 400) return fail(c, MT_ERR_INVALID_ARG, "bad key lookahead");
+      c->opt_key_look = (int)value; return MT_OK;
     case MT_OPT_REFILL_MIN_IDLE:
       if (value < 0 || value > 32) return fail(c, MT_ERR_INVALID_ARG, "bad refill threshold");
       c->opt_min_idle = (int)value; return MT_OK;
@@ -552,6 +555,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
     P.key_x0 = c->geom.x_min; P.key_y0 = c->geom.y_min; P.key_inv = 128.0f / ext;
   }
   P.key_nx = key_nx; P.key_ny = key_ny;
+  P.key_look = (float)(slab * 0.01 * (c->opt_key_look >= 0 ? (double)c->opt_key_look : 50.0));
   const int n_keys = key_nx * key_ny;
   // scratch: [n_pass + 1] work counters (u64), [n_pass + 1] live counts (u32), histogram and offsets [n_keys] (u32)
   const size_t off_counts = (size_t)(n_pass + 1) * 8, off_hist = (off_counts + (size_t)(n_pass + 1) * 4 + 255) & ~(size_t)255;

@@ -76,4 +76,5 @@ struct MtParams {
   uint32_t* key_offset;          // [n_keys] exclusive scan of hist
   float key_x0, key_y0, key_inv; // sort key = iy * key_nx + ix, ix = clamp((int)((x - key_x0) * key_inv), 0, key_nx-1)
   int32_t key_nx, key_ny;
+  float key_look;                // the key uses the position extrapolated this far along z (metres)
 };
