@@ -481,7 +481,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   // Table placement (north_star subsystem 1).  The packed tables start with the most-used material; shared
   // memory takes the longest prefix of whole material blocks that fits.  AUTO stages everything when that still
   // leaves room for two CTAs per SM and otherwise nothing: on config 3 a shared-memory copy of the iron tables
-  // (154 KB, one 768-thread CTA per SM) measured 2 % slower than L1/L2 gathers (profiles/r1_sweeps.md).
+  // (154 KB, one 768-thread CTA per SM) measured 2 % slower than L1/L2 gathers (profiles/r1c_summary.md).
   // MT_PLACE_SMEM stages as many materials as fit.
   MtLaunchCfg cfg;
   cfg.pack = c->pack;
