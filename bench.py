@@ -9,6 +9,8 @@ roofline target is quoted on.  Rank r transports its own 10^7 muons (ids r*M ..)
 path (weak scaling).  One JSON line on stdout (rank 0); everything else goes to stderr.
 
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+`--sweep` runs BASELINE.json configs[4] on one GPU instead (10^8 muons in batches of 10^7 at each table shape and
+placement, then muons-per-launch 2^14 .. 2^24) and prints one JSON line per point.
 """
 import argparse
 import json
@@ -28,6 +30,9 @@ if ROOT not in sys.path:
 # DESIGN.md §3 counted one each; loads not counted as operations)
 ALG_OPS_PER_STEP = {"voxel": 383, "regions": 308}
 ALG_GATHER_BYTES_PER_STEP = {"voxel": 168, "regions": 40}
+# DRAM bytes (read + written) of ONE launch of the dominant kernel, from the `ncu --set full` capture summarised in
+# profiles/r1c_transport_kernel_full.csv (mean of the three captured z-slab passes of config 3)
+NCU_DRAM_BYTES_PER_LAUNCH = {"voxel": 0.756e9, "regions": None}
 SM_COUNT, LANES_PER_SM = 148, 128          # B200: 4 SMSPs x 32 lanes issue one warp instruction per clock
 
 
@@ -183,8 +188,9 @@ def run_ours(args, rank, world, local_rank):
         dist.barrier()
     b.lib()
 
-    n = args.muons
-    id_base = rank * n
+    from paper_2512_10520_b200.sharding import reduce_job, weak_shard
+    shard = weak_shard(args.muons, rank, world)               # own batch, own id range, no collective
+    n, id_base = shard.n, shard.id_base
     wl = make_workload(args.config, n, dev, rank)
     mode = "voxel" if wl.geom.mode == 1 else "regions"
     h = b.MuonTransport(local_rank).setup(wl.hist, wl.geom, args.placement)
@@ -257,13 +263,8 @@ def run_ours(args, rank, world, local_rank):
     d2h = h_out["pos_flag"].numel() * 4 + h_out["mom_steps"].numel() * 4 + 64
 
     # ---- max over ranks, totals over ranks
-    t = torch.tensor([t_dev, t_e2e, wall], dtype=torch.float64, device=dev)
-    tot = torch.tensor([steps_per_call, n], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    t_dev_max, t_e2e_max, wall_max = t.tolist()
-    steps_all, muons_all = tot.tolist()
+    (t_dev_max, t_e2e_max, wall_max), (steps_all, muons_all) = reduce_job(
+        [t_dev, t_e2e, wall], [steps_per_call, n], dist if world > 1 else None, dev)
     h.close()
     if rank != 0:
         return
@@ -293,8 +294,11 @@ def run_ours(args, rank, world, local_rank):
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "T thread-ops/s",
-                     "frac": achieved / alu_peak, "traffic": None,
-                     "kernel": "transport_kernel (%d launches per step)" % launches_per_step,
+                     "frac": achieved / alu_peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH[mode],
+                     "traffic_unit": "DRAM bytes per launch of the kernel (ncu, profiles/r1c_transport_kernel_full.csv)",
+                     "kernel": ("wave_transport_kernel: %d z-slab passes among the %d launches of a step (the rest sort the "
+                                "live list)" % ((launches_per_step - 1) // 3, launches_per_step)) if launches_per_step > 1
+                     else "transport_kernel (1 launch per step)",
                      "ops_per_muon_step": ALG_OPS_PER_STEP[mode], "peak_source": "148 SM x 128 lanes x %s sm_max_mhz"
                      % peaks["source"], "gather_tb_per_s": gather_tbs,
                      "gather_bytes_per_muon_step": ALG_GATHER_BYTES_PER_STEP[mode],
@@ -309,6 +313,81 @@ def run_ours(args, rank, world, local_rank):
         line["cpu_baseline"] = {"value": s / dt, "unit": "muon-steps/s", "cores": cores, "kind": "oracle",
                                 "sample": desc, "muons_per_s": m / dt, "seconds": dt}
     print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------ configs[4] sweep
+def run_sweep(args):
+    """BASELINE.json configs[4] on one GPU: (A) 10^8 muons in 10 batches of 10^7 (id_base = batch * 10^7) for every
+    table shape x placement; (B) muons per launch 2^14 .. 2^24 on the middle shape.  One JSON line per point."""
+    import torch
+    from paper_2512_10520_b200 import binding as b, build as lib_build, workloads as w
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the transport path has no CPU fallback")
+    lib_build.build()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    peaks = load_peaks()
+    alu_peak = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6
+    n_batch, n_batches = args.muons, args.sweep_batches
+    stream = torch.cuda.Stream(device=dev)
+    base = w.config3(n=8, device=dev)                        # grids once; histograms are regenerated per shape
+    out = {"pos_flag": torch.empty((n_batch, 4), dtype=torch.float32, device=dev),
+           "mom_steps": torch.empty((n_batch, 4), dtype=torch.float32, device=dev)}
+
+    def timed(h, d_pos, d_mom, id_base, o):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            r = h.transport(d_pos, d_mom, base.seed, id_base=id_base, out=o, stream=stream)
+            e1.record(stream)
+            stream.synchronize()
+        return e0.elapsed_time(e1) * 1e-3, int(r["counters"][0].item())
+
+    def emit(**kw):
+        kw["roofline_frac"] = kw["muon_steps_per_s"] * ALG_OPS_PER_STEP["voxel"] / alu_peak
+        print(json.dumps(kw), flush=True)
+
+    batches = [w.spectrum_muons(3, n_batch, "square", batch=k) for k in range(n_batches)]
+    for shape in w.CONFIG4_TABLE_SHAPES:
+        t0 = time.time()
+        hist = w.shield_histograms(3, [1.0, 1.0, 10.0], shape[0], shape[1], shape[2], args.sweep_draws)
+        log("[sweep] tables %dx%dx%d generated in %.1f s" % (shape + (time.time() - t0,)))
+        for placement, pname in ((b.MT_PLACE_AUTO, "auto"), (b.MT_PLACE_L2, "l2"), (b.MT_PLACE_SMEM, "smem")):
+            h = b.MuonTransport(0)
+            try:
+                h.setup(hist, base.geom, placement)
+                h.set_option(b.MT_OPT_SCHEDULE, args.sched)
+                d0, m0 = torch.from_numpy(batches[0].pos_q).to(dev), torch.from_numpy(batches[0].mom).to(dev)
+                for _ in range(2):
+                    timed(h, d0, m0, 0, out)                 # warm-up
+                t_tot, s_tot = 0.0, 0
+                for k, mu in enumerate(batches):
+                    d_pos, d_mom = torch.from_numpy(mu.pos_q).to(dev), torch.from_numpy(mu.mom).to(dev)
+                    dt, st = timed(h, d_pos, d_mom, k * n_batch, out)
+                    t_tot += dt; s_tot += st
+                emit(sweep="table_shape", pbins_x_dp_x_theta="%dx%dx%d" % shape, placement=pname,
+                     muons=n_batch * n_batches, batches=n_batches, muon_steps=s_tot, seconds=t_tot,
+                     muon_steps_per_s=s_tot / t_tot, muons_per_s=n_batch * n_batches / t_tot)
+            except b.MtError as e:
+                emit(sweep="table_shape", pbins_x_dp_x_theta="%dx%dx%d" % shape, placement=pname,
+                     muon_steps_per_s=0.0, unsupported=str(e))
+            finally:
+                h.close()
+        if shape == w.CONFIG4_TABLE_SHAPES[1]:
+            h = b.MuonTransport(0).setup(hist, base.geom, b.MT_PLACE_AUTO)
+            h.set_option(b.MT_OPT_SCHEDULE, args.sched)
+            d_pos, d_mom = torch.from_numpy(batches[0].pos_q).to(dev), torch.from_numpy(batches[0].mom).to(dev)
+            n_all = min(n_batch, 1 << 24)
+            for log2n in range(14, 25, 2):
+                n = min(1 << log2n, n_all)
+                o = {"pos_flag": out["pos_flag"][:n], "mom_steps": out["mom_steps"][:n]}
+                best, st = None, 0
+                for rep in range(4):
+                    dt, st = timed(h, d_pos[:n], d_mom[:n], 0, o)
+                    best = dt if best is None or (rep > 0 and dt < best) else best
+                emit(sweep="muons_per_launch", pbins_x_dp_x_theta="%dx%dx%d" % shape, placement="auto", muons=n,
+                     muon_steps=st, seconds=best, muon_steps_per_s=st / best, muons_per_s=n / best)
+            h.close()
 
 
 def main():
@@ -328,13 +407,19 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-seconds", type=float, default=15.0, help="CPU work per oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
+    ap.add_argument("--sweep-batches", type=int, default=10)
+    ap.add_argument("--sweep-draws", type=int, default=1_000_000, help="draws per generated histogram")
     args = ap.parse_args()
     if args.warmup < 1:
         args.warmup = 1
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_ours(args, rank, world, local_rank)

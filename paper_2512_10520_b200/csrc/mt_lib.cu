@@ -539,7 +539,9 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   // WAVEFRONT: one pass per z-slab; between passes the live muons are counting-sorted by xy cell.
   const bool voxel = (c->geom.mode == MT_GEOM_VOXEL);
   const double unit = voxel ? (double)c->geom.cell : 0.01;
-  const double slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : 64.0) * unit;
+  // default slab: 64 cells; small batches are bound by the latency of one muon's ~3000 dependent steps, so they take
+  // thicker slabs (fewer passes to launch) — profiles/r1d_config4_sweep.md
+  const double slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : (n < ((uint64_t)1 << 19) ? 256.0 : 64.0)) * unit;
   const double span = (double)c->geom.z_exit - (double)c->geom.z_min;
   const int n_pass = (int)std::max(1.0, std::min(ceil(span / slab), 4096.0));
   // sort key: the voxel column (coarsened until there are at most 2^18 keys), or a 128 x 128 grid over the world box

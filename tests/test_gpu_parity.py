@@ -190,3 +190,30 @@ def test_config3_full_size_sampled(mt, oracle):
         h.close()
         del wl
         torch.cuda.empty_cache()
+
+
+# --------------------------------------------- config 4: the three table shapes, batches with id_base
+@pytest.mark.parametrize("shape", [(50, 128, 64), (100, 256, 128), (256, 1024, 512)])
+def test_config4_table_shapes_and_batches(mt, oracle, shape):
+    """BASELINE configs[4] on a reduced grid: every table shape of the sweep (pack32 and pack64 cells, shared-memory
+    and L2 placement), two batches whose ids continue (id_base = batch * n), element by element."""
+    import torch
+    from paper_2512_10520_b200 import workloads as w
+    b = mt.binding
+    n = 20_011
+    wl = w.config3(n=n, n_draws=30_000, n_cells=2, half_width_cells=40, device="cuda", table_shape=shape)
+    T, G = oracle.OracleTables(wl.hist), oracle.OracleGeometry(wl.geom)
+    placements = [b.MT_PLACE_AUTO, b.MT_PLACE_L2] + ([b.MT_PLACE_SMEM] if shape[0] <= 100 else [])
+    for batch in (0, 1):
+        mu = w.spectrum_muons(3, n, "square", batch=batch)
+        mu.pos_q[:, :2] *= np.float32(0.4)
+        mu.mom[::5] *= np.float32(0.2)
+        wl.muons = mu
+        ref = oracle_transport(oracle, wl, id_base=batch * n, tables=T, geom=G)
+        for placement in placements:
+            g = gpu_transport(mt, wl, placement=placement, id_base=batch * n)
+            c = compare(g, ref)
+            _report("config4 %dx%dx%d batch %d placement %d" % (shape + (batch, placement)), c)
+            assert c["matched"] >= MATCH and c["bit_exact"] == 1.0
+    del wl
+    torch.cuda.empty_cache()
