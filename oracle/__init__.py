@@ -26,7 +26,7 @@ class _Geometry(C.Structure):
                 ("n_regions", C.c_int32), ("regions", C.c_void_p),
                 ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("ox", C.c_float), ("oy", C.c_float), ("oz", C.c_float), ("cell", C.c_float),
-                ("material", C.c_void_p), ("field", C.c_void_p)]
+                ("material", C.c_void_p), ("field", C.c_void_p), ("field_mode", C.c_int32)]
 
 
 class _Tables(C.Structure):
@@ -34,7 +34,7 @@ class _Tables(C.Structure):
                 ("p_lo", C.c_double), ("p_hi", C.c_double),
                 ("prob_dp", C.c_void_p), ("alias_dp", C.c_void_p),
                 ("prob_th", C.c_void_p), ("alias_th", C.c_void_p),
-                ("axis_dp", C.c_void_p), ("axis_th", C.c_void_p), ("step_m", C.c_void_p)]
+                ("axis_dp", C.c_void_p), ("axis_th", C.c_void_p), ("step_m", C.c_void_p), ("joint", C.c_int32)]
 
 
 def lib():
@@ -45,6 +45,10 @@ def lib():
         _lib.orc_kick_f32.restype = C.c_float
         _lib.orc_kick_f64.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_uint32]
         _lib.orc_kick_f32.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_uint32]
+        _lib.orc_kick_joint_f64.restype = C.c_double
+        _lib.orc_kick_joint_f32.restype = C.c_float
+        _lib.orc_kick_joint_f64.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_uint32]
+        _lib.orc_kick_joint_f32.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_uint32]
         _lib.orc_rk4_f64.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_double, C.c_int]
         _lib.orc_rk4_f32.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_float, C.c_int]
         _lib.orc_make_edges.argtypes = [C.c_double, C.c_double, C.c_int, C.c_void_p]
@@ -102,6 +106,15 @@ def alias_draw(prob, alias, words):
     prob, alias, words = _c(prob, np.float32), _c(alias, np.uint32), _c(words, np.uint32)
     out = np.empty(words.shape, np.uint32)
     lib().orc_alias_draw(_p(prob), _p(alias), C.c_int(len(prob)), _p(words), C.c_uint64(words.size), _p(out))
+    return out
+
+
+def alias_draw2(prob, alias, w_sel, w_acc):
+    """two-word draw of the joint mode"""
+    prob, alias = _c(prob, np.float32).reshape(-1), _c(alias, np.uint32).reshape(-1)
+    w_sel, w_acc = _c(w_sel, np.uint32), _c(w_acc, np.uint32)
+    out = np.empty(w_sel.shape, np.uint32)
+    lib().orc_alias_draw2(_p(prob), _p(alias), C.c_uint32(len(prob)), _p(w_sel), _p(w_acc), C.c_uint64(w_sel.size), _p(out))
     return out
 
 
@@ -167,6 +180,17 @@ def kick(p, f, theta, k24, dtype=np.float64):
     return p, Pn
 
 
+def kick_joint(p, fz, ft, k24, dtype=np.float64):
+    """one kick of the joint mode -> (new p, new |p|)"""
+    p = _c(p, dtype).copy()
+    P = np.sqrt((p.astype(np.float64) ** 2).sum())
+    if dtype == np.float64:
+        Pn = lib().orc_kick_joint_f64(_p(p), float(P), float(fz), float(ft), int(k24))
+    else:
+        Pn = lib().orc_kick_joint_f32(_p(p), float(np.float32(P)), float(np.float32(fz)), float(np.float32(ft)), int(k24))
+    return p, Pn
+
+
 def rk4(r, p, q, B, h, n_steps, dtype=np.float64):
     """n_steps RK4 steps of length h in a uniform field B -> (r, p)"""
     r, p, B = _c(r, dtype).copy(), _c(p, dtype).copy(), _c(B, dtype)
@@ -203,6 +227,7 @@ class OracleGeometry:
         s.ox, s.oy, s.oz, s.cell = g.ox, g.oy, g.oz, g.cell
         s.material = self.material.ctypes.data if self.material is not None else None
         s.field = self.field.ctypes.data if self.field is not None else None
+        s.field_mode = int(getattr(g, "field_mode", 0))
         self.struct = s
 
 
@@ -221,8 +246,14 @@ class OracleTables:
 
     def __init__(self, h):
         self.h = h
-        self.prob_dp, self.alias_dp = build_alias(h.counts_dp)
-        self.prob_th, self.alias_th = build_alias(h.counts_th)
+        self.joint = bool(getattr(h, "joint", False))
+        if self.joint:       # counts_dp holds the joint histograms [M][nb][n_dp][n_th]; one table per (M, i)
+            flat = _c(h.counts_dp, np.float32).reshape(h.n_materials, h.n_pbins, h.n_dp * h.n_th)
+            self.prob_dp, self.alias_dp = build_alias(flat)
+            self.prob_th, self.alias_th = np.zeros(1, np.float32), np.zeros(1, np.uint32)
+        else:
+            self.prob_dp, self.alias_dp = build_alias(h.counts_dp)
+            self.prob_th, self.alias_th = build_alias(h.counts_th)
         self.axis_dp, self.axis_th = _c(h.axis_dp, np.float32), _c(h.axis_th, np.float32)
         self.step_m = _c(h.step_m, np.float32)
         s = _Tables()
@@ -231,6 +262,7 @@ class OracleTables:
         s.prob_dp, s.alias_dp = self.prob_dp.ctypes.data, self.alias_dp.ctypes.data
         s.prob_th, s.alias_th = self.prob_th.ctypes.data, self.alias_th.ctypes.data
         s.axis_dp, s.axis_th, s.step_m = self.axis_dp.ctypes.data, self.axis_th.ctypes.data, self.step_m.ctypes.data
+        s.joint = 1 if self.joint else 0
         self.struct = s
 
     @property

@@ -16,6 +16,8 @@
 //   field lookup .............. L133 (§4.3; BASELINE.json configs[3] asks for trilinear)
 //   RK4 Lorentz push .......... L135-137 Eq. 4; L168-170 (one GetField per step, then RK4Step)
 //   termination ............... L65, L149
+//   joint 2D histogram mode ... L77 (§3), Fig. 3 L95, L163
+//   nearest-neighbour field ... L133 (§4.3); per-stage field evaluation: Eq. 4 integrated by RK4 proper
 //
 // Two modes from one templated source: Real=float is the parity reference (every + - * is one
 // IEEE binary32 operation in the written order, fma where DESIGN.md says fma; compile with
@@ -26,7 +28,8 @@
 // the mass-conservation identity; alias sampling vs exact enumeration and chi-square; bin edges vs
 // the paper's worked example (118.47-128.48 GeV); straight line; helix; RK4 h^4 convergence;
 // Rodrigues (Eq. 3) in double; trilinear on affine fields; region lookup vs brute force;
-// exp2/sin/cos polynomials vs libm.  Physics fidelity vs Geant4 (Figs. 5, 7): parity unpinned
+// exp2/sin/cos polynomials vs libm; two-word alias draw vs the exact pmf of the table; joint-mode kick vs its
+// geometry; nearest field vs the stored cell values; per-stage push vs h^4 convergence in a field gradient.  Physics fidelity vs Geant4 (Figs. 5, 7): parity unpinned
 // (needs Geant4 histograms, not available).
 
 #include <cmath>
@@ -106,6 +109,13 @@ inline uint32_t alias_draw(const float* prob, const uint32_t* alias, int N, uint
   const uint32_t k = (uint32_t)(m >> 32);
   const uint32_t a24 = ((uint32_t)m) >> 8;
   const float u = (float)a24 * 0x1p-24f;            // exact, in [0,1)
+  return (u < prob[k]) ? k : alias[k];
+}
+
+// joint tables have up to 2^24 cells, so one word selects and a second one accepts
+inline uint32_t alias_draw2(const float* prob, const uint32_t* alias, uint32_t N, uint32_t w_sel, uint32_t w_acc) {
+  const uint32_t k = (uint32_t)(((uint64_t)w_sel * (uint64_t)N) >> 32);
+  const float u = (float)(w_acc >> 8) * 0x1p-24f;    // exact, in [0,1)
   return (u < prob[k]) ? k : alias[k];
 }
 
@@ -207,7 +217,9 @@ struct Geometry {
   int32_t nx, ny, nz; float ox, oy, oz, cell;
   const uint8_t* material;      // [nz][ny][nx]
   const float* field;           // [nz][ny][nx][3]
+  int32_t field_mode;           // bit 0: nearest-neighbour instead of trilinear; bit 1: field at every RK4 stage
 };
+enum { FIELD_NEAREST = 1, FIELD_PER_STAGE = 2 };
 
 struct Tables {
   int32_t n_materials, n_pbins, n_dp, n_th;
@@ -216,6 +228,7 @@ struct Tables {
   const float* prob_th; const uint32_t* alias_th;    // [n_materials][n_pbins][n_th]
   const float* axis_dp; const float* axis_th;        // [n_materials][n_pbins][2] = {lo_log2, dlog2}
   const float* step_m;                               // [n_materials + 1]
+  int32_t joint;   // 1: prob_dp / alias_dp are joint tables [n_materials][n_pbins][n_dp * n_th]
 };
 
 // regions: greatest j with z_lo[j] <= z (binary search), then the half-open box test
@@ -276,7 +289,8 @@ void trilinear(const Geometry& g, R x, R y, R z, R B[3]) {
   }
 }
 
-// material and field at the start-of-step position (Alg. 1 l.5 and l.12 both use r before the move)
+// material and field at a position (Alg. 1 l.5 and l.12 both use r before the move).  Field of a voxel grid:
+// trilinear (BASELINE configs[3]) or, the stored value of the containing cell.
 template <class R>
 void material_and_field(const Geometry& g, R x, R y, R z, int* material, R B[3]) {
   if (g.mode == 0) { region_lookup<R>(g, x, y, z, material, B); return; }
@@ -284,8 +298,13 @@ void material_and_field(const Geometry& g, R x, R y, R z, int* material, R B[3])
   if (!voxel_cell<R>(g, x, y, z, &ix, &iy, &iz)) {
     *material = g.world_material; B[0] = B[1] = B[2] = (R)0; return;
   }
-  *material = g.material[((size_t)iz * g.ny + iy) * g.nx + ix];
-  trilinear<R>(g, x, y, z, B);
+  const size_t cell = ((size_t)iz * g.ny + iy) * g.nx + ix;
+  *material = g.material[cell];
+  if (g.field_mode & FIELD_NEAREST) {
+    for (int c = 0; c < 3; ++c) B[c] = (R)g.field[cell * 3 + c];
+  } else {
+    trilinear<R>(g, x, y, z, B);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -344,6 +363,53 @@ void rk4_step(R r[3], R p[3], R Pn, R q, const R B[3], R h, R h2, R h6) {
   }
 }
 
+// kick of the joint mode, dp = P [ft cos(phi), ft sin(phi), -fz] in the muon's frame (L163),
+// rotated by Eq. 3;  p <- P * [ ft cos(phi) e1 + ft sin(phi) e2 + (1 - fz) d ];  returns the new |p|
+template <class R>
+R kick_joint(R p[3], R P, R fz, R ft, R sin_phi, R cos_phi) {
+  const R inv = rrcp<R>(P);
+  const R a = p[0] * inv, b = p[1] * inv, c = p[2] * inv;
+  R e1[3], e2[3];
+  frame<R>(a, b, c, e1, e2);
+  const R tx = ft * cos_phi, ty = ft * sin_phi;
+  const R g = (R)1 - fz;
+  const R d[3] = {a, b, c};
+  for (int i = 0; i < 3; ++i) p[i] = P * rfma<R>(tx, e1[i], rfma<R>(ty, e2[i], g * d[i]));
+  return std::sqrt(rfma<R>(p[2], p[2], rfma<R>(p[1], p[1], p[0] * p[0])));
+}
+
+// RK4 of the coupled system (r, p) with the field looked up at every stage position
+template <class R>
+void rk4_step_per_stage(const Geometry& g, R r[3], R p[3], R Pn, R q, R h, R h2, R h6) {
+  const R KAPPA = (R)0.299792458f;
+  const R invP = rrcp<R>(Pn);
+  const R c1 = (KAPPA * q) * invP;
+  auto D = [&](const R at[3], const R v[3], R k[3]) {
+    int unused; R B[3];
+    material_and_field<R>(g, at[0], at[1], at[2], &unused, B);
+    const R bx = c1 * B[0], by = c1 * B[1], bz = c1 * B[2];
+    k[0] = rfma<R>(v[1], bz, -(v[2] * by));
+    k[1] = rfma<R>(v[2], bx, -(v[0] * bz));
+    k[2] = rfma<R>(v[0], by, -(v[1] * bx));
+  };
+  const R u = h2 * invP, v = h * invP;
+  R k1[3], k2[3], k3[3], k4[3], p2[3], p3[3], p4[3], r2[3], r3[3], r4[3];
+  D(r, p, k1);
+  for (int i = 0; i < 3; ++i) { p2[i] = rfma<R>(h2, k1[i], p[i]); r2[i] = rfma<R>(u, p[i], r[i]); }
+  D(r2, p2, k2);
+  for (int i = 0; i < 3; ++i) { p3[i] = rfma<R>(h2, k2[i], p[i]); r3[i] = rfma<R>(u, p2[i], r[i]); }
+  D(r3, p3, k3);
+  for (int i = 0; i < 3; ++i) { p4[i] = rfma<R>(h, k3[i], p[i]); r4[i] = rfma<R>(v, p3[i], r[i]); }
+  D(r4, p4, k4);
+  const R w = h6 * invP;
+  for (int i = 0; i < 3; ++i) {
+    const R sp = rfma<R>((R)2, p2[i] + p3[i], p[i] + p4[i]);
+    const R sk = rfma<R>((R)2, k2[i] + k3[i], k1[i] + k4[i]);
+    r[i] = rfma<R>(w, sp, r[i]);
+    p[i] = rfma<R>(h6, sk, p[i]);
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // Algorithm 1, one muon.
 // ------------------------------------------------------------------------------------------------
@@ -381,23 +447,40 @@ void transport_one(const Tables& T, const float* edges, const Geometry& g, uint6
       // l.8 alias draws + jitter, l.9 azimuth
       uint32_t w[4];
       muon_words(seed, id, (uint32_t)step, w);
-      const uint32_t cd = alias_draw(T.prob_dp + t * T.n_dp, T.alias_dp + t * T.n_dp, T.n_dp, w[0]);
-      const uint32_t ct = alias_draw(T.prob_th + t * T.n_th, T.alias_th + t * T.n_th, T.n_th, w[1]);
       const R ud = (R)(w[2] >> 16) * (R)0x1p-16f, ut = (R)(w[2] & 0xFFFFu) * (R)0x1p-16f;
+      uint32_t cd, ct;
+      if (T.joint) {
+        // the paper's own histogram (L77): one draw over the flattened (loss, kick) cells
+        const uint32_t N = (uint32_t)T.n_dp * (uint32_t)T.n_th;
+        const uint32_t cell = alias_draw2(T.prob_dp + t * N, T.alias_dp + t * N, N, w[0], w[1]);
+        cd = cell / (uint32_t)T.n_th;
+        ct = cell - cd * (uint32_t)T.n_th;
+      } else {
+        cd = alias_draw(T.prob_dp + t * T.n_dp, T.alias_dp + t * T.n_dp, T.n_dp, w[0]);
+        ct = alias_draw(T.prob_th + t * T.n_th, T.alias_th + t * T.n_th, T.n_th, w[1]);
+      }
       const R yd = rfma<R>((R)cd + ud, (R)T.axis_dp[2 * t + 1], (R)T.axis_dp[2 * t]);
       const R yt = rfma<R>((R)ct + ut, (R)T.axis_th[2 * t + 1], (R)T.axis_th[2 * t]);
-      const R f = std::min(exp2c<R>(yd), F_MAX);
-      const R theta = exp2c<R>(yt);
-      R st, ctv, sphi, cphi;
-      sincos_polar<R>(theta, &st, &ctv);
+      R sphi, cphi;
       sincos_azimuth<R>(w[3] >> 8, &sphi, &cphi);
-      // l.10-11 kick in the muon's frame, rotated to the lab (Eq. 3)
-      Pn = kick<R>(p, P, f, st, ctv, sphi, cphi);
+      if (T.joint) {
+        const R fz = std::min(exp2c<R>(yd), F_MAX);
+        const R ft = exp2c<R>(yt);
+        Pn = kick_joint<R>(p, P, fz, ft, sphi, cphi);
+      } else {
+        const R f = std::min(exp2c<R>(yd), F_MAX);
+        const R theta = exp2c<R>(yt);
+        R st, ctv;
+        sincos_polar<R>(theta, &st, &ctv);
+        // l.10-11 kick in the muon's frame, rotated to the lab (Eq. 3)
+        Pn = kick<R>(p, P, f, st, ctv, sphi, cphi);
+      }
       tr.pbin = i; tr.cell_dp = (int32_t)cd; tr.cell_th = (int32_t)ct;
     }
     if (trace && step < trace_cap) trace[step] = tr;
-    // l.13 RK4 with the field frozen over the step
-    rk4_step<R>(r, p, Pn, q, B, h, h2, h6);
+    // l.13 RK4: field frozen over the step (paper-literal) or looked up at every stage
+    if (g.field_mode & FIELD_PER_STAGE) rk4_step_per_stage<R>(g, r, p, Pn, q, h, h2, h6);
+    else rk4_step<R>(r, p, Pn, q, B, h, h2, h6);
     ++step;
   }
   *steps_out = step;
@@ -452,6 +535,22 @@ void orc_alias_draw(const float* prob, const uint32_t* alias, int N, const uint3
 void orc_alias_enumerate(const float* prob, const uint32_t* alias, int N, uint64_t* counts) {
   for (int j = 0; j < N; ++j) counts[j] = 0;
   for (uint64_t w = 0; w < (1ull << 32); ++w) counts[alias_draw(prob, alias, N, (uint32_t)w)]++;
+}
+
+void orc_alias_draw2(const float* prob, const uint32_t* alias, uint32_t N, const uint32_t* w_sel,
+                     const uint32_t* w_acc, uint64_t n, uint32_t* cell) {
+  for (uint64_t i = 0; i < n; ++i) cell[i] = alias_draw2(prob, alias, N, w_sel[i], w_acc[i]);
+}
+
+double orc_kick_joint_f64(double* p, double P, double fz, double ft, uint32_t k24) {
+  double sp, cp;
+  sincos_azimuth<double>(k24, &sp, &cp);
+  return kick_joint<double>(p, P, fz, ft, sp, cp);
+}
+float orc_kick_joint_f32(float* p, float P, float fz, float ft, uint32_t k24) {
+  float sp, cp;
+  sincos_azimuth<float>(k24, &sp, &cp);
+  return kick_joint<float>(p, P, fz, ft, sp, cp);
 }
 
 void orc_make_edges(double p_lo, double p_hi, int n, float* edges) { make_edges(p_lo, p_hi, n, edges); }

@@ -18,6 +18,7 @@ REGION_DTYPE = np.dtype([("z_lo", "<f4"), ("z_hi", "<f4"), ("x_lo", "<f4"), ("x_
                          ("bx", "<f4"), ("by", "<f4"), ("bz", "<f4")])
 
 MODE_REGIONS, MODE_VOXEL = 0, 1
+FIELD_TRILINEAR, FIELD_NEAREST, FIELD_PER_STAGE = 0, 1, 2
 
 # material -> (density g/cm3, radiation length cm); BASELINE.json configs[0], configs[2]
 MATERIALS = {"iron": (7.874, 1.757), "concrete": (2.3, 11.55), "air": (1.205e-3, 30390.0)}
@@ -38,6 +39,8 @@ class Histograms:
     axis_dp: np.ndarray     # [n_materials][n_pbins][2] float32 = {log2 lower edge, log2 width per cell}
     axis_th: np.ndarray
     step_m: np.ndarray      # [n_materials + 1] float32, path length per step; index 0 = vacuum
+    joint: bool = False     # True: counts_dp is ONE joint histogram [n_materials][n_pbins][n_dp][n_th] per (M, i) over
+                            # (log2 of -dPz/|P|, log2 of dPt/|P|) as in PAPER.md L77, and counts_th is None
 
 
 @dataclass
@@ -62,6 +65,7 @@ class Geometry:
     cell: float = 0.0
     material: object = None             # uint8 [nz][ny][nx], numpy or torch (any device)
     field: object = None                # float32 [nz][ny][nx][3]
+    field_mode: int = 0                 # FIELD_NEAREST | FIELD_PER_STAGE; 0 = trilinear, frozen
 
 
 @dataclass
@@ -86,7 +90,7 @@ def _rng(config, tag):
 
 # --------------------------------------------------------------------------------------- histograms
 def _one_histogram(args):
-    (config, tag, rho, x0_cm, step_cm, p_a, p_b, n_dp, n_th, n_draws) = args
+    (config, tag, rho, x0_cm, step_cm, p_a, p_b, n_dp, n_th, n_draws, joint) = args
     rng = _rng(config, tag)
     P = rng.uniform(p_a, p_b, n_draws)                                     # GeV
     # momentum loss: Moyal(loc, 0.1 loc) + Exp(mean 3e-6 rho L P)   [GeV]
@@ -102,7 +106,12 @@ def _one_histogram(args):
     tail = rng.random(n_draws) < 0.01
     u = rng.random(n_draws)
     th = np.where(tail, theta0 * (1.0 - 0.999 * u) ** (-1.0 / 3.0), th)
-    out = []
+    if joint:
+        # the paper's variables (L73, L77): longitudinal fractional loss and transverse fractional kick of the
+        # same draw, fz = -dPz/|P| = 1 - (1 - f) cos(theta), ft = dPt/|P| = (1 - f) sin(theta)
+        f = np.minimum(f, 0.999)
+        f, th = 1.0 - (1.0 - f) * np.cos(th), (1.0 - f) * np.sin(th)
+    out, cells = [], []
     for v, n_cells, q_lo in ((f, n_dp, 0.0), (th, n_th, 1e-3)):
         lv = np.log2(np.maximum(v, 1e-300))
         lo = float(np.quantile(lv, q_lo)) if q_lo > 0 else float(lv.min())
@@ -112,11 +121,15 @@ def _one_histogram(args):
         cell = np.clip(np.floor((lv - float(lo32)) / float(d32)), 0, n_cells - 1).astype(np.int64)
         counts = np.bincount(cell, minlength=n_cells).astype(np.float32)
         out.append((counts, np.array([lo32, d32], np.float32)))
+        cells.append(cell)
+    if joint:
+        both = np.bincount(cells[0] * n_th + cells[1], minlength=n_dp * n_th).astype(np.float32)
+        out[0] = (both.reshape(n_dp, n_th), out[0][1])
     return out
 
 
 def make_histograms(config, materials, steps_cm, n_pbins, p_lo, p_hi, n_dp, n_th, n_draws=1_000_000,
-                    vacuum_step_m=None, workers=None):
+                    vacuum_step_m=None, workers=None, joint=False):
     """materials: list of names (material id = index + 1); steps_cm: step length per material."""
     M = len(materials)
     edges = p_lo * (p_hi / p_lo) ** (np.arange(n_pbins + 1) / n_pbins)
@@ -124,18 +137,18 @@ def make_histograms(config, materials, steps_cm, n_pbins, p_lo, p_hi, n_dp, n_th
     for m, (name, step_cm) in enumerate(zip(materials, steps_cm)):
         rho, x0 = MATERIALS[name]
         for i in range(n_pbins):
-            jobs.append((config, m * 4096 + i, rho, x0, step_cm, edges[i], edges[i + 1], n_dp, n_th, n_draws))
+            jobs.append((config, m * 4096 + i, rho, x0, step_cm, edges[i], edges[i + 1], n_dp, n_th, n_draws, joint))
     workers = workers or min(32, os.cpu_count() or 1)
     with ThreadPoolExecutor(workers) as ex:
         res = list(ex.map(_one_histogram, jobs))
-    counts_dp = np.stack([r[0][0] for r in res]).reshape(M, n_pbins, n_dp)
-    counts_th = np.stack([r[1][0] for r in res]).reshape(M, n_pbins, n_th)
+    counts_dp = np.stack([r[0][0] for r in res]).reshape((M, n_pbins, n_dp, n_th) if joint else (M, n_pbins, n_dp))
+    counts_th = None if joint else np.stack([r[1][0] for r in res]).reshape(M, n_pbins, n_th)
     axis_dp = np.stack([r[0][1] for r in res]).reshape(M, n_pbins, 2)
     axis_th = np.stack([r[1][1] for r in res]).reshape(M, n_pbins, 2)
     step_m = np.array([vacuum_step_m if vacuum_step_m is not None else max(steps_cm) / 100.0]
                       + [s / 100.0 for s in steps_cm], np.float32)
     return Histograms(M, n_pbins, n_dp, n_th, float(p_lo), float(p_hi), counts_dp, counts_th,
-                      axis_dp, axis_th, step_m)
+                      axis_dp, axis_th, step_m, joint=joint)
 
 
 # -------------------------------------------------------------------------------------------- muons
@@ -224,9 +237,9 @@ def rasterise(regions, world_material, nx, ny, nz, ox, oy, oz, cell, config, dev
 
 
 # ---------------------------------------------------------------------------------------- configs
-def config0(n=4096, n_draws=1_000_000):
-    """Toy slab, no field (BASELINE.json configs[0])."""
-    hist = make_histograms(0, ["iron"], [2.0], 50, 1.0, 300.0, 128, 64, n_draws)
+def config0(n=4096, n_draws=1_000_000, joint=False):
+    """Toy slab, no field (BASELINE.json configs[0]).  joint=True: the paper's joint 2D histograms (§8(f) row 1)."""
+    hist = make_histograms(0, ["iron"], [2.0], 50, 1.0, 300.0, 128, 64, n_draws, joint=joint)
     regs = np.array([(0.0, 1.0, -10.0, 10.0, -10.0, 10.0, 1, 0.0, 0.0, 0.0)], REGION_DTYPE)
     geom = Geometry(MODE_REGIONS, -10.0, 10.0, -10.0, 10.0, 0.0, 1.0, 1.0, 200, 0, regions=regs)
     pos_q = np.zeros((n, 4), np.float32)
@@ -236,22 +249,22 @@ def config0(n=4096, n_draws=1_000_000):
     return Workload("config0_toy_slab", hist, geom, Muons(pos_q, mom), seed=1)
 
 
-def config1(n=65536, n_draws=1_000_000):
+def config1(n=65536, n_draws=1_000_000, joint=False):
     """Magnetised iron block (configs[1])."""
-    hist = make_histograms(0, ["iron"], [2.0], 50, 1.0, 300.0, 128, 64, n_draws)
+    hist = make_histograms(0, ["iron"], [2.0], 50, 1.0, 300.0, 128, 64, n_draws, joint=joint)
     regs = np.array([(0.0, 6.0, -1.0, 1.0, -1.0, 1.0, 1, 0.0, 1.7, 0.0)], REGION_DTYPE)
     geom = Geometry(MODE_REGIONS, -1.0, 1.0, -1.0, 1.0, 0.0, 6.0, 1.0, 1200, 0, regions=regs)
     return Workload("config1_magnetised_block", hist, geom, spectrum_muons(1, n, "gauss"), seed=1)
 
 
-def shield_histograms(config, steps_cm, n_pbins=100, n_dp=256, n_th=128, n_draws=1_000_000):
+def shield_histograms(config, steps_cm, n_pbins=100, n_dp=256, n_th=128, n_draws=1_000_000, joint=False):
     return make_histograms(config, ["iron", "concrete", "air"], steps_cm, n_pbins, 1.0, 300.0, n_dp, n_th,
-                           n_draws)
+                           n_draws, joint=joint)
 
 
-def config2(n=1_000_000, n_draws=1_000_000, n_cells=8):
+def config2(n=1_000_000, n_draws=1_000_000, n_cells=8, joint=False, table_shape=(100, 256, 128)):
     """Multi-region shield (configs[2]): sorted z-interval table plus per-region xy bounds."""
-    hist = shield_histograms(2, [2.0, 2.0, 2.0], n_draws=n_draws)
+    hist = shield_histograms(2, [2.0, 2.0, 2.0], table_shape[0], table_shape[1], table_shape[2], n_draws, joint=joint)
     z_exit = 3.75 * n_cells
     geom = Geometry(MODE_REGIONS, -1.0, 1.0, -1.0, 1.0, 0.0, z_exit, 1.0, 6000, 3,
                     regions=shield_regions(n_cells))
@@ -259,18 +272,20 @@ def config2(n=1_000_000, n_draws=1_000_000, n_cells=8):
 
 
 def config3(n=10_000_000, n_draws=1_000_000, n_cells=8, half_width_cells=100, device="cpu", hist=None,
-            table_shape=(100, 256, 128)):
+            table_shape=(100, 256, 128), joint=False, field_mode=0):
     """Field-map shield (configs[3]): voxel material + trilinear field grid, 1 cm cells; steps 1 cm in
     iron and concrete, 10 cm in air.  `n_cells` / `half_width_cells` shrink the grid for CPU tests."""
     if hist is None:
-        hist = shield_histograms(3, [1.0, 1.0, 10.0], table_shape[0], table_shape[1], table_shape[2], n_draws)
+        hist = shield_histograms(3, [1.0, 1.0, 10.0], table_shape[0], table_shape[1], table_shape[2], n_draws,
+                                 joint=joint)
     cell = 0.01
     nx = ny = 2 * half_width_cells
     nz = int(round(3.75 * n_cells / cell))
     half = half_width_cells * cell
     material, fld = rasterise(shield_regions(n_cells), 3, nx, ny, nz, -half, -half, 0.0, cell, 3, device)
     geom = Geometry(MODE_VOXEL, -half, half, -half, half, 0.0, nz * cell, 1.0, 12000, 3,
-                    nx=nx, ny=ny, nz=nz, ox=-half, oy=-half, oz=0.0, cell=cell, material=material, field=fld)
+                    nx=nx, ny=ny, nz=nz, ox=-half, oy=-half, oz=0.0, cell=cell, material=material, field=fld,
+                    field_mode=field_mode)
     mu = spectrum_muons(3, n, "square")
     if half < 1.0:                       # shrunken test grid: keep the start square inside it
         mu.pos_q[:, :2] *= np.float32(half)
