@@ -42,6 +42,19 @@ enum { MT_FLAG_STOPPED = 1, MT_FLAG_EXITED = 2, MT_FLAG_ESCAPED = 3, MT_FLAG_MAX
 
 enum { MT_GEOM_REGIONS = 0, MT_GEOM_VOXEL = 1 };
 
+/* what the histograms hold (mt_hist_desc.hist_mode) */
+enum {
+  MT_HIST_MARGINAL = 0,    /* BASELINE.json configs: one Dp/p and one polar-angle histogram per (material, bin)    */
+  MT_HIST_JOINT = 1        /* the paper's own (L77, Fig. 3): ONE 2D histogram per (material, bin) over             */
+};                         /* (log2 of -dPz/|P|, log2 of dPt/|P|), sampled through one alias table*/
+
+/* field lookup (mt_geometry.field_mode): interpolation, optionally | MT_FIELD_PER_STAGE */
+enum {
+  MT_FIELD_TRILINEAR = 0,  /* trilinear over cell centres (BASELINE.json configs[3]); regions: the region's B     */
+  MT_FIELD_NEAREST = 1,    /* VOXEL mode: the value of the cell that contains the point (the paper's own, L133)   */
+  MT_FIELD_PER_STAGE = 2   /* flag: B looked up at every Runge-Kutta stage position instead of once per step       */
+};
+
 /* alias-table placement (north_star subsystem 1) */
 enum { MT_PLACE_AUTO = 0, MT_PLACE_SMEM = 1, MT_PLACE_L2 = 2 };
 
@@ -84,6 +97,9 @@ typedef struct {
   const float* axis_dp;    /* [n_materials][n_pbins][2] = {log2 of the lower edge, log2 width of a cell}   */
   const float* axis_th;    /* same for theta (radians)                                                     */
   const float* step_m;     /* [n_materials + 1] path length per step in material id (index 0 = vacuum)     */
+  int32_t hist_mode;       /* MT_HIST_MARGINAL | MT_HIST_JOINT.  JOINT: counts_dp is [n_materials][n_pbins][n_dp][n_th]*/
+                           /* (axis a = longitudinal loss, n_dp cells, axis_dp; axis b = transverse kick, n_th     */
+                           /* cells, axis_th), counts_th is ignored, and n_dp * n_th <= 2^24, n_dp * n_th^2 < 2^32  */
 } mt_hist_desc;
 int mt_load_histograms(mt_ctx* ctx, const mt_hist_desc* desc);
 
@@ -91,7 +107,8 @@ int mt_load_histograms(mt_ctx* ctx, const mt_hist_desc* desc);
  * and upload them.  MT_ERR_EMPTY_HIST names the offending table in mt_last_error(). */
 int mt_build_alias(mt_ctx* ctx, int placement);
 
-/* Test export of the tables as built: HOST outputs shaped like counts_dp / counts_th. */
+/* Test export of the tables as built: HOST outputs shaped like counts_dp / counts_th.  JOINT mode: prob_dp / alias_dp
+ * are [n_materials][n_pbins][n_dp * n_th]; prob_th / alias_th are not written and may be NULL. */
 int mt_get_alias(const mt_ctx* ctx, float* prob_dp, uint32_t* alias_dp, float* prob_th, uint32_t* alias_th);
 
 /* Geometry G and field map (Alg. 1 "Input", L144-146; L61-63; §4.3).  Regions: axis-aligned boxes,
@@ -115,6 +132,7 @@ typedef struct {
   float ox, oy, oz, cell;
   const uint8_t* d_material; /* DEVICE [nz][ny][nx], read during the call only                            */
   const float* d_field;      /* DEVICE [nz][ny][nx][3], read during the call only                         */
+  int32_t field_mode;        /* MT_FIELD_TRILINEAR | MT_FIELD_NEAREST, optionally | MT_FIELD_PER_STAGE             */
 } mt_geometry;
 /* VOXEL mode repacks both grids into one library-owned 16-byte-per-cell grid {Bx,By,Bz,material}
  * (DESIGN.md §6), so the caller may free d_material / d_field after the call returns. */
@@ -152,7 +170,8 @@ int64_t mt_launch_count(const mt_ctx* ctx);
 
 /* Test hooks (DEVICE buffers, asynchronous on the stream).
  * mt_debug_sample: cell_out[i] = alias draw from table `which` (0 = Dp/p, 1 = theta) of
- * (material, pbin) with word d_words[i].
+ * (material, pbin) with word d_words[i].  JOINT mode (which = 0): d_words holds 2n words, the select word of draw i
+ * at [i] and its accept word at [n + i]; cell_out[i] is the flat cell index.
  * mt_debug_philox: out[i][0..3] = Philox4x32-10 block for (seed, id_base + i, step). */
 int mt_debug_sample(mt_ctx* ctx, int material, int pbin, int which, const uint32_t* d_words, uint64_t n,
                     uint32_t* d_cell_out, void* cuda_stream);

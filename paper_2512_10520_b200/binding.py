@@ -18,6 +18,8 @@ MT_PLACE_AUTO, MT_PLACE_SMEM, MT_PLACE_L2 = 0, 1, 2
 MT_SCHED_AUTO, MT_SCHED_STATIC, MT_SCHED_REFILL, MT_SCHED_WAVEFRONT = 0, 1, 2, 3
 MT_OPT_SCHEDULE, MT_OPT_BLOCK_THREADS, MT_OPT_BLOCKS_PER_SM, MT_OPT_SLAB_CELLS, MT_OPT_REFILL_MIN_IDLE = 1, 2, 3, 4, 5
 MT_OPT_KEY_LOOKAHEAD = 6
+MT_HIST_MARGINAL, MT_HIST_JOINT = 0, 1
+MT_FIELD_TRILINEAR, MT_FIELD_NEAREST, MT_FIELD_PER_STAGE = 0, 1, 2
 
 # every symbol include/muon_transport.h declares (tests check that the library exports each one)
 SYMBOLS = ["mt_strerror", "mt_last_error", "mt_create", "mt_destroy", "mt_set_option", "mt_load_histograms",
@@ -29,7 +31,7 @@ class mt_hist_desc(C.Structure):
     _fields_ = [("n_materials", C.c_int32), ("n_pbins", C.c_int32), ("p_lo", C.c_float), ("p_hi", C.c_float),
                 ("n_dp", C.c_int32), ("n_th", C.c_int32),
                 ("counts_dp", C.c_void_p), ("counts_th", C.c_void_p), ("axis_dp", C.c_void_p),
-                ("axis_th", C.c_void_p), ("step_m", C.c_void_p)]
+                ("axis_th", C.c_void_p), ("step_m", C.c_void_p), ("hist_mode", C.c_int32)]
 
 
 class mt_region(C.Structure):
@@ -46,7 +48,7 @@ class mt_geometry(C.Structure):
                 ("n_regions", C.c_int32), ("regions", C.c_void_p),
                 ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("ox", C.c_float), ("oy", C.c_float), ("oz", C.c_float), ("cell", C.c_float),
-                ("d_material", C.c_void_p), ("d_field", C.c_void_p)]
+                ("d_material", C.c_void_p), ("d_field", C.c_void_p), ("field_mode", C.c_int32)]
 
 
 class mt_muons_in(C.Structure):
@@ -132,13 +134,15 @@ def mt_set_option(ctx, option, value):
 
 def mt_load_histograms(ctx, hist):
     """hist: workloads.Histograms (or any object with the same attributes); host arrays."""
-    keep = [_np(hist.counts_dp, np.float32), _np(hist.counts_th, np.float32), _np(hist.axis_dp, np.float32),
-            _np(hist.axis_th, np.float32), _np(hist.step_m, np.float32)]
-    assert keep[0].size == hist.n_materials * hist.n_pbins * hist.n_dp
-    assert keep[1].size == hist.n_materials * hist.n_pbins * hist.n_th
+    joint = bool(getattr(hist, "joint", False))
+    keep = [_np(hist.counts_dp, np.float32), None if joint else _np(hist.counts_th, np.float32),
+            _np(hist.axis_dp, np.float32), _np(hist.axis_th, np.float32), _np(hist.step_m, np.float32)]
+    assert keep[0].size == hist.n_materials * hist.n_pbins * hist.n_dp * (hist.n_th if joint else 1)
+    assert joint or keep[1].size == hist.n_materials * hist.n_pbins * hist.n_th
     assert keep[2].size == keep[3].size == hist.n_materials * hist.n_pbins * 2 and keep[4].size == hist.n_materials + 1
     d = mt_hist_desc(hist.n_materials, hist.n_pbins, hist.p_lo, hist.p_hi, hist.n_dp, hist.n_th,
-                     *[a.ctypes.data for a in keep])
+                     *[a.ctypes.data if a is not None else None for a in keep],
+                     MT_HIST_JOINT if joint else MT_HIST_MARGINAL)
     _check(ctx, lib().mt_load_histograms(ctx, C.byref(d)))
 
 
@@ -147,6 +151,11 @@ def mt_build_alias(ctx, placement=MT_PLACE_AUTO):
 
 
 def mt_get_alias(ctx, hist):
+    if getattr(hist, "joint", False):
+        shp = (hist.n_materials, hist.n_pbins, hist.n_dp * hist.n_th)
+        prob, alias = np.empty(shp, np.float32), np.empty(shp, np.uint32)
+        _check(ctx, lib().mt_get_alias(ctx, prob.ctypes.data, alias.ctypes.data, None, None))
+        return prob, alias, None, None
     shp_dp = (hist.n_materials, hist.n_pbins, hist.n_dp)
     shp_th = (hist.n_materials, hist.n_pbins, hist.n_th)
     prob_dp, alias_dp = np.empty(shp_dp, np.float32), np.empty(shp_dp, np.uint32)
@@ -162,6 +171,7 @@ def mt_set_geometry(ctx, geom):
     g.mode = geom.mode
     g.x_min, g.x_max, g.y_min, g.y_max, g.z_min, g.z_exit = geom.x_min, geom.x_max, geom.y_min, geom.y_max, geom.z_min, geom.z_exit
     g.p_min, g.max_steps, g.world_material = geom.p_min, geom.max_steps, geom.world_material
+    g.field_mode = int(getattr(geom, "field_mode", 0))
     keep = None
     if geom.mode == MT_GEOM_REGIONS:
         regs = np.ascontiguousarray(geom.regions) if geom.regions is not None else np.zeros(0, np.uint8)
@@ -252,12 +262,14 @@ def mt_launch_count(ctx):
     return int(lib().mt_launch_count(ctx))
 
 
-def mt_debug_sample(ctx, material, pbin, which, words, stream=None):
+def mt_debug_sample(ctx, material, pbin, which, words, stream=None, joint=False):
+    """words: int32 CUDA tensor [n]; joint mode: [2n] = n select words then n accept words -> [n] cells"""
     import torch
     words = words.contiguous()
     assert words.is_cuda and words.dtype == torch.int32
-    out = torch.empty_like(words)
-    _check(ctx, lib().mt_debug_sample(ctx, material, pbin, which, words.data_ptr(), words.numel(), out.data_ptr(),
+    n = words.numel() // 2 if joint else words.numel()
+    out = torch.empty(n, dtype=torch.int32, device=words.device)
+    _check(ctx, lib().mt_debug_sample(ctx, material, pbin, which, words.data_ptr(), n, out.data_ptr(),
                                       _stream_ptr(stream)))
     return out
 

@@ -97,7 +97,7 @@ MT_DEV void write_final(const MtParams& P, const Muon& m, uint32_t idx, int flag
 // ------------------------------------------------------------------------------------------------
 // STATIC and REFILL
 // ------------------------------------------------------------------------------------------------
-template <int GEOM, int PACK, bool TAB_SMEM, int SCHED>
+template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD, int SCHED>
 __global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
 transport_kernel(const __grid_constant__ MtParams P) {
   const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
@@ -153,7 +153,7 @@ transport_kernel(const __grid_constant__ MtParams P) {
       int flag = 0;
       if (active) {
         const uint64_t id = P.id_base + idx;
-        flag = step_once<GEOM, PACK, TAB_SMEM, false>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
+        flag = step_once<GEOM, PACK, TAB_SMEM, false, JOINT, FIELD>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
         if (flag == 0) tally.steps += 1;
       }
       write_final(P, m, idx, flag, lane);
@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(256) wave_scatter_kernel(const __grid_constant
   }
 }
 
-template <int GEOM, int PACK, bool TAB_SMEM>
+template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD>
 __global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
 wave_transport_kernel(const __grid_constant__ MtParams P) {
   const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
@@ -293,7 +293,7 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
 
     // ---- step until every lane has terminated or reached the end of the slab
     for (;;) {
-      if (flag == 0) flag = step_once<GEOM, PACK, TAB_SMEM, true>(P, V, m, id_lo, id_hi, P.slab_z_end);
+      if (flag == 0) flag = step_once<GEOM, PACK, TAB_SMEM, true, JOINT, FIELD>(P, V, m, id_lo, id_hi, P.slab_z_end);
       if (!__any_sync(kFull, flag == 0)) break;
     }
     tally.steps += (unsigned)(m.step - step_in);
@@ -376,20 +376,43 @@ __global__ void debug_philox_kernel(uint32_t k0, uint32_t k1, uint64_t id_base, 
   reinterpret_cast<uint4*>(out)[i] = make_uint4(w[0], w[1], w[2], w[3]);
 }
 
+// two-word draw of the joint tables: words[i] selects, words[n + i] accepts
+__global__ void debug_sample_joint_kernel(const uint2* tab, uint32_t N, const uint32_t* words, uint64_t n, uint32_t* out) {
+  const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t k = __umulhi(words[i], N);
+  const uint2 e = __ldg(tab + k);
+  out[i] = ((words[n + i] >> 8) < e.x) ? k : e.y;
+}
+
 typedef void (*kernel_fn)(const MtParams);
 
-template <int GEOM, int PACK, bool TAB_SMEM>
+// Instantiated combinations: geometry x table kind {pack32, pack32 + shared prefix, pack64, pack64 + shared prefix,
+// joint (pack64)} x field mode {trilinear / region, per-stage; voxel only: nearest, nearest per-stage} x schedule.
+template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD>
 kernel_fn pick_sched(int sched) {
   switch (sched) {
-    case SCHED_STATIC: return transport_kernel<GEOM, PACK, TAB_SMEM, SCHED_STATIC>;
-    case SCHED_REFILL: return transport_kernel<GEOM, PACK, TAB_SMEM, SCHED_REFILL>;
-    default: return wave_transport_kernel<GEOM, PACK, TAB_SMEM>;
+    case SCHED_STATIC: return transport_kernel<GEOM, PACK, TAB_SMEM, JOINT, FIELD, SCHED_STATIC>;
+    case SCHED_REFILL: return transport_kernel<GEOM, PACK, TAB_SMEM, JOINT, FIELD, SCHED_REFILL>;
+    default: return wave_transport_kernel<GEOM, PACK, TAB_SMEM, JOINT, FIELD>;
   }
 }
-template <int GEOM>
-kernel_fn pick_pack(int pack, bool tab_smem, int sched) {
-  if (pack == 32) return tab_smem ? pick_sched<GEOM, 32, true>(sched) : pick_sched<GEOM, 32, false>(sched);
-  return tab_smem ? pick_sched<GEOM, 64, true>(sched) : pick_sched<GEOM, 64, false>(sched);
+template <int GEOM, int FIELD>
+kernel_fn pick_tables(const MtLaunchCfg& cfg) {
+  if (cfg.joint) return pick_sched<GEOM, 64, false, true, FIELD>(cfg.sched);
+  if (cfg.pack == 32) return cfg.tab_smem ? pick_sched<GEOM, 32, true, false, FIELD>(cfg.sched)
+                                          : pick_sched<GEOM, 32, false, false, FIELD>(cfg.sched);
+  return cfg.tab_smem ? pick_sched<GEOM, 64, true, false, FIELD>(cfg.sched)
+                      : pick_sched<GEOM, 64, false, false, FIELD>(cfg.sched);
+}
+kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
+  if (mode == 0) return (cfg.field & 2) ? pick_tables<0, 2>(cfg) : pick_tables<0, 0>(cfg);
+  switch (cfg.field & 3) {
+    case 1: return pick_tables<1, 1>(cfg);
+    case 2: return pick_tables<1, 2>(cfg);
+    case 3: return pick_tables<1, 3>(cfg);
+    default: return pick_tables<1, 0>(cfg);
+  }
 }
 
 }  // namespace
@@ -398,8 +421,7 @@ kernel_fn pick_pack(int pack, bool tab_smem, int sched) {
 // launchers (called from mt_lib.cu)
 // ------------------------------------------------------------------------------------------------
 cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream) {
-  kernel_fn fn = (P.mode == 0) ? pick_pack<0>(cfg.pack, cfg.tab_smem, cfg.sched)
-                               : pick_pack<1>(cfg.pack, cfg.tab_smem, cfg.sched);
+  kernel_fn fn = pick_kernel(P.mode, cfg);
   cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
   if (e != cudaSuccess) return e;
   void* args[] = {(void*)&P};
@@ -407,8 +429,7 @@ cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaS
 }
 
 cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm) {
-  kernel_fn fn = (P.mode == 0) ? pick_pack<0>(cfg.pack, cfg.tab_smem, cfg.sched)
-                               : pick_pack<1>(cfg.pack, cfg.tab_smem, cfg.sched);
+  kernel_fn fn = pick_kernel(P.mode, cfg);
   cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
   if (e != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, (const void*)fn, cfg.block, cfg.smem_bytes);
@@ -442,11 +463,12 @@ cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, MtCellPair* o
   return cudaGetLastError();
 }
 
-cudaError_t mt_launch_debug_sample(int pack, const void* tab, uint32_t N, const uint32_t* words, uint64_t n,
+cudaError_t mt_launch_debug_sample(int pack, bool joint, const void* tab, uint32_t N, const uint32_t* words, uint64_t n,
                                    uint32_t* out, cudaStream_t stream) {
   if (n == 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + 255) / 256);
-  if (pack == 32) debug_sample_kernel<32><<<grid, 256, 0, stream>>>((const uint32_t*)tab, N, words, n, out);
+  if (joint) debug_sample_joint_kernel<<<grid, 256, 0, stream>>>((const uint2*)tab, N, words, n, out);
+  else if (pack == 32) debug_sample_kernel<32><<<grid, 256, 0, stream>>>((const uint32_t*)tab, N, words, n, out);
   else debug_sample_kernel<64><<<grid, 256, 0, stream>>>((const uint2*)tab, N, words, n, out);
   return cudaGetLastError();
 }

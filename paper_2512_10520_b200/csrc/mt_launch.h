@@ -17,6 +17,8 @@ struct MtLaunchCfg {
   int pack;        // 32 or 64 (bits per packed alias cell)
   bool tab_smem;   // the hot prefix of the tables (P.hot_cells > 0) is staged in shared memory
   int sched;       // MT_SCHED_STATIC / _REFILL / _WAVEFRONT
+  bool joint;      // MT_HIST_JOINT tables (pack64, never staged)
+  int field;       // MT_FIELD_* of the geometry
 };
 
 cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream);
@@ -29,7 +31,7 @@ cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src
 // d_material_cells: [256] counters (zeroed by the caller) of grid cells per material id
 cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, MtCellPair* out, int nx, int ny, int nz,
                              unsigned long long* d_material_cells, cudaStream_t stream);
-cudaError_t mt_launch_debug_sample(int pack, const void* tab, uint32_t N, const uint32_t* words, uint64_t n,
-                                   uint32_t* out, cudaStream_t stream);
+cudaError_t mt_launch_debug_sample(int pack, bool joint, const void* tab, uint32_t N, const uint32_t* words,
+                                   uint64_t n, uint32_t* out, cudaStream_t stream);
 cudaError_t mt_launch_debug_philox(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,
                                    uint32_t* out, cudaStream_t stream);

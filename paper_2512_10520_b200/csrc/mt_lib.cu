@@ -43,6 +43,7 @@ struct mt_ctx {
   // histograms (host copies)
   bool have_hist = false, have_tables = false, have_geom = false;
   int32_t n_materials = 0, n_pbins = 0, n_dp = 0, n_th = 0;
+  int hist_mode = MT_HIST_MARGINAL;      // MT_HIST_JOINT: counts_dp / prob_dp / alias_dp hold n_dp * n_th cells per table
   float p_lo = 0, p_hi = 0;
   std::vector<float> counts_dp, counts_th, axis_dp, axis_th, step_m;
   // built tables (host, for mt_get_alias) and packed device copies
@@ -170,7 +171,8 @@ int rebuild_blob(mt_ctx* c) {
 // Pack the host tables (per (material, pbin): the Dp/p cells followed by the theta cells) with the material
 // blocks in the order c->mat_order, upload them, and record where each block starts.
 int upload_tables(mt_ctx* c) {
-  const int n_dp = c->n_dp, n_th = c->n_th, n_cells = n_dp + n_th;
+  const bool joint = (c->hist_mode == MT_HIST_JOINT);
+  const int n_dp = joint ? c->n_dp * c->n_th : c->n_dp, n_th = joint ? 0 : c->n_th, n_cells = n_dp + n_th;
   const size_t nt = (size_t)c->n_materials * c->n_pbins;
   const int wpc = (c->pack == 32) ? 1 : 2;                 // 32-bit words per cell
   std::vector<uint32_t> packed(nt * n_cells * wpc + 8, 0u);
@@ -288,13 +290,19 @@ int mt_set_option(mt_ctx* c, int option, int64_t value) {
 
 int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) {
   if (!c || !d) return MT_ERR_INVALID_ARG;
-  if (!d->counts_dp || !d->counts_th || !d->axis_dp || !d->axis_th || !d->step_m)
+  if (d->hist_mode != MT_HIST_MARGINAL && d->hist_mode != MT_HIST_JOINT) return fail(c, MT_ERR_INVALID_ARG, "bad hist_mode");
+  const bool joint = (d->hist_mode == MT_HIST_JOINT);
+  if (!d->counts_dp || (!joint && !d->counts_th) || !d->axis_dp || !d->axis_th || !d->step_m)
     return fail(c, MT_ERR_INVALID_ARG, "null histogram array");
   if (d->n_materials < 1 || d->n_materials > 255 || d->n_pbins < 1 || d->n_pbins > 4096 || d->n_dp < 1 ||
       d->n_dp > 65536 || d->n_th < 1 || d->n_th > 65536)
     return fail(c, MT_ERR_UNSUPPORTED, "histogram shape out of range");
-  if ((uint64_t)d->n_materials * d->n_pbins * ((uint64_t)d->n_dp + d->n_th) >= ((uint64_t)1 << 31))
+  const uint64_t cells_per_table = joint ? (uint64_t)d->n_dp * d->n_th : (uint64_t)d->n_dp + d->n_th;
+  if ((uint64_t)d->n_materials * d->n_pbins * cells_per_table >= ((uint64_t)1 << 31))
     return fail(c, MT_ERR_UNSUPPORTED, "more than 2^31 table cells");
+  // JOINT: 24-bit cell indices, and the kernel's exact cell / n_th by a 32-bit reciprocal needs cell * n_th < 2^32
+  if (joint && (cells_per_table > ((uint64_t)1 << 24) || cells_per_table * (uint64_t)d->n_th >= ((uint64_t)1 << 32)))
+    return fail(c, MT_ERR_UNSUPPORTED, "joint tables need n_dp * n_th <= 2^24 and n_dp * n_th^2 < 2^32");
   if ((uint64_t)d->n_materials * d->n_pbins > 4096)        // edges and axes live in shared memory (<= 80 KB)
     return fail(c, MT_ERR_UNSUPPORTED, "more than 4096 (material, momentum bin) tables");
   if (!(d->p_lo > 0.0f) || !(d->p_hi > d->p_lo) || isinf(d->p_hi))
@@ -314,8 +322,10 @@ int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) {
   const size_t nt = (size_t)d->n_materials * d->n_pbins;
   c->n_materials = d->n_materials; c->n_pbins = d->n_pbins; c->n_dp = d->n_dp; c->n_th = d->n_th;
   c->p_lo = d->p_lo; c->p_hi = d->p_hi;
-  c->counts_dp.assign(d->counts_dp, d->counts_dp + nt * d->n_dp);
-  c->counts_th.assign(d->counts_th, d->counts_th + nt * d->n_th);
+  c->hist_mode = d->hist_mode;
+  c->counts_dp.assign(d->counts_dp, d->counts_dp + nt * (joint ? cells_per_table : (uint64_t)d->n_dp));
+  if (joint) c->counts_th.clear();
+  else c->counts_th.assign(d->counts_th, d->counts_th + nt * d->n_th);
   c->axis_dp.assign(d->axis_dp, d->axis_dp + nt * 2);
   c->axis_th.assign(d->axis_th, d->axis_th + nt * 2);
   c->step_m.assign(d->step_m, d->step_m + d->n_materials + 1);
@@ -330,18 +340,19 @@ int mt_build_alias(mt_ctx* c, int placement) {
   if (placement < MT_PLACE_AUTO || placement > MT_PLACE_L2) return fail(c, MT_ERR_INVALID_ARG, "bad placement");
   DeviceGuard g(c->device);
   const size_t nt = (size_t)c->n_materials * c->n_pbins;
-  const int n_dp = c->n_dp, n_th = c->n_th;
+  const bool joint = (c->hist_mode == MT_HIST_JOINT);
+  const int n_dp = joint ? c->n_dp * c->n_th : c->n_dp, n_th = joint ? 0 : c->n_th;   // JOINT: one table of n_dp * n_th cells
   c->prob_dp.assign(nt * n_dp, 0.0f); c->alias_dp.assign(nt * n_dp, 0u);
   c->prob_th.assign(nt * n_th, 0.0f); c->alias_th.assign(nt * n_th, 0u);
   for (size_t t = 0; t < nt; ++t) {
     if (!build_one_alias(&c->counts_dp[t * n_dp], n_dp, &c->prob_dp[t * n_dp], &c->alias_dp[t * n_dp]))
-      return fail(c, MT_ERR_EMPTY_HIST, "Dp/p histogram of material %d, momentum bin %d is empty or invalid",
-                  (int)(t / c->n_pbins) + 1, (int)(t % c->n_pbins));
-    if (!build_one_alias(&c->counts_th[t * n_th], n_th, &c->prob_th[t * n_th], &c->alias_th[t * n_th]))
+      return fail(c, MT_ERR_EMPTY_HIST, "%s histogram of material %d, momentum bin %d is empty or invalid",
+                  joint ? "joint" : "Dp/p", (int)(t / c->n_pbins) + 1, (int)(t % c->n_pbins));
+    if (!joint && !build_one_alias(&c->counts_th[t * n_th], n_th, &c->prob_th[t * n_th], &c->alias_th[t * n_th]))
       return fail(c, MT_ERR_EMPTY_HIST, "theta histogram of material %d, momentum bin %d is empty or invalid",
                   (int)(t / c->n_pbins) + 1, (int)(t % c->n_pbins));
   }
-  c->pack = (std::max(n_dp, n_th) <= 256) ? 32 : 64;
+  c->pack = (!joint && std::max(n_dp, n_th) <= 256) ? 32 : 64;
   order_materials(c, std::vector<double>(c->n_materials + 1, 0.0));       // caller order until a geometry says otherwise
   int rc = upload_tables(c);
   if (rc != MT_OK) return rc;
@@ -351,12 +362,16 @@ int mt_build_alias(mt_ctx* c, int placement) {
 }
 
 int mt_get_alias(const mt_ctx* c, float* prob_dp, uint32_t* alias_dp, float* prob_th, uint32_t* alias_th) {
-  if (!c || !prob_dp || !alias_dp || !prob_th || !alias_th) return MT_ERR_INVALID_ARG;
+  if (!c || !prob_dp || !alias_dp) return MT_ERR_INVALID_ARG;
   if (!c->have_tables) return MT_ERR_STATE;
+  const bool joint = (c->hist_mode == MT_HIST_JOINT);
+  if (!joint && (!prob_th || !alias_th)) return MT_ERR_INVALID_ARG;
   memcpy(prob_dp, c->prob_dp.data(), c->prob_dp.size() * sizeof(float));
   memcpy(alias_dp, c->alias_dp.data(), c->alias_dp.size() * sizeof(uint32_t));
-  memcpy(prob_th, c->prob_th.data(), c->prob_th.size() * sizeof(float));
-  memcpy(alias_th, c->alias_th.data(), c->alias_th.size() * sizeof(uint32_t));
+  if (!joint) {
+    memcpy(prob_th, c->prob_th.data(), c->prob_th.size() * sizeof(float));
+    memcpy(alias_th, c->alias_th.data(), c->alias_th.size() * sizeof(uint32_t));
+  }
   return MT_OK;
 }
 
@@ -368,6 +383,10 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
     return fail(c, MT_ERR_INVALID_ARG, "empty world box");
   if (gm->max_steps < 0 || gm->world_material < 0 || gm->world_material > c->n_materials)
     return fail(c, MT_ERR_INVALID_ARG, "bad max_steps or world_material");
+  if (gm->field_mode < 0 || gm->field_mode > (MT_FIELD_NEAREST | MT_FIELD_PER_STAGE))
+    return fail(c, MT_ERR_INVALID_ARG, "bad field_mode");
+  if ((gm->field_mode & MT_FIELD_NEAREST) && gm->mode != MT_GEOM_VOXEL)
+    return fail(c, MT_ERR_INVALID_ARG, "MT_FIELD_NEAREST needs a voxel geometry");
   DeviceGuard g(c->device);
   std::vector<mt_region> regs;
   std::vector<double> weight(256, 0.0);                     // how much of the geometry each material fills
@@ -445,6 +464,11 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.gsy = g.nx + 2; P.gsz = (g.nx + 2) * (g.ny + 2);
   P.fnx = (float)g.nx; P.fny = (float)g.ny; P.fnz = (float)g.nz;
   P.n_materials = c->n_materials; P.n_pbins = c->n_pbins; P.n_dp = c->n_dp; P.n_th = c->n_th;
+  const bool joint = (c->hist_mode == MT_HIST_JOINT);
+  P.n_joint = joint ? (uint32_t)(c->n_dp * c->n_th) : 0u;
+  P.cells_per_bin = joint ? P.n_joint : (uint32_t)(c->n_dp + c->n_th);
+  P.nth_magic = (uint32_t)((((uint64_t)1 << 32) + (uint64_t)c->n_th - 1) / (uint64_t)c->n_th);   // n_th = 1 wraps to 0: unused then
+  P.field_mode = g.field_mode;
   P.inv_p_lo = 1.0f / c->p_lo;
   P.bin_scale = (float)((double)c->n_pbins / log2((double)c->p_hi / (double)c->p_lo));
   P.tab32 = (c->pack == 32) ? (const uint32_t*)c->d_tab.p : nullptr;
@@ -486,14 +510,18 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   MtLaunchCfg cfg;
   cfg.pack = c->pack;
   cfg.sched = sched;
+  cfg.joint = (c->hist_mode == MT_HIST_JOINT);
+  cfg.field = c->geom.field_mode;
   const size_t blob_b = ((blob_bytes(c) + 15) & ~(size_t)15);
   const size_t smem_budget = c->smem_optin;
   if (blob_b + 16 > smem_budget) return fail(c, MT_ERR_UNSUPPORTED, "edges, axes and regions (%zu B) do not fit in shared memory", blob_b);
   const size_t cell_b = (c->pack == 32) ? 4 : 8;
-  const size_t block_cells = (size_t)c->n_pbins * (c->n_dp + c->n_th);                // cells per material
+  const size_t block_cells = (size_t)c->n_pbins * P.cells_per_bin;                    // cells per material
   const size_t fit_blocks = std::min<size_t>((smem_budget - blob_b - 16) / (block_cells * cell_b), c->n_materials);
   size_t hot_blocks = 0;
-  if (c->placement == MT_PLACE_SMEM) {
+  if (cfg.joint) {                                           // joint tables are MBs per material: always gathered from L2
+    if (c->placement == MT_PLACE_SMEM) return fail(c, MT_ERR_UNSUPPORTED, "joint tables are not staged in shared memory");
+  } else if (c->placement == MT_PLACE_SMEM) {
     if (fit_blocks == 0) return fail(c, MT_ERR_UNSUPPORTED, "no material's tables (%zu B) fit in shared memory", block_cells * cell_b);
     hot_blocks = fit_blocks;
   } else if (c->placement == MT_PLACE_AUTO) {
@@ -657,10 +685,13 @@ int mt_debug_sample(mt_ctx* c, int material, int pbin, int which, const uint32_t
   if (material < 1 || material > c->n_materials || pbin < 0 || pbin >= c->n_pbins || which < 0 || which > 1)
     return fail(c, MT_ERR_INVALID_ARG, "bad table selector");
   DeviceGuard g(c->device);
-  const size_t cell = (size_t)c->mat_cell0[material] + (size_t)pbin * (c->n_dp + c->n_th) + (which ? c->n_dp : 0);
+  const bool joint = (c->hist_mode == MT_HIST_JOINT);
+  if (joint && which != 0) return fail(c, MT_ERR_INVALID_ARG, "joint tables have one table per (material, bin)");
+  const size_t per_bin = joint ? (size_t)c->n_dp * c->n_th : (size_t)(c->n_dp + c->n_th);
+  const size_t cell = (size_t)c->mat_cell0[material] + (size_t)pbin * per_bin + (which ? c->n_dp : 0);
   const char* tab = (const char*)c->d_tab.p + cell * (c->pack == 32 ? 4 : 8);
-  MT_CUDA(c, mt_launch_debug_sample(c->pack, tab, (uint32_t)(which ? c->n_th : c->n_dp), d_words, n, d_cell_out,
-                                    (cudaStream_t)cuda_stream));
+  const uint32_t N = joint ? (uint32_t)per_bin : (uint32_t)(which ? c->n_th : c->n_dp);
+  MT_CUDA(c, mt_launch_debug_sample(c->pack, joint, tab, N, d_words, n, d_cell_out, (cudaStream_t)cuda_stream));
   c->launches += 1;
   return MT_OK;
 }

@@ -47,6 +47,10 @@ struct MtParams {
   MtBlobLayout bl;
   uint32_t hot_cells;            // the first hot_cells cells of the packed tables are staged in shared memory
                                  // (whole material blocks; 0 = none)
+  uint32_t cells_per_bin;        // cells of one (material, momentum bin): n_dp + n_th, or n_dp * n_th in JOINT mode
+  uint32_t n_joint;              // JOINT mode: n_dp * n_th cells per table, pack64 cells
+  uint32_t nth_magic;            // ceil(2^32 / n_th): cell / n_th == umulhi(cell, nth_magic) for cell * n_th < 2^32
+  int32_t field_mode;            // MT_FIELD_*
   // ---- this call
   uint64_t n, id_base;
   uint32_t key0, key1;           // Philox key = seed lo, hi

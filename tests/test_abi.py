@@ -28,9 +28,9 @@ def test_library_exports_every_declared_symbol(mt):
 def test_struct_layouts_match_the_header(mt):
     b = mt.binding
     assert ctypes.sizeof(b.mt_region) == 40
-    assert ctypes.sizeof(b.mt_hist_desc) == 24 + 5 * 8
+    assert ctypes.sizeof(b.mt_hist_desc) == 24 + 5 * 8 + 8 and b.mt_hist_desc.hist_mode.offset == 64
     assert b.mt_geometry.regions.offset == 48 and b.mt_geometry.d_material.offset == 88
-    assert ctypes.sizeof(b.mt_geometry) == 104
+    assert ctypes.sizeof(b.mt_geometry) == 112 and b.mt_geometry.field_mode.offset == 104
     assert ctypes.sizeof(b.mt_muons_in) == 16 and ctypes.sizeof(b.mt_muons_out) == 48
     assert b.lib().mt_strerror(b.MT_ERR_EMPTY_HIST).decode().startswith("empty")
 
