@@ -100,18 +100,20 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ workload
-def make_workload(config, n_muons, device, rank):
+def make_workload(config, n_muons, device, rank, joint=False, field_mode=0):
     """BASELINE.json configs[config] with this rank's batch of muons (generator batch = rank)."""
     from paper_2512_10520_b200 import workloads as w
     t0 = time.time()
     if config == 3:
-        wl = w.config3(n=8, device=device)                       # histograms + voxel grids (made on the GPU)
+        wl = w.config3(n=8, device=device, joint=joint, field_mode=field_mode)   # histograms + voxel grids (made on the GPU)
         wl.muons = w.spectrum_muons(3, n_muons, "square", batch=rank)
     elif config == 2:
-        wl = w.config2(n=8)
+        wl = w.config2(n=8, joint=joint)
+        wl.geom.field_mode = field_mode & 2
         wl.muons = w.spectrum_muons(2, n_muons, "square", batch=rank)
     elif config == 1:
-        wl = w.config1(n=8)
+        wl = w.config1(n=8, joint=joint)
+        wl.geom.field_mode = field_mode & 2
         wl.muons = w.spectrum_muons(1, n_muons, "gauss", batch=rank)
     else:
         raise SystemExit("bench.py times configs 1, 2 and 3 (config 0 is the oracle-sized parity case)")
@@ -149,7 +151,7 @@ def run_reference(args, rank, world):
         return
     import torch
     dev = "cuda" if torch.cuda.is_available() else "cpu"          # the grid generator may use the GPU; the timed code never does
-    wl = make_workload(args.config, args.muons, dev, 0)
+    wl = make_workload(args.config, args.muons, dev, 0, args.joint, args.field_mode)
     cores, desc, runner = oracle_sample(wl, args.muons, 0, args.ref_seconds)
     for _ in range(args.warmup):
         runner()
@@ -191,7 +193,7 @@ def run_ours(args, rank, world, local_rank):
     from paper_2512_10520_b200.sharding import reduce_job, weak_shard
     shard = weak_shard(args.muons, rank, world)               # own batch, own id range, no collective
     n, id_base = shard.n, shard.id_base
-    wl = make_workload(args.config, n, dev, rank)
+    wl = make_workload(args.config, n, dev, rank, args.joint, args.field_mode)
     mode = "voxel" if wl.geom.mode == 1 else "regions"
     h = b.MuonTransport(local_rank).setup(wl.hist, wl.geom, args.placement)
     h.set_option(b.MT_OPT_SCHEDULE, args.sched).set_option(b.MT_OPT_BLOCK_THREADS, args.block)
@@ -283,7 +285,8 @@ def run_ours(args, rank, world, local_rank):
         "muons_per_s": muons_all * args.steps / t_dev_max,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_dev_max / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": wl.name, "muons_per_gpu": n, "muon_steps_per_gpu_step": steps_per_call,
+        "config": {"workload": wl.name + ("+joint2d" if args.joint else "") + ("+field_mode%d" % args.field_mode if args.field_mode else ""),
+                   "muons_per_gpu": n, "muon_steps_per_gpu_step": steps_per_call,
                    "schedule": args.sched, "placement": args.placement, "block": args.block, "slab_cells": args.slab,
                    "parallelism": "id-range sharding x%d, replicated tables and grids, no collective" % world,
                    "l2": "inputs larger than L2 (320 MB muon state, 1.9 GB field grid per step)",
@@ -407,6 +410,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-seconds", type=float, default=15.0, help="CPU work per oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--joint", action="store_true", help="the paper's joint 2D histograms (DESIGN.md 3.10) instead of two 1D ones")
+    ap.add_argument("--field-mode", type=int, default=0, help="MT_FIELD_*: 1 nearest, 2 per-stage, 3 both (DESIGN.md 3.11)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
     ap.add_argument("--sweep-batches", type=int, default=10)
     ap.add_argument("--sweep-draws", type=int, default=1_000_000, help="draws per generated histogram")
