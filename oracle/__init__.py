@@ -17,6 +17,10 @@ REGION_DTYPE = np.dtype([("z_lo", "<f4"), ("z_hi", "<f4"), ("x_lo", "<f4"), ("x_
                          ("y_lo", "<f4"), ("y_hi", "<f4"), ("material", "<i4"),
                          ("bx", "<f4"), ("by", "<f4"), ("bz", "<f4")])
 
+# vertex i of the lower face is joined to vertex i of the upper face
+POLY_DTYPE = np.dtype([("z_lo", "<f4"), ("z_hi", "<f4"), ("xy_lo", "<f4", (4, 2)), ("xy_hi", "<f4", (4, 2)),
+                       ("material", "<i4"), ("bx", "<f4"), ("by", "<f4"), ("bz", "<f4")])
+
 
 class _Geometry(C.Structure):
     _fields_ = [("mode", C.c_int32),
@@ -26,7 +30,8 @@ class _Geometry(C.Structure):
                 ("n_regions", C.c_int32), ("regions", C.c_void_p),
                 ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("ox", C.c_float), ("oy", C.c_float), ("oz", C.c_float), ("cell", C.c_float),
-                ("material", C.c_void_p), ("field", C.c_void_p), ("field_mode", C.c_int32)]
+                ("material", C.c_void_p), ("field", C.c_void_p), ("field_mode", C.c_int32),
+                ("n_blocks", C.c_int32), ("blocks", C.c_void_p)]
 
 
 class _Tables(C.Structure):
@@ -228,6 +233,10 @@ class OracleGeometry:
         s.material = self.material.ctypes.data if self.material is not None else None
         s.field = self.field.ctypes.data if self.field is not None else None
         s.field_mode = int(getattr(g, "field_mode", 0))
+        blocks = getattr(g, "blocks", None)
+        self.blocks = _c(blocks, POLY_DTYPE) if blocks is not None else np.zeros(0, POLY_DTYPE)
+        s.n_blocks = len(self.blocks)
+        s.blocks = self.blocks.ctypes.data if len(self.blocks) else None
         self.struct = s
 
 

@@ -18,6 +18,8 @@
 //   termination ............... L65, L149
 //   joint 2D histogram mode ... L77 (§3), Fig. 3 L95, L163
 //   nearest-neighbour field ... L133 (§4.3); per-stage field evaluation: Eq. 4 integrated by RK4 proper
+//   convex-polyhedra lookup ... L109-120 (§4.1), Eq. 2; the spatial hash of L120 only prunes, so the
+//                               oracle scans every block
 //
 // Two modes from one templated source: Real=float is the parity reference (every + - * is one
 // IEEE binary32 operation in the written order, fma where DESIGN.md says fma; compile with
@@ -29,7 +31,8 @@
 // the paper's worked example (118.47-128.48 GeV); straight line; helix; RK4 h^4 convergence;
 // Rodrigues (Eq. 3) in double; trilinear on affine fields; region lookup vs brute force;
 // exp2/sin/cos polynomials vs libm; two-word alias draw vs the exact pmf of the table; joint-mode kick vs its
-// geometry; nearest field vs the stored cell values; per-stage push vs h^4 convergence in a field gradient.  Physics fidelity vs Geant4 (Figs. 5, 7): parity unpinned
+// geometry; nearest field vs the stored cell values; per-stage push vs h^4 convergence in a field gradient;
+// polyhedra containment vs scipy's convex hull of the eight vertices, the prismatoid volume, and the box regions.  Physics fidelity vs Geant4 (Figs. 5, 7): parity unpinned
 // (needs Geant4 histograms, not available).
 
 #include <cmath>
@@ -209,8 +212,11 @@ template <class R> void sincos_polar(R theta, R* sn, R* cs) {
 // ------------------------------------------------------------------------------------------------
 struct Region { float z_lo, z_hi, x_lo, x_hi, y_lo, y_hi; int32_t material; float bx, by, bz; };
 
+// the solid between two quadrilateral faces, vertex i of the lower face joined to vertex i of the upper
+struct PolyBlock { float z_lo, z_hi; float xy_lo[4][2]; float xy_hi[4][2]; int32_t material; float bx, by, bz; };
+
 struct Geometry {
-  int32_t mode;                 // 0 = regions, 1 = voxel
+  int32_t mode;                 // 0 = regions, 1 = voxel, 2 = convex polyhedra
   float x_min, x_max, y_min, y_max, z_min, z_exit;
   float p_min; int32_t max_steps; int32_t world_material;
   int32_t n_regions; const Region* regions;
@@ -218,6 +224,7 @@ struct Geometry {
   const uint8_t* material;      // [nz][ny][nx]
   const float* field;           // [nz][ny][nx][3]
   int32_t field_mode;           // bit 0: nearest-neighbour instead of trilinear; bit 1: field at every RK4 stage
+  int32_t n_blocks; const PolyBlock* blocks;   // mode 2
 };
 enum { FIELD_NEAREST = 1, FIELD_PER_STAGE = 2 };
 
@@ -289,11 +296,50 @@ void trilinear(const Geometry& g, R x, R y, R z, R B[3]) {
   }
 }
 
+// PAPER.md L111-120, Eq. 2; DESIGN.md §3.12.  The quadrilateral slice of the block at height z, then the sign of
+// S_i = (e_i x (p - v_i))_z for each of its four edges.
+template <class R>
+bool poly_contains(const PolyBlock& b, R x, R y, R z) {
+  if (!((R)b.z_lo <= z && z < (R)b.z_hi)) return false;
+  const R inv_dz = rrcp<R>((R)b.z_hi - (R)b.z_lo);
+  const R t = (z - (R)b.z_lo) * inv_dz;
+  R vx[4], vy[4];
+  for (int i = 0; i < 4; ++i) {
+    vx[i] = rfma<R>(t, (R)b.xy_hi[i][0] - (R)b.xy_lo[i][0], (R)b.xy_lo[i][0]);
+    vy[i] = rfma<R>(t, (R)b.xy_hi[i][1] - (R)b.xy_lo[i][1], (R)b.xy_lo[i][1]);
+  }
+  bool all_ge = true, all_le = true, any_gt = false, any_lt = false;
+  for (int i = 0; i < 4; ++i) {
+    const int j = (i + 1) % 4;
+    const R ex = vx[j] - vx[i], ey = vy[j] - vy[i];
+    const R S = rfma<R>(ex, y - vy[i], -(ey * (x - vx[i])));
+    all_ge = all_ge && (S >= (R)0);
+    all_le = all_le && (S <= (R)0);
+    any_gt = any_gt || (S > (R)0);
+    any_lt = any_lt || (S < (R)0);
+  }
+  return (all_ge && any_gt) || (all_le && any_lt);
+}
+
+// first block, in index order, that contains the point (no pruning: L120's spatial hash only saves time)
+template <class R>
+void poly_lookup(const Geometry& g, R x, R y, R z, int* material, R B[3]) {
+  *material = g.world_material; B[0] = B[1] = B[2] = (R)0;
+  for (int j = 0; j < g.n_blocks; ++j) {
+    if (poly_contains<R>(g.blocks[j], x, y, z)) {
+      const PolyBlock& b = g.blocks[j];
+      *material = b.material; B[0] = (R)b.bx; B[1] = (R)b.by; B[2] = (R)b.bz;
+      return;
+    }
+  }
+}
+
 // material and field at a position (Alg. 1 l.5 and l.12 both use r before the move).  Field of a voxel grid:
 // trilinear (BASELINE configs[3]) or, the stored value of the containing cell.
 template <class R>
 void material_and_field(const Geometry& g, R x, R y, R z, int* material, R B[3]) {
   if (g.mode == 0) { region_lookup<R>(g, x, y, z, material, B); return; }
+  if (g.mode == 2) { poly_lookup<R>(g, x, y, z, material, B); return; }
   int ix, iy, iz;
   if (!voxel_cell<R>(g, x, y, z, &ix, &iy, &iz)) {
     *material = g.world_material; B[0] = B[1] = B[2] = (R)0; return;

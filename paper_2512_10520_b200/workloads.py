@@ -17,7 +17,11 @@ REGION_DTYPE = np.dtype([("z_lo", "<f4"), ("z_hi", "<f4"), ("x_lo", "<f4"), ("x_
                          ("y_lo", "<f4"), ("y_hi", "<f4"), ("material", "<i4"),
                          ("bx", "<f4"), ("by", "<f4"), ("bz", "<f4")])
 
-MODE_REGIONS, MODE_VOXEL = 0, 1
+# convex-polyhedra block: two quadrilateral faces, vertex i joined to vertex i
+POLY_DTYPE = np.dtype([("z_lo", "<f4"), ("z_hi", "<f4"), ("xy_lo", "<f4", (4, 2)), ("xy_hi", "<f4", (4, 2)),
+                       ("material", "<i4"), ("bx", "<f4"), ("by", "<f4"), ("bz", "<f4")])
+
+MODE_REGIONS, MODE_VOXEL, MODE_POLY = 0, 1, 2
 FIELD_TRILINEAR, FIELD_NEAREST, FIELD_PER_STAGE = 0, 1, 2
 
 # material -> (density g/cm3, radiation length cm); BASELINE.json configs[0], configs[2]
@@ -66,6 +70,7 @@ class Geometry:
     material: object = None             # uint8 [nz][ny][nx], numpy or torch (any device)
     field: object = None                # float32 [nz][ny][nx][3]
     field_mode: int = 0                 # FIELD_NEAREST | FIELD_PER_STAGE; 0 = trilinear, frozen
+    blocks: np.ndarray = None           # POLY_DTYPE (MODE_POLY); the first block that contains a point wins
 
 
 @dataclass
@@ -269,6 +274,53 @@ def config2(n=1_000_000, n_draws=1_000_000, n_cells=8, joint=False, table_shape=
     geom = Geometry(MODE_REGIONS, -1.0, 1.0, -1.0, 1.0, 0.0, z_exit, 1.0, 6000, 3,
                     regions=shield_regions(n_cells))
     return Workload("config2_multi_region_shield", hist, geom, spectrum_muons(2, n, "square"), seed=1)
+
+
+def regions_as_blocks(regions):
+    """The same boxes written as polyhedra blocks (rectangular faces, counter-clockwise)."""
+    out = np.zeros(len(regions), POLY_DTYPE)
+    for b, r in zip(out, regions):
+        rect = [(r["x_lo"], r["y_lo"]), (r["x_hi"], r["y_lo"]), (r["x_hi"], r["y_hi"]), (r["x_lo"], r["y_hi"])]
+        b["z_lo"], b["z_hi"], b["xy_lo"], b["xy_hi"] = r["z_lo"], r["z_hi"], rect, rect
+        b["material"], b["bx"], b["by"], b["bz"] = r["material"], r["bx"], r["by"], r["bz"]
+    return out
+
+
+def shield_polyhedra(n_cells=8):
+    """A tapered-magnet shield in the shape of the paper's own geometry ("a sequence of
+    magnets composed of iron blocks ... walls made of concrete"): per 3.75 m cell an iron core whose half-width in x
+    tapers 0.25 -> 0.45 m (even cells) or 0.45 -> 0.25 m (odd cells) and whose half-height tapers 0.5 -> 0.6 m,
+    By = +/-1.7 T alternating; two iron return yokes beside it (from 2 cm outside the core to twice its width) with the
+    opposite field; a 0.5 m concrete wall (full xy).  Air is the world material.  The -x yokes are listed clockwise, the
+    rest counter-clockwise.  Materials: 1 iron, 2 concrete, 3 air."""
+    blocks = []
+
+    def quad(x0, x1, y0, y1, clockwise=False):
+        q = [(x0, y0), (x1, y0), (x1, y1), (x0, y1)]
+        return q[::-1] if clockwise else q
+
+    for c in range(n_cells):
+        z0 = 3.75 * c
+        by = 1.7 if c % 2 == 0 else -1.7
+        w = (0.25, 0.45) if c % 2 == 0 else (0.45, 0.25)
+        hh = (0.5, 0.6)
+        gap = 0.02
+        blocks.append((z0, z0 + 2.75, quad(-w[0], w[0], -hh[0], hh[0]), quad(-w[1], w[1], -hh[1], hh[1]), 1, 0.0, by, 0.0))
+        blocks.append((z0, z0 + 2.75, quad(w[0] + gap, 2 * w[0] + gap, -hh[0], hh[0]),
+                       quad(w[1] + gap, 2 * w[1] + gap, -hh[1], hh[1]), 1, 0.0, -by, 0.0))
+        blocks.append((z0, z0 + 2.75, quad(-2 * w[0] - gap, -w[0] - gap, -hh[0], hh[0], True),
+                       quad(-2 * w[1] - gap, -w[1] - gap, -hh[1], hh[1], True), 1, 0.0, -by, 0.0))
+        blocks.append((z0 + 3.0, z0 + 3.5, quad(-1.0, 1.0, -1.0, 1.0), quad(-1.0, 1.0, -1.0, 1.0), 2, 0.0, 0.0, 0.0))
+    return np.array(blocks, POLY_DTYPE)
+
+
+def config2p(n=1_000_000, n_draws=1_000_000, n_cells=8, joint=False, table_shape=(100, 256, 128), field_mode=0):
+    """Polyhedral shield: config 2's muons and histograms in the tapered-magnet geometry of
+    shield_polyhedra(), looked up with the paper's slice + Eq. 2 test."""
+    hist = shield_histograms(2, [2.0, 2.0, 2.0], table_shape[0], table_shape[1], table_shape[2], n_draws, joint=joint)
+    geom = Geometry(MODE_POLY, -1.0, 1.0, -1.0, 1.0, 0.0, 3.75 * n_cells, 1.0, 6000, 3,
+                    blocks=shield_polyhedra(n_cells), field_mode=field_mode)
+    return Workload("config2p_polyhedral_shield", hist, geom, spectrum_muons(2, n, "square"), seed=1)
 
 
 def config3(n=10_000_000, n_draws=1_000_000, n_cells=8, half_width_cells=100, device="cpu", hist=None,
