@@ -28,11 +28,11 @@ if ROOT not in sys.path:
 
 # algorithmic thread-operations and gathered bytes per muon-step (contract operations of
 # DESIGN.md §3 counted one each; loads not counted as operations)
-ALG_OPS_PER_STEP = {"voxel": 383, "regions": 308}
-ALG_GATHER_BYTES_PER_STEP = {"voxel": 168, "regions": 40}
+ALG_OPS_PER_STEP = {"voxel": 383, "regions": 308, "poly": 349}
+ALG_GATHER_BYTES_PER_STEP = {"voxel": 168, "regions": 40, "poly": 50}
 # DRAM bytes (read + written) of ONE launch of the dominant kernel, from the `ncu --set full` capture summarised in
 # profiles/r1c_transport_kernel_full.csv (mean of the three captured z-slab passes of config 3)
-NCU_DRAM_BYTES_PER_LAUNCH = {"voxel": 0.756e9, "regions": None}
+NCU_DRAM_BYTES_PER_LAUNCH = {"voxel": 0.756e9, "regions": None, "poly": None}
 SM_COUNT, LANES_PER_SM = 148, 128          # B200: 4 SMSPs x 32 lanes issue one warp instruction per clock
 
 
@@ -100,7 +100,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ workload
-def make_workload(config, n_muons, device, rank, joint=False, field_mode=0):
+def make_workload(config, n_muons, device, rank, joint=False, field_mode=0, poly=False):
     """BASELINE.json configs[config] with this rank's batch of muons (generator batch = rank)."""
     from paper_2512_10520_b200 import workloads as w
     t0 = time.time()
@@ -108,7 +108,8 @@ def make_workload(config, n_muons, device, rank, joint=False, field_mode=0):
         wl = w.config3(n=8, device=device, joint=joint, field_mode=field_mode)   # histograms + voxel grids (made on the GPU)
         wl.muons = w.spectrum_muons(3, n_muons, "square", batch=rank)
     elif config == 2:
-        wl = w.config2(n=8, joint=joint)
+        # --poly: config 2's muons and tables in the tapered-magnet polyhedra geometry
+        wl = w.config2p(n=8, joint=joint) if poly else w.config2(n=8, joint=joint)
         wl.geom.field_mode = field_mode & 2
         wl.muons = w.spectrum_muons(2, n_muons, "square", batch=rank)
     elif config == 1:
@@ -151,7 +152,7 @@ def run_reference(args, rank, world):
         return
     import torch
     dev = "cuda" if torch.cuda.is_available() else "cpu"          # the grid generator may use the GPU; the timed code never does
-    wl = make_workload(args.config, args.muons, dev, 0, args.joint, args.field_mode)
+    wl = make_workload(args.config, args.muons, dev, 0, args.joint, args.field_mode, args.poly)
     cores, desc, runner = oracle_sample(wl, args.muons, 0, args.ref_seconds)
     for _ in range(args.warmup):
         runner()
@@ -193,8 +194,8 @@ def run_ours(args, rank, world, local_rank):
     from paper_2512_10520_b200.sharding import reduce_job, weak_shard
     shard = weak_shard(args.muons, rank, world)               # own batch, own id range, no collective
     n, id_base = shard.n, shard.id_base
-    wl = make_workload(args.config, n, dev, rank, args.joint, args.field_mode)
-    mode = "voxel" if wl.geom.mode == 1 else "regions"
+    wl = make_workload(args.config, n, dev, rank, args.joint, args.field_mode, args.poly)
+    mode = {0: "regions", 1: "voxel", 2: "poly"}[wl.geom.mode]
     h = b.MuonTransport(local_rank).setup(wl.hist, wl.geom, args.placement)
     h.set_option(b.MT_OPT_SCHEDULE, args.sched).set_option(b.MT_OPT_BLOCK_THREADS, args.block)
     h.set_option(b.MT_OPT_SLAB_CELLS, args.slab).set_option(b.MT_OPT_REFILL_MIN_IDLE, args.min_idle)
@@ -412,6 +413,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--joint", action="store_true", help="the paper's joint 2D histograms (DESIGN.md 3.10) instead of two 1D ones")
     ap.add_argument("--field-mode", type=int, default=0, help="MT_FIELD_*: 1 nearest, 2 per-stage, 3 both (DESIGN.md 3.11)")
+    ap.add_argument("--poly", action="store_true", help="with --config 2: the convex-polyhedra shield (DESIGN.md 3.12)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
     ap.add_argument("--sweep-batches", type=int, default=10)
     ap.add_argument("--sweep-draws", type=int, default=1_000_000, help="draws per generated histogram")

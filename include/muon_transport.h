@@ -40,7 +40,11 @@ enum {
 /* termination flags written to the outputs (Alg. 1 l.2-4, L148-151) */
 enum { MT_FLAG_STOPPED = 1, MT_FLAG_EXITED = 2, MT_FLAG_ESCAPED = 3, MT_FLAG_MAXSTEPS = 4 };
 
-enum { MT_GEOM_REGIONS = 0, MT_GEOM_VOXEL = 1 };
+enum {
+  MT_GEOM_REGIONS = 0,     /* axis-aligned boxes found through a sorted z-interval table (BASELINE.json configs[0-2])      */
+  MT_GEOM_VOXEL = 1,       /* uint8 material grid + float32x3 field grid (configs[3-4])                                    */
+  MT_GEOM_POLY = 2         /* the paper's own: convex polyhedra, slice + Eq. 2 sign test, spatial-hash pruning (L109-120)  */
+};
 
 /* what the histograms hold (mt_hist_desc.hist_mode) */
 enum {
@@ -73,8 +77,11 @@ enum {
   MT_OPT_BLOCKS_PER_SM = 3,  /* 0 = library default (persistent kernels)                                   */
   MT_OPT_SLAB_CELLS = 4,     /* wavefront: slab thickness along z, in units of 1 cm; 0 = default           */
   MT_OPT_REFILL_MIN_IDLE = 5,/* refill: lanes of a warp that must be idle before it refills; 0 = default   */
-  MT_OPT_KEY_LOOKAHEAD = 6   /* wavefront: the sort key is the xy cell a muon reaches after this many percent */
+  MT_OPT_KEY_LOOKAHEAD = 6,  /* wavefront: the sort key is the xy cell a muon reaches after this many percent */
                              /* of a slab on a straight line; -1 = default (50), 0 = its current cell         */
+  MT_OPT_HASH_NXY = 7,       /* POLY: cells of the spatial hash along x and along y; 0 = default (16); 1..256 */
+  MT_OPT_HASH_NZ = 8         /* POLY: cells of the spatial hash along z; 0 = default (256); 1..4096.  Both    */
+                             /* take effect at the next mt_set_geometry; results never depend on them         */
 };
 
 const char* mt_strerror(int code);
@@ -120,8 +127,22 @@ typedef struct {
   float bx, by, bz;        /* uniform field inside the box                                                 */
 } mt_region;
 
+/* One convex block of MT_GEOM_POLY (§4.1): the solid between a lower
+ * quadrilateral face at z_lo and an upper one at z_hi, vertex i of one joined to vertex i of the other.  The four
+ * vertices go round the face in either orientation (the same for both faces); each face must be convex; a
+ * repeated vertex gives a triangle, four equal vertices an apex.  A point is inside if z_lo <= z < z_hi and the
+ * cross products S_i of Eq. 2 against the four edges of the slice interpolated at its z have one sign (zeros
+ * allowed, not all zero).  Where blocks overlap the one with the lowest index wins. */
 typedef struct {
-  int32_t mode;            /* MT_GEOM_REGIONS | MT_GEOM_VOXEL                                              */
+  float z_lo, z_hi;
+  float xy_lo[4][2];       /* (x, y) of the lower face's vertices                                          */
+  float xy_hi[4][2];       /* (x, y) of the upper face's vertices                                          */
+  int32_t material;
+  float bx, by, bz;        /* uniform field inside the block                                               */
+} mt_poly_block;
+
+typedef struct {
+  int32_t mode;            /* MT_GEOM_REGIONS | MT_GEOM_VOXEL | MT_GEOM_POLY                               */
   float x_min, x_max, y_min, y_max, z_min, z_exit; /* world box; z >= z_exit -> EXITED                    */
   float p_min;             /* |p| < p_min -> STOPPED                                                       */
   int32_t max_steps;       /* step cap -> MAXSTEPS                                                         */
@@ -133,6 +154,9 @@ typedef struct {
   const uint8_t* d_material; /* DEVICE [nz][ny][nx], read during the call only                            */
   const float* d_field;      /* DEVICE [nz][ny][nx][3], read during the call only                         */
   int32_t field_mode;        /* MT_FIELD_TRILINEAR | MT_FIELD_NEAREST, optionally | MT_FIELD_PER_STAGE             */
+  int32_t n_blocks;          /* POLY mode: 0..1024                                                           */
+  const mt_poly_block* blocks; /* HOST, copied.  The library bins their bounding boxes into a uniform grid  */
+                             /* over the world box (the spatial hash of L120) and tests only a cell's candidates */
 } mt_geometry;
 /* VOXEL mode repacks both grids into one library-owned 16-byte-per-cell grid {Bx,By,Bz,material}
  * (DESIGN.md §6), so the caller may free d_material / d_field after the call returns. */
@@ -177,6 +201,11 @@ int mt_debug_sample(mt_ctx* ctx, int material, int pbin, int which, const uint32
                     uint32_t* d_cell_out, void* cuda_stream);
 int mt_debug_philox(mt_ctx* ctx, uint64_t seed, uint64_t id_base, uint32_t step, uint64_t n,
                     uint32_t* d_out, void* cuda_stream);
+/* mt_debug_lookup: material_out[i] and field_out[i][0..2] = the material id and the field the step loop sees at the
+ * point d_xyz[i][0..2] in the geometry that is set — regions, voxel (trilinear or
+ * nearest per field_mode) or polyhedra (through the spatial hash). */
+int mt_debug_lookup(mt_ctx* ctx, const float* d_xyz, uint64_t n, int32_t* d_material_out, float* d_field_out,
+                    void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -13,18 +13,18 @@ LIB_PATH = os.path.join(HERE, "libmuon_transport.so")
 MT_OK = 0
 MT_ERR_INVALID_ARG, MT_ERR_STATE, MT_ERR_EMPTY_HIST, MT_ERR_UNSUPPORTED, MT_ERR_CUDA, MT_ERR_NOMEM = -1, -2, -3, -4, -5, -6
 MT_FLAG_STOPPED, MT_FLAG_EXITED, MT_FLAG_ESCAPED, MT_FLAG_MAXSTEPS = 1, 2, 3, 4
-MT_GEOM_REGIONS, MT_GEOM_VOXEL = 0, 1
+MT_GEOM_REGIONS, MT_GEOM_VOXEL, MT_GEOM_POLY = 0, 1, 2
 MT_PLACE_AUTO, MT_PLACE_SMEM, MT_PLACE_L2 = 0, 1, 2
 MT_SCHED_AUTO, MT_SCHED_STATIC, MT_SCHED_REFILL, MT_SCHED_WAVEFRONT = 0, 1, 2, 3
 MT_OPT_SCHEDULE, MT_OPT_BLOCK_THREADS, MT_OPT_BLOCKS_PER_SM, MT_OPT_SLAB_CELLS, MT_OPT_REFILL_MIN_IDLE = 1, 2, 3, 4, 5
-MT_OPT_KEY_LOOKAHEAD = 6
+MT_OPT_KEY_LOOKAHEAD, MT_OPT_HASH_NXY, MT_OPT_HASH_NZ = 6, 7, 8
 MT_HIST_MARGINAL, MT_HIST_JOINT = 0, 1
 MT_FIELD_TRILINEAR, MT_FIELD_NEAREST, MT_FIELD_PER_STAGE = 0, 1, 2
 
 # every symbol include/muon_transport.h declares (tests check that the library exports each one)
 SYMBOLS = ["mt_strerror", "mt_last_error", "mt_create", "mt_destroy", "mt_set_option", "mt_load_histograms",
            "mt_build_alias", "mt_get_alias", "mt_set_geometry", "mt_transport", "mt_transport_host",
-           "mt_launch_count", "mt_debug_sample", "mt_debug_philox"]
+           "mt_launch_count", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
 
 
 class mt_hist_desc(C.Structure):
@@ -40,6 +40,11 @@ class mt_region(C.Structure):
                 ("bx", C.c_float), ("by", C.c_float), ("bz", C.c_float)]
 
 
+class mt_poly_block(C.Structure):
+    _fields_ = [("z_lo", C.c_float), ("z_hi", C.c_float), ("xy_lo", C.c_float * 2 * 4), ("xy_hi", C.c_float * 2 * 4),
+                ("material", C.c_int32), ("bx", C.c_float), ("by", C.c_float), ("bz", C.c_float)]
+
+
 class mt_geometry(C.Structure):
     _fields_ = [("mode", C.c_int32),
                 ("x_min", C.c_float), ("x_max", C.c_float), ("y_min", C.c_float), ("y_max", C.c_float),
@@ -48,7 +53,8 @@ class mt_geometry(C.Structure):
                 ("n_regions", C.c_int32), ("regions", C.c_void_p),
                 ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("ox", C.c_float), ("oy", C.c_float), ("oz", C.c_float), ("cell", C.c_float),
-                ("d_material", C.c_void_p), ("d_field", C.c_void_p), ("field_mode", C.c_int32)]
+                ("d_material", C.c_void_p), ("d_field", C.c_void_p), ("field_mode", C.c_int32),
+                ("n_blocks", C.c_int32), ("blocks", C.c_void_p)]
 
 
 class mt_muons_in(C.Structure):
@@ -89,6 +95,7 @@ def lib():
         L.mt_launch_count.argtypes = [C.c_void_p]
         L.mt_debug_sample.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_philox.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p]
+        L.mt_debug_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -179,6 +186,12 @@ def mt_set_geometry(ctx, geom):
         keep = regs
         g.n_regions = len(regs)
         g.regions = regs.ctypes.data if len(regs) else None
+    elif geom.mode == MT_GEOM_POLY:
+        blocks = np.ascontiguousarray(geom.blocks) if geom.blocks is not None else np.zeros(0, np.uint8)
+        assert blocks.size == 0 or blocks.dtype.itemsize == C.sizeof(mt_poly_block)
+        keep = blocks
+        g.n_blocks = len(blocks)
+        g.blocks = blocks.ctypes.data if len(blocks) else None
     else:
         import torch
         mat, fld = geom.material, geom.field
@@ -272,6 +285,18 @@ def mt_debug_sample(ctx, material, pbin, which, words, stream=None, joint=False)
     _check(ctx, lib().mt_debug_sample(ctx, material, pbin, which, words.data_ptr(), n, out.data_ptr(),
                                       _stream_ptr(stream)))
     return out
+
+
+def mt_debug_lookup(ctx, xyz, stream=None):
+    """xyz: float32 CUDA tensor [n,3] -> (material int32 [n], field float32 [n,3]) as the step loop looks them up"""
+    import torch
+    xyz = xyz.contiguous()
+    assert xyz.is_cuda and xyz.dtype == torch.float32 and xyz.shape[-1] == 3
+    n = xyz.shape[0]
+    mat = torch.empty(n, dtype=torch.int32, device=xyz.device)
+    fld = torch.empty((n, 3), dtype=torch.float32, device=xyz.device)
+    _check(ctx, lib().mt_debug_lookup(ctx, xyz.data_ptr(), n, mat.data_ptr(), fld.data_ptr(), _stream_ptr(stream)))
+    return mat, fld
 
 
 def mt_debug_philox(ctx, seed, id_base, step, n, device="cuda", stream=None):

@@ -9,6 +9,7 @@
 //              cell column at the same z, so its eight field-corner gathers fall into one or two cache lines
 //              instead of 32, and the slab's few z-layers of the 1.9 GB grid stay L1/L2-resident.
 #include <cuda_runtime.h>
+#include <algorithm>
 #include <stdint.h>
 #include "mt_launch.h"
 #include "mt_step.cuh"
@@ -34,6 +35,7 @@ MT_DEV View<PACK> stage_view(const MtParams& P) {
   V.axes = reinterpret_cast<const float4*>(sblob + P.bl.off_axes);
   V.zlo = sblob + P.bl.off_zlo;
   V.regions = reinterpret_cast<const MtRegionDev*>(sblob + P.bl.off_regions);
+  V.blocks = reinterpret_cast<const MtBlockDev*>(sblob + P.bl.off_blocks);
   const uint32_t* gtab = (PACK == 32) ? P.tab32 : reinterpret_cast<const uint32_t*>(P.tab64);
   V.tab = reinterpret_cast<const typename Tab<PACK>::cell_t*>(gtab);
   uint4* stab = reinterpret_cast<uint4*>(sblob + ((P.bl.n_words + 3) & ~3));
@@ -385,6 +387,23 @@ __global__ void debug_sample_joint_kernel(const uint2* tab, uint32_t N, const ui
   out[i] = ((words[n + i] >> 8) < e.x) ? k : e.y;
 }
 
+// test hook: material and field at arbitrary points through the same lookups as the step loop
+template <int GEOM, bool NEAREST>
+__global__ void __launch_bounds__(256) debug_lookup_kernel(const __grid_constant__ MtParams P, const float* __restrict__ xyz,
+                                                           uint64_t n, int32_t* __restrict__ mat_out, float* __restrict__ b_out) {
+  const View<32> V = stage_view<32, false>(P);
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    const float x = xyz[3 * i], y = xyz[3 * i + 1], z = xyz[3 * i + 2];
+    int material;
+    float bx, by, bz;
+    if (GEOM == 0) lookup_regions<32>(P, V, x, y, z, material, bx, by, bz);
+    else if (GEOM == 2) lookup_poly<32>(P, V, x, y, z, material, bx, by, bz);
+    else lookup_voxel<NEAREST, true>(P, x, y, z, material, bx, by, bz);
+    mat_out[i] = material;
+    b_out[3 * i] = bx; b_out[3 * i + 1] = by; b_out[3 * i + 2] = bz;
+  }
+}
+
 typedef void (*kernel_fn)(const MtParams);
 
 // Instantiated combinations: geometry x table kind {pack32, pack32 + shared prefix, pack64, pack64 + shared prefix,
@@ -407,6 +426,7 @@ kernel_fn pick_tables(const MtLaunchCfg& cfg) {
 }
 kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
   if (mode == 0) return (cfg.field & 2) ? pick_tables<0, 2>(cfg) : pick_tables<0, 0>(cfg);
+  if (mode == 2) return (cfg.field & 2) ? pick_tables<2, 2>(cfg) : pick_tables<2, 0>(cfg);
   switch (cfg.field & 3) {
     case 1: return pick_tables<1, 1>(cfg);
     case 2: return pick_tables<1, 2>(cfg);
@@ -470,6 +490,20 @@ cudaError_t mt_launch_debug_sample(int pack, bool joint, const void* tab, uint32
   if (joint) debug_sample_joint_kernel<<<grid, 256, 0, stream>>>((const uint2*)tab, N, words, n, out);
   else if (pack == 32) debug_sample_kernel<32><<<grid, 256, 0, stream>>>((const uint32_t*)tab, N, words, n, out);
   else debug_sample_kernel<64><<<grid, 256, 0, stream>>>((const uint2*)tab, N, words, n, out);
+  return cudaGetLastError();
+}
+
+cudaError_t mt_launch_debug_lookup(const MtParams& P, size_t smem_bytes, const float* xyz, uint64_t n, int32_t* mat_out,
+                                   float* b_out, cudaStream_t stream) {
+  if (n == 0) return cudaSuccess;
+  typedef void (*fn_t)(const MtParams, const float*, uint64_t, int32_t*, float*);
+  fn_t fn = (P.mode == 0) ? debug_lookup_kernel<0, false>
+          : (P.mode == 2) ? debug_lookup_kernel<2, false>
+          : (P.field_mode & 1) ? debug_lookup_kernel<1, true> : debug_lookup_kernel<1, false>;
+  cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+  if (e != cudaSuccess) return e;
+  const unsigned grid = (unsigned)std::min<uint64_t>((n + 255) / 256, 148 * 8);
+  fn<<<grid, 256, smem_bytes, stream>>>(P, xyz, n, mat_out, b_out);
   return cudaGetLastError();
 }
 

@@ -33,5 +33,7 @@ cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, MtCellPair* o
                              unsigned long long* d_material_cells, cudaStream_t stream);
 cudaError_t mt_launch_debug_sample(int pack, bool joint, const void* tab, uint32_t N, const uint32_t* words,
                                    uint64_t n, uint32_t* out, cudaStream_t stream);
+cudaError_t mt_launch_debug_lookup(const MtParams& P, size_t smem_bytes, const float* xyz, uint64_t n, int32_t* mat_out,
+                                   float* b_out, cudaStream_t stream);
 cudaError_t mt_launch_debug_philox(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,
                                    uint32_t* out, cudaStream_t stream);

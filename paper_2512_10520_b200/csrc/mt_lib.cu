@@ -54,10 +54,15 @@ struct mt_ctx {
   size_t table_bytes = 0;
   std::vector<int> mat_order;        // material ids, most-used first: the order of their blocks in the packed tables
   std::vector<uint32_t> mat_cell0;   // [n_materials + 1] first cell of material m's block in the packed tables
-  DevBuf d_tab, d_blob, d_grid, d_scratch, d_wave, d_stage_in, d_stage_out, d_stage_misc;
+  DevBuf d_tab, d_blob, d_grid, d_scratch, d_wave, d_stage_in, d_stage_out, d_stage_misc, d_hash;
+  int opt_hash_nxy = 0, opt_hash_nz = 0;
   // geometry
   mt_geometry geom{};
   std::vector<mt_region> regions;
+  std::vector<mt_poly_block> blocks;     // POLY mode
+  int hnx = 0, hny = 0, hnz = 0;         // spatial hash
+  float h_inv[3] = {0, 0, 0};
+  size_t hash_list_off = 0;              // byte offset of the candidate lists inside d_hash
   MtBlobLayout bl{};
   int64_t launches = 0;
 };
@@ -138,7 +143,9 @@ int rebuild_blob(mt_ctx* c) {
   bl.off_axes = bl.off_steps + 4 * (c->n_materials + 1);
   bl.off_zlo = bl.off_axes + 4 * nt;
   bl.off_regions = (bl.off_zlo + n_reg + 3) & ~3;
-  bl.n_words = bl.off_regions + 10 * n_reg;
+  const int n_blk = c->have_geom ? (int)c->blocks.size() : 0;
+  bl.off_blocks = (bl.off_regions + 10 * n_reg + 3) & ~3;
+  bl.n_words = bl.off_blocks + 24 * n_blk;
   std::vector<float> blob((size_t)bl.n_words + 4, 0.0f);
   const double lo = (double)c->p_lo, hi = (double)c->p_hi;
   for (int j = 0; j <= c->n_pbins; ++j)
@@ -161,6 +168,22 @@ int rebuild_blob(mt_ctx* c) {
     blob[bl.off_zlo + j] = c->regions[j].z_lo;
     static_assert(sizeof(mt_region) == 40 && sizeof(MtRegionDev) == 40, "region layout");
     memcpy(&blob[bl.off_regions + 10 * j], &c->regions[j], sizeof(mt_region));
+  }
+  for (int j = 0; j < n_blk; ++j) {
+    // §3.12: the per-block constants of the slice interpolation, each ONE float32 operation
+    static_assert(sizeof(MtBlockDev) == 96, "block layout");
+    const mt_poly_block& b = c->blocks[j];
+    MtBlockDev d;
+    d.z_lo = b.z_lo; d.z_hi = b.z_hi;
+    const volatile float dz = b.z_hi - b.z_lo;
+    d.inv_dz = 1.0f / dz;
+    d.material = b.material; d.bx = b.bx; d.by = b.by; d.bz = b.bz; d.pad = 0.0f;
+    for (int i = 0; i < 4; ++i) {
+      d.xl[i] = b.xy_lo[i][0]; d.yl[i] = b.xy_lo[i][1];
+      const volatile float dx = b.xy_hi[i][0] - b.xy_lo[i][0], dy = b.xy_hi[i][1] - b.xy_lo[i][1];
+      d.dx[i] = dx; d.dy[i] = dy;
+    }
+    memcpy(&blob[bl.off_blocks + 24 * j], &d, sizeof d);
   }
   c->bl = bl;
   MT_CUDA(c, c->d_blob.reserve(blob.size() * sizeof(float)));
@@ -213,6 +236,95 @@ void order_materials(mt_ctx* c, const std::vector<double>& weight) {
   std::stable_sort(c->mat_order.begin(), c->mat_order.end(), [&](int a, int b) { return weight[a] > weight[b]; });
 }
 
+// POLY mode: validate the blocks and bin their padded bounding boxes into a uniform grid over the
+// world box — the spatial hash of PAPER.md L120.  The hash only prunes: a point's cell (computed on the device in
+// float32, clamped into the grid) must list every block that the float32 containment test could accept for that
+// point, so each box is grown by a pad that dwarfs float32 rounding (1e-4 of the largest coordinate + 0.1 mm, against
+// 2^-22 relative) and cell ranges are taken with the device's own float32 scale factors.
+int build_hash(mt_ctx* c, const mt_geometry* gm, const std::vector<mt_poly_block>& blks, std::vector<double>& weight) {
+  const int hnx = c->opt_hash_nxy ? c->opt_hash_nxy : 16, hny = hnx, hnz = c->opt_hash_nz ? c->opt_hash_nz : 256;
+  const double w_lo[3] = {gm->x_min, gm->y_min, gm->z_min};
+  const double w_ext[3] = {(double)gm->x_max - gm->x_min, (double)gm->y_max - gm->y_min, (double)gm->z_exit - gm->z_min};
+  const int hn[3] = {hnx, hny, hnz};
+  float inv[3];
+  for (int a = 0; a < 3; ++a) inv[a] = (float)((double)hn[a] / w_ext[a]);
+  double world = w_ext[0] * w_ext[1] * w_ext[2];
+  auto area2 = [](const double q[4][2]) {                   // twice the signed area (shoelace)
+    double s = 0.0;
+    for (int i = 0; i < 4; ++i) { const int j = (i + 1) & 3; s += q[i][0] * q[j][1] - q[j][0] * q[i][1]; }
+    return s;
+  };
+  std::vector<int> range(blks.size() * 6);
+  std::vector<uint32_t> count((size_t)hnx * hny * hnz + 1, 0u);
+  for (size_t j = 0; j < blks.size(); ++j) {
+    const mt_poly_block& b = blks[j];
+    if (!(b.z_lo < b.z_hi) || !std::isfinite(b.z_lo) || !std::isfinite(b.z_hi)) return fail(c, MT_ERR_INVALID_ARG, "block %zu: empty z range", j);
+    if (b.material < 0 || b.material > c->n_materials) return fail(c, MT_ERR_INVALID_ARG, "block %zu: bad material", j);
+    double lo[3] = {INFINITY, INFINITY, b.z_lo}, hi[3] = {-INFINITY, -INFINITY, b.z_hi}, big = std::max(fabs(b.z_lo), fabs(b.z_hi));
+    double face[3][4][2];                                   // lower, upper, middle
+    int orient = 0;
+    for (int f = 0; f < 2; ++f) {
+      const float (*v)[2] = f ? b.xy_hi : b.xy_lo;
+      for (int i = 0; i < 4; ++i) {
+        if (!std::isfinite(v[i][0]) || !std::isfinite(v[i][1])) return fail(c, MT_ERR_INVALID_ARG, "block %zu: non-finite vertex", j);
+        face[f][i][0] = v[i][0]; face[f][i][1] = v[i][1];
+        lo[0] = std::min(lo[0], (double)v[i][0]); hi[0] = std::max(hi[0], (double)v[i][0]);
+        lo[1] = std::min(lo[1], (double)v[i][1]); hi[1] = std::max(hi[1], (double)v[i][1]);
+      }
+      // convex: the turns at the four corners have one sign; both faces go round the same way
+      int pos = 0, neg = 0;
+      for (int i = 0; i < 4; ++i) {
+        const int i1 = (i + 1) & 3, i2 = (i + 2) & 3;
+        const double ax = face[f][i1][0] - face[f][i][0], ay = face[f][i1][1] - face[f][i][1];
+        const double bx = face[f][i2][0] - face[f][i1][0], by = face[f][i2][1] - face[f][i1][1];
+        const double cr = ax * by - ay * bx;
+        pos += cr > 0; neg += cr < 0;
+      }
+      if (pos && neg) return fail(c, MT_ERR_INVALID_ARG, "block %zu: %s face is not convex", j, f ? "upper" : "lower");
+      const int o = pos ? 1 : (neg ? -1 : 0);
+      if (o && orient && o != orient) return fail(c, MT_ERR_INVALID_ARG, "block %zu: faces listed in opposite orientations", j);
+      if (o) orient = o;
+    }
+    for (int a = 0; a < 2; ++a) big = std::max(big, std::max(fabs(lo[a]), fabs(hi[a])));
+    for (int a = 0; a < 3; ++a) big = std::max(big, std::max(fabs(w_lo[a]), fabs(w_lo[a] + w_ext[a])));
+    const double pad = 1e-4 * big + 1e-4;
+    for (int a = 0; a < 3; ++a) {
+      const double c_lo = floor((lo[a] - pad - w_lo[a]) * (double)inv[a]), c_hi = floor((hi[a] + pad - w_lo[a]) * (double)inv[a]);
+      range[6 * j + 2 * a] = (int)std::min(std::max(c_lo, 0.0), (double)(hn[a] - 1));
+      range[6 * j + 2 * a + 1] = (int)std::min(std::max(c_hi, 0.0), (double)(hn[a] - 1));
+    }
+    for (int z = range[6 * j + 4]; z <= range[6 * j + 5]; ++z)
+      for (int y = range[6 * j + 2]; y <= range[6 * j + 3]; ++y)
+        for (int x = range[6 * j]; x <= range[6 * j + 1]; ++x) count[((size_t)z * hny + y) * hnx + x] += 1;
+    // volume (Simpson over z is exact for linearly moving vertices), for the table order only
+    for (int i = 0; i < 4; ++i) for (int k = 0; k < 2; ++k) face[2][i][k] = 0.5 * (face[0][i][k] + face[1][i][k]);
+    const double vol = ((double)b.z_hi - b.z_lo) / 12.0 * (fabs(area2(face[0])) + 4.0 * fabs(area2(face[2])) + fabs(area2(face[1])));
+    weight[b.material] += vol;
+    world -= vol;
+  }
+  weight[gm->world_material] += std::max(world, 0.0);
+  const size_t n_cells = (size_t)hnx * hny * hnz;
+  std::vector<uint32_t> first(n_cells + 1, 0u);
+  for (size_t k = 0; k < n_cells; ++k) first[k + 1] = first[k] + count[k];
+  const size_t n_list = first[n_cells];
+  std::vector<uint16_t> list(n_list + 8, 0);
+  std::vector<uint32_t> fill(first.begin(), first.end() - 1);
+  for (size_t j = 0; j < blks.size(); ++j)                   // ascending j: every list ends up in index order
+    for (int z = range[6 * j + 4]; z <= range[6 * j + 5]; ++z)
+      for (int y = range[6 * j + 2]; y <= range[6 * j + 3]; ++y)
+        for (int x = range[6 * j]; x <= range[6 * j + 1]; ++x) list[fill[((size_t)z * hny + y) * hnx + x]++] = (uint16_t)j;
+  std::vector<uint2> cells(n_cells);
+  for (size_t k = 0; k < n_cells; ++k) cells[k] = make_uint2(first[k], count[k]);
+  const size_t list_off = (n_cells * sizeof(uint2) + 255) & ~(size_t)255;
+  MT_CUDA(c, c->d_hash.reserve(list_off + list.size() * sizeof(uint16_t)));
+  MT_CUDA(c, cudaMemcpy(c->d_hash.p, cells.data(), n_cells * sizeof(uint2), cudaMemcpyHostToDevice));
+  MT_CUDA(c, cudaMemcpy((char*)c->d_hash.p + list_off, list.data(), list.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+  c->hnx = hnx; c->hny = hny; c->hnz = hnz;
+  c->h_inv[0] = inv[0]; c->h_inv[1] = inv[1]; c->h_inv[2] = inv[2];
+  c->hash_list_off = list_off;
+  return MT_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -256,7 +368,7 @@ int mt_destroy(mt_ctx* c) {
   if (!c) return MT_OK;
   DeviceGuard g(c->device);
   DevBuf* bufs[] = {&c->d_tab, &c->d_blob, &c->d_grid, &c->d_scratch, &c->d_wave,
-                    &c->d_stage_in, &c->d_stage_out, &c->d_stage_misc};
+                    &c->d_stage_in, &c->d_stage_out, &c->d_stage_misc, &c->d_hash};
   for (DevBuf* b : bufs) b->release();
   delete c;
   return MT_OK;
@@ -284,6 +396,12 @@ int mt_set_option(mt_ctx* c, int option, int64_t value) {
     case MT_OPT_REFILL_MIN_IDLE:
       if (value < 0 || value > 32) return fail(c, MT_ERR_INVALID_ARG, "bad refill threshold");
       c->opt_min_idle = (int)value; return MT_OK;
+    case MT_OPT_HASH_NXY:
+      if (value < 0 || value > 256) return fail(c, MT_ERR_INVALID_ARG, "bad hash resolution");
+      c->opt_hash_nxy = (int)value; return MT_OK;
+    case MT_OPT_HASH_NZ:
+      if (value < 0 || value > 4096) return fail(c, MT_ERR_INVALID_ARG, "bad hash resolution");
+      c->opt_hash_nz = (int)value; return MT_OK;
     default: return fail(c, MT_ERR_INVALID_ARG, "unknown option %d", option);
   }
 }
@@ -378,7 +496,8 @@ int mt_get_alias(const mt_ctx* c, float* prob_dp, uint32_t* alias_dp, float* pro
 int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
   if (!c || !gm) return MT_ERR_INVALID_ARG;
   if (!c->have_tables) return fail(c, MT_ERR_STATE, "mt_set_geometry before mt_build_alias");
-  if (gm->mode != MT_GEOM_REGIONS && gm->mode != MT_GEOM_VOXEL) return fail(c, MT_ERR_INVALID_ARG, "bad geometry mode");
+  if (gm->mode != MT_GEOM_REGIONS && gm->mode != MT_GEOM_VOXEL && gm->mode != MT_GEOM_POLY)
+    return fail(c, MT_ERR_INVALID_ARG, "bad geometry mode");
   if (!(gm->x_min < gm->x_max) || !(gm->y_min < gm->y_max) || !(gm->z_min < gm->z_exit))
     return fail(c, MT_ERR_INVALID_ARG, "empty world box");
   if (gm->max_steps < 0 || gm->world_material < 0 || gm->world_material > c->n_materials)
@@ -389,8 +508,15 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
     return fail(c, MT_ERR_INVALID_ARG, "MT_FIELD_NEAREST needs a voxel geometry");
   DeviceGuard g(c->device);
   std::vector<mt_region> regs;
+  std::vector<mt_poly_block> blks;
   std::vector<double> weight(256, 0.0);                     // how much of the geometry each material fills
-  if (gm->mode == MT_GEOM_REGIONS) {
+  if (gm->mode == MT_GEOM_POLY) {
+    if (gm->n_blocks < 0 || gm->n_blocks > 1024) return fail(c, MT_ERR_UNSUPPORTED, "0..1024 blocks supported");
+    if (gm->n_blocks > 0 && !gm->blocks) return fail(c, MT_ERR_INVALID_ARG, "null block array");
+    blks.assign(gm->blocks, gm->blocks + gm->n_blocks);
+    const int rc = build_hash(c, gm, blks, weight);
+    if (rc != MT_OK) return rc;
+  } else if (gm->mode == MT_GEOM_REGIONS) {
     if (gm->n_regions < 0 || gm->n_regions > 1024) return fail(c, MT_ERR_UNSUPPORTED, "0..1024 regions supported");
     if (gm->n_regions > 0 && !gm->regions) return fail(c, MT_ERR_INVALID_ARG, "null region array");
     regs.assign(gm->regions, gm->regions + gm->n_regions);
@@ -432,8 +558,11 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
   }
   c->geom = *gm;
   c->geom.regions = nullptr; c->geom.d_material = nullptr; c->geom.d_field = nullptr;
+  c->geom.blocks = nullptr;
   c->regions.swap(regs);
+  c->blocks.swap(blks);
   c->geom.n_regions = (int32_t)c->regions.size();
+  c->geom.n_blocks = (int32_t)c->blocks.size();
   c->have_geom = true;
   // the most-used materials come first in the packed tables, so that a shared-memory prefix holds them
   order_materials(c, weight);
@@ -469,6 +598,11 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.cells_per_bin = joint ? P.n_joint : (uint32_t)(c->n_dp + c->n_th);
   P.nth_magic = (uint32_t)((((uint64_t)1 << 32) + (uint64_t)c->n_th - 1) / (uint64_t)c->n_th);   // n_th = 1 wraps to 0: unused then
   P.field_mode = g.field_mode;
+  P.n_blocks = g.n_blocks;
+  P.hash_cells = (const uint2*)c->d_hash.p;
+  P.hash_list = (const uint16_t*)((const char*)c->d_hash.p + c->hash_list_off);
+  P.hnx = c->hnx; P.hny = c->hny; P.hnz = c->hnz;
+  P.h_inv_x = c->h_inv[0]; P.h_inv_y = c->h_inv[1]; P.h_inv_z = c->h_inv[2];
   P.inv_p_lo = 1.0f / c->p_lo;
   P.bin_scale = (float)((double)c->n_pbins / log2((double)c->p_hi / (double)c->p_lo));
   P.tab32 = (c->pack == 32) ? (const uint32_t*)c->d_tab.p : nullptr;
@@ -499,7 +633,9 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   P.counters = (unsigned long long*)out->counters;
 
   int sched = c->opt_sched;
-  if (sched == MT_SCHED_AUTO) sched = (c->geom.mode == MT_GEOM_VOXEL) ? MT_SCHED_WAVEFRONT : MT_SCHED_REFILL;
+  // POLY: muons sorted by xy cell and advanced slab by slab share a hash cell and its candidate blocks, so a warp's
+  // containment tests stay convergent: 53.0 against 42.0 G muon-steps/s under REFILL (profiles/r1g_poly.md)
+  if (sched == MT_SCHED_AUTO) sched = (c->geom.mode == MT_GEOM_REGIONS) ? MT_SCHED_REFILL : MT_SCHED_WAVEFRONT;
   P.refill_min_idle = c->opt_min_idle ? c->opt_min_idle : 1;
 
   // Table placement (north_star subsystem 1).  The packed tables start with the most-used material; shared
@@ -692,6 +828,20 @@ int mt_debug_sample(mt_ctx* c, int material, int pbin, int which, const uint32_t
   const char* tab = (const char*)c->d_tab.p + cell * (c->pack == 32 ? 4 : 8);
   const uint32_t N = joint ? (uint32_t)per_bin : (uint32_t)(which ? c->n_th : c->n_dp);
   MT_CUDA(c, mt_launch_debug_sample(c->pack, joint, tab, N, d_words, n, d_cell_out, (cudaStream_t)cuda_stream));
+  c->launches += 1;
+  return MT_OK;
+}
+
+int mt_debug_lookup(mt_ctx* c, const float* d_xyz, uint64_t n, int32_t* d_material_out, float* d_field_out,
+                    void* cuda_stream) {
+  if (!c || !d_xyz || !d_material_out || !d_field_out) return MT_ERR_INVALID_ARG;
+  if (!c->have_geom) return fail(c, MT_ERR_STATE, "mt_debug_lookup before mt_set_geometry");
+  DeviceGuard g(c->device);
+  MtParams P;
+  fill_params(c, P);
+  const size_t smem = ((blob_bytes(c) + 15) & ~(size_t)15) + 16;
+  if (smem > c->smem_optin) return fail(c, MT_ERR_UNSUPPORTED, "const blob (%zu B) does not fit in shared memory", smem);
+  MT_CUDA(c, mt_launch_debug_lookup(P, smem, d_xyz, n, d_material_out, d_field_out, (cudaStream_t)cuda_stream));
   c->launches += 1;
   return MT_OK;
 }

@@ -17,8 +17,18 @@ struct MtRegionDev {
 //   [off_axes + 4*t .. +3]               lo_dp, d_dp * 2^-16, lo_th, d_th * 2^-16 (log2) of table t = (m-1)*n_pbins + i
 //   [off_zlo  + j]                       z_lo of region j (search array)
 //   [off_regions + 10*j ..]              MtRegionDev j
+//   [off_blocks + 24*j ..]               MtBlockDev j (POLY mode)
 struct MtBlobLayout {
-  int32_t off_steps, off_axes, off_zlo, off_regions, n_words;
+  int32_t off_steps, off_axes, off_zlo, off_regions, off_blocks, n_words;
+};
+
+// Polyhedra block as staged in shared memory: six float4.  inv_dz = 1 / (z_hi - z_lo), dx_i = xh_i - xl_i and
+// dy_i = yh_i - yl_i are the float32 operations of DESIGN.md §3.12, done once on the host.
+struct __align__(16) MtBlockDev {
+  float z_lo, z_hi, inv_dz;
+  int32_t material;
+  float bx, by, bz, pad;
+  float xl[4], yl[4], dx[4], dy[4];
 };
 
 // Two x-neighbours of the padded field grid in one 32-byte record, so that the x-pair of a trilinear corner set
@@ -51,6 +61,13 @@ struct MtParams {
   uint32_t n_joint;              // JOINT mode: n_dp * n_th cells per table, pack64 cells
   uint32_t nth_magic;            // ceil(2^32 / n_th): cell / n_th == umulhi(cell, nth_magic) for cell * n_th < 2^32
   int32_t field_mode;            // MT_FIELD_*
+  // ---- POLY mode: spatial hash over the world box; a cell lists, in ascending order, the blocks whose
+  //      padded bounding box meets it
+  int32_t n_blocks;
+  const uint2* hash_cells;       // [hnz][hny][hnx] = {first entry in hash_list, number of candidates}
+  const uint16_t* hash_list;     // block indices
+  int32_t hnx, hny, hnz;
+  float h_inv_x, h_inv_y, h_inv_z;   // cells per metre along each axis
   // ---- this call
   uint64_t n, id_base;
   uint32_t key0, key1;           // Philox key = seed lo, hi
