@@ -199,7 +199,7 @@ def run_ours(args, rank, world, local_rank):
     h = b.MuonTransport(local_rank).setup(wl.hist, wl.geom, args.placement)
     h.set_option(b.MT_OPT_SCHEDULE, args.sched).set_option(b.MT_OPT_BLOCK_THREADS, args.block)
     h.set_option(b.MT_OPT_SLAB_CELLS, args.slab).set_option(b.MT_OPT_REFILL_MIN_IDLE, args.min_idle)
-    h.set_option(b.MT_OPT_BLOCKS_PER_SM, args.blocks_per_sm)
+    h.set_option(b.MT_OPT_BLOCKS_PER_SM, args.blocks_per_sm).set_option(b.MT_OPT_NO_LEAN, int(args.no_lean))
     host_geom = None
     if rank == 0 and not args.no_cpu_baseline:
         import copy
@@ -413,6 +413,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--joint", action="store_true", help="the paper's joint 2D histograms (DESIGN.md 3.10) instead of two 1D ones")
     ap.add_argument("--field-mode", type=int, default=0, help="MT_FIELD_*: 1 nearest, 2 per-stage, 3 both (DESIGN.md 3.11)")
+    ap.add_argument("--no-lean", action="store_true", help="MT_OPT_NO_LEAN: general kernels even where the lean variant applies")
     ap.add_argument("--poly", action="store_true", help="with --config 2: the convex-polyhedra shield (DESIGN.md 3.12)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
     ap.add_argument("--sweep-batches", type=int, default=10)

@@ -80,8 +80,10 @@ enum {
   MT_OPT_KEY_LOOKAHEAD = 6,  /* wavefront: the sort key is the xy cell a muon reaches after this many percent */
                              /* of a slab on a straight line; -1 = default (50), 0 = its current cell         */
   MT_OPT_HASH_NXY = 7,       /* POLY: cells of the spatial hash along x and along y; 0 = default (16); 1..256 */
-  MT_OPT_HASH_NZ = 8         /* POLY: cells of the spatial hash along z; 0 = default (256); 1..4096.  Both    */
+  MT_OPT_HASH_NZ = 8,        /* POLY: cells of the spatial hash along z; 0 = default (256); 1..4096.  Both    */
                              /* take effect at the next mt_set_geometry; results never depend on them         */
+  MT_OPT_NO_LEAN = 9         /* 1: never take the kernel variants that drop operations the host has proven to  */
+                             /* be identities for the loaded tables and geometry; for testing    */
 };
 
 const char* mt_strerror(int code);
@@ -191,6 +193,14 @@ int mt_transport_host(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t i
 
 /* Number of kernel launches made by this context so far (bench.py's gpu_launches). */
 int64_t mt_launch_count(const mt_ctx* ctx);
+
+/* Introspection for tests and bench.py: *value = the item `what` of the context. */
+enum {
+  MT_INFO_LEAN_FACTS = 1,  /* bit 0: table axes proven inside the clamps; bit 1: world box proven inside the voxel grid   */
+  MT_INFO_LAST_LEAN = 2,   /* 1 if the last mt_transport call ran the lean kernel variant                                */
+  MT_INFO_LAST_SCHEDULE = 3/* MT_SCHED_* the last mt_transport call ran under                                            */
+};
+int mt_get_info(const mt_ctx* ctx, int what, int64_t* value);
 
 /* Test hooks (DEVICE buffers, asynchronous on the stream).
  * mt_debug_sample: cell_out[i] = alias draw from table `which` (0 = Dp/p, 1 = theta) of

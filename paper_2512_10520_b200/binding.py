@@ -17,14 +17,15 @@ MT_GEOM_REGIONS, MT_GEOM_VOXEL, MT_GEOM_POLY = 0, 1, 2
 MT_PLACE_AUTO, MT_PLACE_SMEM, MT_PLACE_L2 = 0, 1, 2
 MT_SCHED_AUTO, MT_SCHED_STATIC, MT_SCHED_REFILL, MT_SCHED_WAVEFRONT = 0, 1, 2, 3
 MT_OPT_SCHEDULE, MT_OPT_BLOCK_THREADS, MT_OPT_BLOCKS_PER_SM, MT_OPT_SLAB_CELLS, MT_OPT_REFILL_MIN_IDLE = 1, 2, 3, 4, 5
-MT_OPT_KEY_LOOKAHEAD, MT_OPT_HASH_NXY, MT_OPT_HASH_NZ = 6, 7, 8
+MT_OPT_KEY_LOOKAHEAD, MT_OPT_HASH_NXY, MT_OPT_HASH_NZ, MT_OPT_NO_LEAN = 6, 7, 8, 9
 MT_HIST_MARGINAL, MT_HIST_JOINT = 0, 1
+MT_INFO_LEAN_FACTS, MT_INFO_LAST_LEAN, MT_INFO_LAST_SCHEDULE = 1, 2, 3
 MT_FIELD_TRILINEAR, MT_FIELD_NEAREST, MT_FIELD_PER_STAGE = 0, 1, 2
 
 # every symbol include/muon_transport.h declares (tests check that the library exports each one)
 SYMBOLS = ["mt_strerror", "mt_last_error", "mt_create", "mt_destroy", "mt_set_option", "mt_load_histograms",
            "mt_build_alias", "mt_get_alias", "mt_set_geometry", "mt_transport", "mt_transport_host",
-           "mt_launch_count", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
+           "mt_launch_count", "mt_get_info", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
 
 
 class mt_hist_desc(C.Structure):
@@ -93,6 +94,7 @@ def lib():
                                          C.POINTER(mt_muons_out), C.c_void_p]
         L.mt_launch_count.restype = C.c_int64
         L.mt_launch_count.argtypes = [C.c_void_p]
+        L.mt_get_info.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]
         L.mt_debug_sample.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_philox.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -273,6 +275,14 @@ def _host_ptr(a):
 
 def mt_launch_count(ctx):
     return int(lib().mt_launch_count(ctx))
+
+
+def mt_get_info(ctx, what):
+    v = C.c_int64(0)
+    rc = lib().mt_get_info(ctx, what, C.byref(v))
+    if rc != MT_OK:
+        raise MtError(rc, "mt_get_info")
+    return int(v.value)
 
 
 def mt_debug_sample(ctx, material, pbin, which, words, stream=None, joint=False):

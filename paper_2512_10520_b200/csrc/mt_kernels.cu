@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(256) wave_scatter_kernel(const __grid_constant
   }
 }
 
-template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD>
+template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD, bool LEAN = false>
 __global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
 wave_transport_kernel(const __grid_constant__ MtParams P) {
   const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
@@ -282,12 +282,12 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
     int flag = -1;                                    // -1: no muon on this lane
     m.x = m.y = m.z = m.q = m.px = m.py = m.pz = 0.0f;
     m.step = 0;
-    if (item < n_items) {
+      if (item < n_items) {
       const float4 a = P.s_pos_q[item], b = P.s_mom_step[item];
       idx = P.s_idx[item];
       m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z;
       m.step = __float_as_int(b.w);
-      flag = 0;
+        flag = 0;
     }
     const uint64_t id = P.id_base + idx;
     const uint32_t id_lo = (uint32_t)id, id_hi = (uint32_t)(id >> 32);
@@ -295,7 +295,7 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
 
     // ---- step until every lane has terminated or reached the end of the slab
     for (;;) {
-      if (flag == 0) flag = step_once<GEOM, PACK, TAB_SMEM, true, JOINT, FIELD>(P, V, m, id_lo, id_hi, P.slab_z_end);
+      if (flag == 0) flag = step_once<GEOM, PACK, TAB_SMEM, true, JOINT, FIELD, true, LEAN>(P, V, m, id_lo, id_hi, P.slab_z_end);
       if (!__any_sync(kFull, flag == 0)) break;
     }
     tally.steps += (unsigned)(m.step - step_in);
@@ -425,6 +425,8 @@ kernel_fn pick_tables(const MtLaunchCfg& cfg) {
                       : pick_sched<GEOM, 64, false, false, FIELD>(cfg.sched);
 }
 kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
+  if (cfg.lean && mt_has_lean(mode, cfg))
+    return (cfg.pack == 32) ? wave_transport_kernel<1, 32, false, false, 0, true> : wave_transport_kernel<1, 64, false, false, 0, true>;
   if (mode == 0) return (cfg.field & 2) ? pick_tables<0, 2>(cfg) : pick_tables<0, 0>(cfg);
   if (mode == 2) return (cfg.field & 2) ? pick_tables<2, 2>(cfg) : pick_tables<2, 0>(cfg);
   switch (cfg.field & 3) {
@@ -436,6 +438,10 @@ kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
 }
 
 }  // namespace
+
+bool mt_has_lean(int mode, const MtLaunchCfg& cfg) {
+  return mode == 1 && cfg.sched == SCHED_WAVEFRONT && !cfg.joint && !cfg.tab_smem && (cfg.field & 3) == 0;
+}
 
 // ------------------------------------------------------------------------------------------------
 // launchers (called from mt_lib.cu)

@@ -19,7 +19,11 @@ struct MtLaunchCfg {
   int sched;       // MT_SCHED_STATIC / _REFILL / _WAVEFRONT
   bool joint;      // MT_HIST_JOINT tables (pack64, never staged)
   int field;       // MT_FIELD_* of the geometry
+  bool lean;       // P.lean == MT_LEAN_ALL and a LEAN kernel exists for this combination (mt_has_lean)
 };
+// LEAN variants are compiled for the hot combination only: voxel geometry, marginal tables in L2, trilinear frozen
+// field, WAVEFRONT schedule
+bool mt_has_lean(int mode, const MtLaunchCfg& cfg);
 
 cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream);
 cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm);

@@ -55,7 +55,9 @@ struct mt_ctx {
   std::vector<int> mat_order;        // material ids, most-used first: the order of their blocks in the packed tables
   std::vector<uint32_t> mat_cell0;   // [n_materials + 1] first cell of material m's block in the packed tables
   DevBuf d_tab, d_blob, d_grid, d_scratch, d_wave, d_stage_in, d_stage_out, d_stage_misc, d_hash;
-  int opt_hash_nxy = 0, opt_hash_nz = 0;
+  int opt_hash_nxy = 0, opt_hash_nz = 0, opt_no_lean = 0;
+  float lean_box[6] = {0, 0, 0, 0, 0, 0};        // x_lo, x_hi, y_lo, y_hi, z_lo, z_hi of MT_LEAN_INSIDE
+  bool lean_axes = false, lean_inside = false;   // MT_LEAN_* facts (mt_params.h), proven in rebuild_blob / mt_set_geometry
   // geometry
   mt_geometry geom{};
   std::vector<mt_region> regions;
@@ -65,6 +67,7 @@ struct mt_ctx {
   size_t hash_list_off = 0;              // byte offset of the candidate lists inside d_hash
   MtBlobLayout bl{};
   int64_t launches = 0;
+  int last_lean = 0, last_sched = 0;
 };
 
 namespace {
@@ -158,12 +161,21 @@ int rebuild_blob(mt_ctx* c) {
     const int32_t cell0 = (int32_t)c->mat_cell0[m];
     memcpy(&blob[bl.off_steps + 4 * m + 3], &cell0, sizeof cell0);
   }
+  bool axes_ok = (c->hist_mode == MT_HIST_MARGINAL);
   for (int t = 0; t < nt; ++t) {
     // cell widths carry the jitter's 2^-16 (exact: a power of two; mt_step.cuh decode)
     float* ax = &blob[bl.off_axes + 4 * t];
     ax[0] = c->axis_dp[2 * t]; ax[1] = c->axis_dp[2 * t + 1] * 0x1p-16f;
     ax[2] = c->axis_th[2 * t]; ax[3] = c->axis_th[2 * t + 1] * 0x1p-16f;
+    // MT_LEAN_AXES: y = fma(v, d, lo) is monotone in v for d >= 0 and v runs over [0, n * 2^16), so the ends bound it.
+    // exp2c's polynomial is within 1e-6 relative of 2^y: 2^-0.0034 = 0.99765 < 0.999 and 2^-0.36 = 0.7792 < pi/4 = 0.7854
+    // (theta * 2/pi < 0.4961 rounds to quadrant 0).
+    const float v_dp = (float)((uint32_t)c->n_dp * 65536u - 1u), v_th = (float)((uint32_t)c->n_th * 65536u - 1u);
+    const float hi_dp = fmaf(v_dp, ax[1], ax[0]), hi_th = fmaf(v_th, ax[3], ax[2]);
+    axes_ok = axes_ok && ax[1] >= 0.0f && ax[3] >= 0.0f && ax[0] >= -120.0f && ax[2] >= -120.0f &&
+              hi_dp <= -0.0034f && hi_th <= -0.36f;
   }
+  c->lean_axes = axes_ok;
   for (int j = 0; j < n_reg; ++j) {
     blob[bl.off_zlo + j] = c->regions[j].z_lo;
     static_assert(sizeof(mt_region) == 40 && sizeof(MtRegionDev) == 40, "region layout");
@@ -396,6 +408,8 @@ int mt_set_option(mt_ctx* c, int option, int64_t value) {
     case MT_OPT_REFILL_MIN_IDLE:
       if (value < 0 || value > 32) return fail(c, MT_ERR_INVALID_ARG, "bad refill threshold");
       c->opt_min_idle = (int)value; return MT_OK;
+    case MT_OPT_NO_LEAN:
+      c->opt_no_lean = value != 0; return MT_OK;
     case MT_OPT_HASH_NXY:
       if (value < 0 || value > 256) return fail(c, MT_ERR_INVALID_ARG, "bad hash resolution");
       c->opt_hash_nxy = (int)value; return MT_OK;
@@ -556,6 +570,25 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
       weight[m] = (double)cells[m];
     }
   }
+  // MT_LEAN_INSIDE: g(x) = fl(fl(x - o) * inv_cell) is monotone in x, so the floats of the world box's half-open range
+  // that map into [0, n) form an interval [lo, hi); it is the whole range but for a few floats next to a face (on
+  // config 3, x = 1 - 2^-24 gives g = 200 = nx).  Found by stepping inward from each end.
+  c->lean_inside = false;
+  if (gm->mode == MT_GEOM_VOXEL) {
+    const float inv_cell = 1.0f / gm->cell;
+    auto g_of = [&](float x, float o) { const volatile float d = x - o; const volatile float g = d * inv_cell; return (float)g; };
+    auto interval = [&](float lo, float hi, float o, int n, float* out) {
+      float a = lo, b = nextafterf(hi, -INFINITY);                   // first and last float of [lo, hi)
+      int k = 0;
+      while (!(g_of(a, o) >= 0.0f) && k++ < 64) a = nextafterf(a, INFINITY);
+      while (!(g_of(b, o) < (float)n) && k++ < 128) b = nextafterf(b, -INFINITY);
+      out[0] = a; out[1] = nextafterf(b, INFINITY);
+      return g_of(a, o) >= 0.0f && g_of(b, o) < (float)n && a <= b;
+    };
+    c->lean_inside = interval(gm->x_min, gm->x_max, gm->ox, gm->nx, c->lean_box) &&
+                     interval(gm->y_min, gm->y_max, gm->oy, gm->ny, c->lean_box + 2) &&
+                     interval(gm->z_min, gm->z_exit, gm->oz, gm->nz, c->lean_box + 4);
+  }
   c->geom = *gm;
   c->geom.regions = nullptr; c->geom.d_material = nullptr; c->geom.d_field = nullptr;
   c->geom.blocks = nullptr;
@@ -572,6 +605,16 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
 }
 
 int64_t mt_launch_count(const mt_ctx* c) { return c ? c->launches : 0; }
+
+int mt_get_info(const mt_ctx* c, int what, int64_t* value) {
+  if (!c || !value) return MT_ERR_INVALID_ARG;
+  switch (what) {
+    case MT_INFO_LEAN_FACTS: *value = (c->lean_axes ? 1 : 0) | (c->lean_inside ? 2 : 0); return MT_OK;
+    case MT_INFO_LAST_LEAN: *value = c->last_lean; return MT_OK;
+    case MT_INFO_LAST_SCHEDULE: *value = c->last_sched; return MT_OK;
+    default: return MT_ERR_INVALID_ARG;
+  }
+}
 
 }  // extern "C"
 
@@ -592,6 +635,10 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.grid = (const MtCellPair*)c->d_grid.p;
   P.gsy = g.nx + 2; P.gsz = (g.nx + 2) * (g.ny + 2);
   P.fnx = (float)g.nx; P.fny = (float)g.ny; P.fnz = (float)g.nz;
+  P.grid_k = (0x4B400000u - 1u) * (uint32_t)(P.gsz + P.gsy + 1);
+  P.lean = (c->lean_axes ? MT_LEAN_AXES : 0) | (c->lean_inside ? MT_LEAN_INSIDE : 0);
+  P.lean_x_lo = c->lean_box[0]; P.lean_x_hi = c->lean_box[1]; P.lean_y_lo = c->lean_box[2]; P.lean_y_hi = c->lean_box[3];
+  P.lean_z_lo = c->lean_box[4]; P.lean_z_hi = c->lean_box[5];
   P.n_materials = c->n_materials; P.n_pbins = c->n_pbins; P.n_dp = c->n_dp; P.n_th = c->n_th;
   const bool joint = (c->hist_mode == MT_HIST_JOINT);
   P.n_joint = joint ? (uint32_t)(c->n_dp * c->n_th) : 0u;
@@ -648,6 +695,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   cfg.sched = sched;
   cfg.joint = (c->hist_mode == MT_HIST_JOINT);
   cfg.field = c->geom.field_mode;
+  cfg.lean = false;
   const size_t blob_b = ((blob_bytes(c) + 15) & ~(size_t)15);
   const size_t smem_budget = c->smem_optin;
   if (blob_b + 16 > smem_budget) return fail(c, MT_ERR_UNSUPPORTED, "edges, axes and regions (%zu B) do not fit in shared memory", blob_b);
@@ -665,6 +713,8 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   }
   P.hot_cells = (uint32_t)(hot_blocks * block_cells);
   cfg.tab_smem = hot_blocks > 0;
+  cfg.lean = !c->opt_no_lean && P.lean == MT_LEAN_ALL && mt_has_lean(c->geom.mode, cfg);
+  c->last_lean = cfg.lean; c->last_sched = sched;
   cfg.smem_bytes = blob_b + ((hot_blocks * block_cells * cell_b + 15) & ~(size_t)15) + 16;
 
   // block size: the one that keeps the most threads resident (ties -> the smaller block)
@@ -750,6 +800,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
     P.live_out_count = counts + s + 1;
     P.work_counter = work + s;
     P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * slab);
+    P.lean_z_hi = std::min(c->lean_box[5], P.slab_z_end);
     MT_CUDA(c, mt_launch_transport(P, cfg, stream));
     c->launches += 1;
     if (s < n_pass - 1) {

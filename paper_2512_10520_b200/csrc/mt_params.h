@@ -37,6 +37,15 @@ struct __align__(32) MtCellPair {
   float4 a, b;
 };
 
+// Facts the host proves about a (tables, geometry) pair; when all hold, the LEAN kernel variant drops the operations
+// that they turn into identities (results unchanged):
+//   MT_LEAN_AXES    every table axis keeps y = fma(cell.jitter, d, lo) inside [-120, 120] (exp2c's clamps), every Dp/p axis
+//                   ends below log2(0.999) with a margin of 2^-9 (the cap on f) and every theta axis below log2(0.78)
+//                   (theta < pi/4: the cap at pi and the quadrant reduction of its sine and cosine)
+//   MT_LEAN_INSIDE  lean_{x,y,z}_{lo,hi} bound the part of the world box whose every float32 position maps to a cell of
+//                   the voxel grid (the whole box but for a few floats next to a face, which take the general code)
+enum { MT_LEAN_AXES = 1, MT_LEAN_INSIDE = 2, MT_LEAN_ALL = 3 };
+
 struct MtParams {
   // ---- geometry
   int32_t mode;
@@ -46,8 +55,12 @@ struct MtParams {
   float ox, oy, oz, inv_cell;
   const MtCellPair* grid;        // [nz+2][ny+2][nx+2] pairs {cell x, cell x+1} of {Bx, By, Bz, material}: the caller's grids
                                  // with a one-cell clamp-replicated border, library-owned
-  int32_t gsy, gsz;              // grid strides in cells: nx+2 and (nx+2)(ny+2)
+  uint32_t gsy, gsz;             // grid strides in cells: nx+2 and (nx+2)(ny+2)
   float fnx, fny, fnz;           // (float)nx, ny, nz for the inside test
+  uint32_t grid_k;               // (0x4B400000 - 1) * (gsz + gsy + 1) mod 2^32: see lookup_voxel
+  uint32_t lean;                 // MT_LEAN_* facts proven on the host that let a kernel variant skip work
+  float lean_x_lo, lean_x_hi, lean_y_lo, lean_y_hi, lean_z_lo;
+  float lean_z_hi;               // per pass: also capped by the end of the slab
   // ---- tables
   int32_t n_materials, n_pbins, n_dp, n_th;
   float inv_p_lo, bin_scale;     // bin guess: floor(log2(P * inv_p_lo) * bin_scale), then fixed on the edges
