@@ -31,6 +31,7 @@ MT_DEV View<PACK> stage_view(const MtParams& P) {
   for (int i = threadIdx.x; i < P.bl.n_words; i += blockDim.x) sblob[i] = __ldg(P.blob + i);
   View<PACK> V;
   V.edges = sblob;
+  V.edges_open = sblob + P.bl.off_edges_open;
   V.steps = sblob + P.bl.off_steps;
   V.axes = reinterpret_cast<const float4*>(sblob + P.bl.off_axes);
   V.zlo = sblob + P.bl.off_zlo;

@@ -142,7 +142,8 @@ int rebuild_blob(mt_ctx* c) {
   const int n_reg = c->have_geom ? (int)c->regions.size() : 0;
   const int nt = c->n_materials * c->n_pbins;
   MtBlobLayout bl;
-  bl.off_steps = (n_edges + 3) & ~3;
+  bl.off_edges_open = (n_edges + 3) & ~3;
+  bl.off_steps = (bl.off_edges_open + n_edges + 3) & ~3;
   bl.off_axes = bl.off_steps + 4 * (c->n_materials + 1);
   bl.off_zlo = bl.off_axes + 4 * nt;
   bl.off_regions = (bl.off_zlo + n_reg + 3) & ~3;
@@ -153,6 +154,8 @@ int rebuild_blob(mt_ctx* c) {
   const double lo = (double)c->p_lo, hi = (double)c->p_hi;
   for (int j = 0; j <= c->n_pbins; ++j)
     blob[j] = (float)(lo * pow(hi / lo, (double)j / (double)c->n_pbins));                 // §3.4
+  for (int j = 0; j <= c->n_pbins; ++j)
+    blob[bl.off_edges_open + j] = (j == 0) ? -INFINITY : (j == c->n_pbins) ? INFINITY : blob[j];
   for (int m = 0; m <= c->n_materials; ++m) {
     const float h = c->step_m[m];
     blob[bl.off_steps + 4 * m + 0] = h;
@@ -636,6 +639,8 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.gsy = g.nx + 2; P.gsz = (g.nx + 2) * (g.ny + 2);
   P.fnx = (float)g.nx; P.fny = (float)g.ny; P.fnz = (float)g.nz;
   P.grid_k = (0x4B400000u - 1u) * (uint32_t)(P.gsz + P.gsy + 1);
+  P.gsy_bytes = (uint64_t)P.gsy * sizeof(MtCellPair); P.gsz_bytes = (uint64_t)P.gsz * sizeof(MtCellPair);
+  P.gsyz_bytes = P.gsy_bytes + P.gsz_bytes;
   P.lean = (c->lean_axes ? MT_LEAN_AXES : 0) | (c->lean_inside ? MT_LEAN_INSIDE : 0);
   P.lean_x_lo = c->lean_box[0]; P.lean_x_hi = c->lean_box[1]; P.lean_y_lo = c->lean_box[2]; P.lean_y_hi = c->lean_box[3];
   P.lean_z_lo = c->lean_box[4]; P.lean_z_hi = c->lean_box[5];

@@ -12,6 +12,7 @@ struct MtRegionDev {
 
 // The "const blob": small read-only arrays every CTA stages into shared memory at start.
 //   [0, n_pbins]                         momentum-bin edges, float32
+//   [off_edges_open + 0 .. n_pbins]      the same edges with the first replaced by -inf and the last by +inf
 //   [off_steps + 4*m .. +3]              h, h/2, h/6 of material m, m = 0..n_materials, and the
 //                                        first cell of the material's tables in the packed array (int bits)
 //   [off_axes + 4*t .. +3]               lo_dp, d_dp * 2^-16, lo_th, d_th * 2^-16 (log2) of table t = (m-1)*n_pbins + i
@@ -19,7 +20,7 @@ struct MtRegionDev {
 //   [off_regions + 10*j ..]              MtRegionDev j
 //   [off_blocks + 24*j ..]               MtBlockDev j (POLY mode)
 struct MtBlobLayout {
-  int32_t off_steps, off_axes, off_zlo, off_regions, off_blocks, n_words;
+  int32_t off_edges_open, off_steps, off_axes, off_zlo, off_regions, off_blocks, n_words;
 };
 
 // Polyhedra block as staged in shared memory: six float4.  inv_dz = 1 / (z_hi - z_lo), dx_i = xh_i - xl_i and
@@ -56,6 +57,7 @@ struct MtParams {
   const MtCellPair* grid;        // [nz+2][ny+2][nx+2] pairs {cell x, cell x+1} of {Bx, By, Bz, material}: the caller's grids
                                  // with a one-cell clamp-replicated border, library-owned
   uint32_t gsy, gsz;             // grid strides in cells: nx+2 and (nx+2)(ny+2)
+  uint64_t gsy_bytes, gsz_bytes, gsyz_bytes;   // the same in bytes (32 per cell), and their sum
   float fnx, fny, fnz;           // (float)nx, ny, nz for the inside test
   uint32_t grid_k;               // (0x4B400000 - 1) * (gsz + gsy + 1) mod 2^32: see lookup_voxel
   uint32_t lean;                 // MT_LEAN_* facts proven on the host that let a kernel variant skip work
