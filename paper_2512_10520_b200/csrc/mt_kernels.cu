@@ -426,8 +426,22 @@ kernel_fn pick_tables(const MtLaunchCfg& cfg) {
                       : pick_sched<GEOM, 64, false, false, FIELD>(cfg.sched);
 }
 kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
-  if (cfg.lean && mt_has_lean(mode, cfg))
-    return (cfg.pack == 32) ? wave_transport_kernel<1, 32, false, false, 0, true> : wave_transport_kernel<1, 64, false, false, 0, true>;
+  if (cfg.lean && mt_has_lean(mode, cfg)) {
+    switch ((cfg.field & 3) | (cfg.joint ? 8 : (cfg.pack == 32 ? 0 : 4))) {
+      case 0: return wave_transport_kernel<1, 32, false, false, 0, true>;
+      case 1: return wave_transport_kernel<1, 32, false, false, 1, true>;
+      case 2: return wave_transport_kernel<1, 32, false, false, 2, true>;
+      case 3: return wave_transport_kernel<1, 32, false, false, 3, true>;
+      case 4: return wave_transport_kernel<1, 64, false, false, 0, true>;
+      case 5: return wave_transport_kernel<1, 64, false, false, 1, true>;
+      case 6: return wave_transport_kernel<1, 64, false, false, 2, true>;
+      case 7: return wave_transport_kernel<1, 64, false, false, 3, true>;
+      case 8: return wave_transport_kernel<1, 64, false, true, 0, true>;
+      case 9: return wave_transport_kernel<1, 64, false, true, 1, true>;
+      case 10: return wave_transport_kernel<1, 64, false, true, 2, true>;
+      default: return wave_transport_kernel<1, 64, false, true, 3, true>;
+    }
+  }
   if (mode == 0) return (cfg.field & 2) ? pick_tables<0, 2>(cfg) : pick_tables<0, 0>(cfg);
   if (mode == 2) return (cfg.field & 2) ? pick_tables<2, 2>(cfg) : pick_tables<2, 0>(cfg);
   switch (cfg.field & 3) {
@@ -441,7 +455,7 @@ kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
 }  // namespace
 
 bool mt_has_lean(int mode, const MtLaunchCfg& cfg) {
-  return mode == 1 && cfg.sched == SCHED_WAVEFRONT && !cfg.joint && !cfg.tab_smem && (cfg.field & 3) == 0;
+  return mode == 1 && cfg.sched == SCHED_WAVEFRONT && !cfg.tab_smem;
 }
 
 // ------------------------------------------------------------------------------------------------

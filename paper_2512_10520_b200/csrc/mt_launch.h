@@ -21,8 +21,8 @@ struct MtLaunchCfg {
   int field;       // MT_FIELD_* of the geometry
   bool lean;       // P.lean == MT_LEAN_ALL and a LEAN kernel exists for this combination (mt_has_lean)
 };
-// LEAN variants are compiled for the hot combination only: voxel geometry, marginal tables in L2, trilinear frozen
-// field, WAVEFRONT schedule
+// LEAN variants are compiled for the WAVEFRONT schedule on a voxel geometry with the tables gathered from L2 (every
+// field mode, marginal or joint tables)
 bool mt_has_lean(int mode, const MtLaunchCfg& cfg);
 
 cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream);

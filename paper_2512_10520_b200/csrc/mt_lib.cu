@@ -164,7 +164,8 @@ int rebuild_blob(mt_ctx* c) {
     const int32_t cell0 = (int32_t)c->mat_cell0[m];
     memcpy(&blob[bl.off_steps + 4 * m + 3], &cell0, sizeof cell0);
   }
-  bool axes_ok = (c->hist_mode == MT_HIST_MARGINAL);
+  const bool joint_axes = (c->hist_mode == MT_HIST_JOINT);   // axis b is then the transverse fraction ft: proven <= 1
+  bool axes_ok = true;
   for (int t = 0; t < nt; ++t) {
     // cell widths carry the jitter's 2^-16 (exact: a power of two; mt_step.cuh decode)
     float* ax = &blob[bl.off_axes + 4 * t];
@@ -176,7 +177,7 @@ int rebuild_blob(mt_ctx* c) {
     const float v_dp = (float)((uint32_t)c->n_dp * 65536u - 1u), v_th = (float)((uint32_t)c->n_th * 65536u - 1u);
     const float hi_dp = fmaf(v_dp, ax[1], ax[0]), hi_th = fmaf(v_th, ax[3], ax[2]);
     axes_ok = axes_ok && ax[1] >= 0.0f && ax[3] >= 0.0f && ax[0] >= -120.0f && ax[2] >= -120.0f &&
-              hi_dp <= -0.0034f && hi_th <= -0.36f;
+              hi_dp <= -0.0034f && hi_th <= (joint_axes ? 0.0f : -0.36f);
   }
   c->lean_axes = axes_ok;
   for (int j = 0; j < n_reg; ++j) {

@@ -42,7 +42,8 @@ struct __align__(32) MtCellPair {
 // that they turn into identities (results unchanged):
 //   MT_LEAN_AXES    every table axis keeps y = fma(cell.jitter, d, lo) inside [-120, 120] (exp2c's clamps), every Dp/p axis
 //                   ends below log2(0.999) with a margin of 2^-9 (the cap on f) and every theta axis below log2(0.78)
-//                   (theta < pi/4: the cap at pi and the quadrant reduction of its sine and cosine)
+//                   (theta < pi/4: the cap at pi and the quadrant reduction of its sine and cosine); JOINT tables: the
+//                   transverse axis ends at or below 0 (ft <= 1: the new |p| stays in the fast sqrt / rcp range)
 //   MT_LEAN_INSIDE  lean_{x,y,z}_{lo,hi} bound the part of the world box whose every float32 position maps to a cell of
 //                   the voxel grid (the whole box but for a few floats next to a face, which take the general code)
 enum { MT_LEAN_AXES = 1, MT_LEAN_INSIDE = 2, MT_LEAN_ALL = 3 };

@@ -99,3 +99,21 @@ def test_lean_facts_are_refused_when_an_axis_reaches_a_clamp(mt, oracle):
     ref = oracle_transport(oracle, wl)
     c = compare(got, ref)
     assert c["bit_exact"] == 1.0
+
+
+@pytest.mark.parametrize("joint,field_mode", [(False, 1), (False, 2), (False, 3), (True, 0), (True, 2)])
+def test_lean_variants_of_the_other_voxel_modes(mt, oracle, joint, field_mode):
+    # nearest-neighbour / per-stage field and the joint 2D tables have lean kernels too (the stage lookups keep their
+    # inside test: a stage position may lie outside the grid)
+    from paper_2512_10520_b200 import workloads as w
+    shape = (20, 32, 16) if joint else (100, 256, 128)
+    wl = w.config3(n=20_000, n_draws=100_000, n_cells=1, half_width_cells=30, device="cuda", joint=joint,
+                   table_shape=shape, field_mode=field_mode)
+    lean, info = _run(mt, wl, 0)
+    assert info["facts"] == 3 and info["lean"] == 1
+    gen, info2 = _run(mt, wl, 1)
+    assert info2["lean"] == 0
+    ref = oracle_transport(oracle, wl)
+    for got in (lean, gen):
+        c = compare(got, ref)
+        assert c["bit_exact"] == 1.0 and c["matched"] >= 0.999
