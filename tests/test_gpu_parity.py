@@ -217,3 +217,36 @@ def test_config4_table_shapes_and_batches(mt, oracle, shape):
             assert c["matched"] >= MATCH and c["bit_exact"] == 1.0
     del wl
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("shape,batch", [((256, 1024, 512), 3), ((50, 128, 64), 7)])
+def test_config4_full_size_sampled(mt, oracle, shape, batch):
+    """BASELINE configs[4] as `bench.py --sweep` times it: the full 200x200x3000 grid, one 10^7-muon batch of the 10^8
+    (generator batch and id_base = batch * 10^7), the largest (8-byte cells, 9.4 MB) and the smallest (fits shared memory)
+    table shapes; the oracle recomputes every 5000th muon one by one from its id."""
+    import torch
+    from paper_2512_10520_b200 import workloads as w
+    b = mt.binding
+    free, _ = torch.cuda.mem_get_info()
+    if free < 12 * 2 ** 30:
+        pytest.skip("needs 12 GiB of device memory")
+    n = 10_000_000
+    wl = w.config3(n=8, device="cuda", table_shape=shape, n_draws=200_000)
+    wl.muons = w.spectrum_muons(3, n, "square", batch=batch)
+    id_base = batch * n
+    h = b.MuonTransport(0).setup(wl.hist, wl.geom)
+    try:
+        g = gpu_transport(mt, wl, handle=h, id_base=id_base)
+        assert b.mt_get_info(h.ctx, b.MT_INFO_LAST_SCHEDULE) == b.MT_SCHED_WAVEFRONT
+        assert g["counters"][1:5].sum() == n and g["counters"][0] == g["steps"].sum()
+        sel = np.arange(0, n, 5000)
+        ref = oracle_transport(oracle, wl, sel=sel, ids=(sel + id_base).astype(np.uint64))
+        sub = {k: g[k][sel] for k in ("pos", "mom", "flag", "steps")}
+        c = compare(sub, ref)
+        _report("config4 full %dx%dx%d batch %d (every 5000th)" % (shape + (batch,)), c)
+        assert c["matched"] >= MATCH and c["bit_exact"] == 1.0
+        assert np.all((g["flag"] >= 1) & (g["flag"] <= 4))
+    finally:
+        h.close()
+        del wl
+        torch.cuda.empty_cache()
