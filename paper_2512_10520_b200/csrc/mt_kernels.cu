@@ -5,7 +5,7 @@
 //   STATIC     one lane per muon for its whole life (the paper's own mapping, L59, L174);
 //   REFILL     persistent warps; lanes whose muon has terminated take new muons from a global counter;
 //   WAVEFRONT  one pass per z-slab over the live muons, which are re-sorted by xy cell between passes
-//              (counting sort: wave_bin / wave_scan / wave_scatter).  A warp then holds 32 muons of the same
+//              (counting sort of record indices: wave_bin / wave_scan / wave_perm).  A warp then holds 32 muons of the same
 //              cell column at the same z, so its eight field-corner gathers fall into one or two cache lines
 //              instead of 32, and the slab's few z-layers of the 1.9 GB grid stay L1/L2-resident.
 #include <cuda_runtime.h>
@@ -186,14 +186,14 @@ MT_DEV uint32_t sort_key(const MtParams& P, float x, float y, float px, float py
   return (uint32_t)((int)fy * P.key_nx + (int)fx);
 }
 
-// pass "-1": key and rank of every input muon (the state itself is read by wave_scatter from the caller's arrays)
+// pass "-1": key and rank of every input muon (the first transport pass reads the state from the caller's arrays)
 __global__ void __launch_bounds__(256) wave_bin_kernel(const __grid_constant__ MtParams P) {
   const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += stride) {
     const float4 a = __ldg(P.in_pos_q + i), b = __ldg(P.in_mom + i);
     const uint32_t key = sort_key(P, a.x, a.y, b.x, b.y, b.z);
     const uint32_t rank = atomicAdd(P.hist + key, 1u);
-    P.u_key[i] = make_uint4((uint32_t)i, key, rank, 0u);
+    P.sort_key[i] = make_uint2(key, rank);
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) *P.live_out_count = (uint32_t)P.n;
 }
@@ -245,20 +245,14 @@ __global__ void __launch_bounds__(1024) wave_scan_kernel(uint32_t* __restrict__ 
   }
 }
 
-// parked list (arrival order) -> sorted list; `first` reads the caller's input arrays (whose mom.w is unused)
-__global__ void __launch_bounds__(256) wave_scatter_kernel(const __grid_constant__ MtParams P, const float4* __restrict__ src_a,
-                                                           const float4* __restrict__ src_b, int first) {
+// sorted order of the parked records: perm[first position of the key + rank within the key] = record.  The 4-byte
+// scattered writes land in a 40 MB array that stays in L2; the records themselves do not move.
+__global__ void __launch_bounds__(256) wave_perm_kernel(const __grid_constant__ MtParams P) {
   const uint32_t n = *P.live_out_count;
   const uint32_t stride = gridDim.x * blockDim.x;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const uint4 k = P.u_key[i];
-    const uint32_t dst = P.key_offset[k.y] + k.z;
-    const float4 a = src_a[i];
-    float4 b = src_b[i];
-    if (first) b.w = __int_as_float(0);
-    P.s_pos_q[dst] = a;
-    P.s_mom_step[dst] = b;
-    P.s_idx[dst] = k.x;
+    const uint2 k = P.sort_key[i];
+    P.perm[P.key_offset[k.x] + k.y] = i;
   }
 }
 
@@ -283,12 +277,21 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
     int flag = -1;                                    // -1: no muon on this lane
     m.x = m.y = m.z = m.q = m.px = m.py = m.pz = 0.0f;
     m.step = 0;
-      if (item < n_items) {
-      const float4 a = P.s_pos_q[item], b = P.s_mom_step[item];
-      idx = P.s_idx[item];
+    if (item < n_items) {
+      const uint32_t rec = P.perm[item];
+      float4 a, b;
+      if (P.first_pass) {
+        a = __ldg(P.in_pos_q + rec); b = __ldg(P.in_mom + rec);
+        b.w = __int_as_float(0);
+        idx = rec;
+      } else {
+        const float4* r = P.rec_in + 3 * (size_t)rec;
+        a = __ldg(r); b = __ldg(r + 1);
+        idx = __ldg(reinterpret_cast<const uint32_t*>(r + 2));
+      }
       m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z;
       m.step = __float_as_int(b.w);
-        flag = 0;
+      flag = 0;
     }
     const uint64_t id = P.id_base + idx;
     const uint32_t id_lo = (uint32_t)id, id_hi = (uint32_t)(id >> 32);
@@ -320,9 +323,11 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
         if ((int)lane == pl) r0 = atomicAdd(P.hist + key, (unsigned)__popc(peers));
         r0 = __shfl_sync(peers, r0, pl);
         const unsigned slot = slot0 + (unsigned)__popc(pm & lt_mask);
-        P.u_pos_q[slot] = make_float4(m.x, m.y, m.z, m.q);
-        P.u_mom_step[slot] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
-        P.u_key[slot] = make_uint4(idx, key, r0 + (unsigned)__popc(peers & lt_mask), 0u);
+        float4* r = P.rec_out + 3 * (size_t)slot;                       // a warp's records are contiguous: full sectors
+        r[0] = make_float4(m.x, m.y, m.z, m.q);
+        r[1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
+        r[2] = make_float4(__uint_as_float(idx), 0.0f, 0.0f, 0.0f);
+        P.sort_key[slot] = make_uint2(key, r0 + (unsigned)__popc(peers & lt_mask));
       }
     }
   }
@@ -481,8 +486,7 @@ cudaError_t mt_launch_wave_bin(const MtParams& P, unsigned grid, cudaStream_t st
   return cudaGetLastError();
 }
 
-cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src_a, const float4* src_b, int first,
-                                unsigned grid, cudaStream_t stream) {
+cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, unsigned grid, cudaStream_t stream) {
   const size_t stage_b = (size_t)n_keys * sizeof(uint32_t);
   cudaError_t e;
   if (stage_b <= 200 * 1024) {
@@ -494,7 +498,7 @@ cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src
   }
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  wave_scatter_kernel<<<grid, 256, 0, stream>>>(P, src_a, src_b, first);
+  wave_perm_kernel<<<grid, 256, 0, stream>>>(P);
   return cudaGetLastError();
 }
 

@@ -27,11 +27,10 @@ bool mt_has_lean(int mode, const MtLaunchCfg& cfg);
 
 cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream);
 cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm);
-// WAVEFRONT helpers: key + rank of the input muons; scan of the key histogram followed by the scatter of the
-// parked list (src_a / src_b) into the sorted list
+// WAVEFRONT helpers: key + rank of the input muons; scan of the key histogram followed by the permutation that
+// puts the parked records (P.sort_key) in sorted order (P.perm)
 cudaError_t mt_launch_wave_bin(const MtParams& P, unsigned grid, cudaStream_t stream);
-cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, const float4* src_a, const float4* src_b, int first,
-                                unsigned grid, cudaStream_t stream);
+cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, unsigned grid, cudaStream_t stream);
 // d_material_cells: [256] counters (zeroed by the caller) of grid cells per material id
 cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, MtCellPair* out, int nx, int ny, int nz,
                              unsigned long long* d_material_cells, cudaStream_t stream);

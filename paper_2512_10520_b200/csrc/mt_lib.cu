@@ -788,29 +788,34 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   uint32_t* counts = (uint32_t*)((char*)c->d_scratch.p + off_counts);
   P.hist = (uint32_t*)((char*)c->d_scratch.p + off_hist);
   P.key_offset = P.hist + n_keys;
-  // in-flight state: S (sorted) 36 B and U (parked) 48 B per muon
-  const size_t n16 = ((size_t)n * 16 + 255) & ~(size_t)255, n4 = ((size_t)n * 4 + 255) & ~(size_t)255;
-  MT_CUDA(c, c->d_wave.reserve(5 * n16 + n4));
+  // in-flight state: two buffers of 48-byte records (read by a pass / parked by it), {key, rank} 8 B and the
+  // permutation 4 B per muon
+  const size_t n48 = ((size_t)n * 48 + 255) & ~(size_t)255, n8 = ((size_t)n * 8 + 255) & ~(size_t)255, n4 = ((size_t)n * 4 + 255) & ~(size_t)255;
+  MT_CUDA(c, c->d_wave.reserve(2 * n48 + n8 + n4));
   char* w = (char*)c->d_wave.p;
-  P.s_pos_q = (float4*)w; P.s_mom_step = (float4*)(w + n16); P.u_pos_q = (float4*)(w + 2 * n16);
-  P.u_mom_step = (float4*)(w + 3 * n16); P.u_key = (uint4*)(w + 4 * n16); P.s_idx = (uint32_t*)(w + 5 * n16);
+  float4* rec[2] = {(float4*)w, (float4*)(w + n48)};
+  P.sort_key = (uint2*)(w + 2 * n48);
+  P.perm = (uint32_t*)(w + 2 * n48 + n8);
   const unsigned aux_grid = (unsigned)std::min<uint64_t>((uint64_t)c->sm_count * 8, (n + 255) / 256);
   cfg.grid = (unsigned)std::min<uint64_t>(persistent_grid, (n + cfg.block - 1) / cfg.block);
 
   P.live_out_count = counts;                                   // counts[s] = muons entering pass s
   MT_CUDA(c, mt_launch_wave_bin(P, aux_grid, stream));
-  MT_CUDA(c, mt_launch_wave_sort(P, n_keys, P.in_pos_q, P.in_mom, 1, aux_grid, stream));
+  MT_CUDA(c, mt_launch_wave_sort(P, n_keys, aux_grid, stream));
   c->launches += 3;
   for (int s = 0; s < n_pass; ++s) {
     P.live_in_count = counts + s;
     P.live_out_count = counts + s + 1;
     P.work_counter = work + s;
+    P.first_pass = (s == 0);
+    P.rec_in = rec[(s + 1) & 1];
+    P.rec_out = rec[s & 1];
     P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * slab);
     P.lean_z_hi = std::min(c->lean_box[5], P.slab_z_end);
     MT_CUDA(c, mt_launch_transport(P, cfg, stream));
     c->launches += 1;
     if (s < n_pass - 1) {
-      MT_CUDA(c, mt_launch_wave_sort(P, n_keys, P.u_pos_q, P.u_mom_step, 0, aux_grid, stream));
+      MT_CUDA(c, mt_launch_wave_sort(P, n_keys, aux_grid, stream));
       c->launches += 2;
     }
   }

@@ -98,17 +98,18 @@ struct MtParams {
   unsigned long long* counters;  // optional [8]
   unsigned long long* work_counter;   // refill scheduler
   int32_t refill_min_idle;
-  // ---- wavefront scheduler (mt_kernels.cu): one pass per z-slab.  In-flight muons live in
-  //      library scratch: S = sorted by xy cell (read by a pass), U = parked in arrival order (written by it).
-  const uint32_t* live_in_count; // device count of S
-  uint32_t* live_out_count;      // device count of U (zero on entry)
+  // ---- wavefront scheduler (mt_kernels.cu): one pass per z-slab.  In-flight muons live in library
+  //      scratch as 48-byte records {x,y,z,q | px,py,pz,step | index,-,-,-} in the order in which a pass parked them;
+  //      the next pass reads them THROUGH a permutation (perm[sorted position] = record), so sorting moves 4 bytes
+  //      per muon instead of the records.  Two record buffers alternate between passes.
+  const uint32_t* live_in_count; // device count of the records a pass reads
+  uint32_t* live_out_count;      // device count of the records it parks (zero on entry)
   float slab_z_end;              // a pass advances each muon until z >= slab_z_end (or it terminates)
-  float4* s_pos_q;               // [live] x, y, z, q
-  float4* s_mom_step;            // [live] px, py, pz, step (int bits)
-  uint32_t* s_idx;               // [live] muon index within the call
-  float4* u_pos_q;
-  float4* u_mom_step;
-  uint4* u_key;                  // [parked] {muon index, sort key, rank within key, -}
+  int32_t first_pass;            // 1: the records are the caller's input arrays (step 0, index = position)
+  const float4* rec_in;          // [live][3]
+  float4* rec_out;               // [parked][3]
+  uint2* sort_key;               // [parked] {sort key, rank within key} of the records just parked / of the inputs
+  uint32_t* perm;                // [live] record of each position of the sorted order
   uint32_t* hist;                // [n_keys] muons parked per sort key (zero on entry; the scan zeroes it again)
   uint32_t* key_offset;          // [n_keys] exclusive scan of hist
   float key_x0, key_y0, key_inv; // sort key = iy * key_nx + ix, ix = clamp((int)((x - key_x0) * key_inv), 0, key_nx-1)
