@@ -8,16 +8,18 @@ rounding themselves (csrc/mt_step.cuh), -fmad=false is belt and braces.
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmuon_transport.so")
-SOURCES = ["mt_lib.cu", "mt_kernels.cu"]
-DEPS = SOURCES + ["mt_step.cuh", "mt_params.h", "mt_launch.h"]
+SOURCES = ["mt_lib.cu", "mt_kernels.cu", "mt_inst_regions.cu", "mt_inst_poly.cu", "mt_inst_voxel_a.cu",
+           "mt_inst_voxel_b.cu", "mt_inst_lean.cu"]
+DEPS = SOURCES + ["mt_kernels.cuh", "mt_step.cuh", "mt_params.h", "mt_launch.h"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
-              "-Xcompiler", "-fPIC,-Wall", "-shared", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC,-Wall", "-Xptxas", "-v"]
 
 
 def _nvcc():
@@ -28,22 +30,49 @@ def _nvcc():
 
 
 def build(force: bool = False, verbose: bool = False, defines=()) -> str:
-    """`defines`: extra -D macros (e.g. MT_MIN_BLOCKS=4, MT_MAX_THREADS=128) for tuning experiments."""
+    """Compile the translation units in parallel (the kernel instantiations are split over several so that this takes
+    well under a minute), then link.  `defines`: extra -D macros (e.g. MT_MAX_THREADS=1024) for tuning experiments."""
     deps = [os.path.join(CSRC, d) for d in DEPS] + [os.path.join(INCLUDE, "muon_transport.h"), __file__]
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
-    tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [_nvcc(), *NVCC_FLAGS, *["-D" + d for d in defines], "-I", INCLUDE, "-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
-    res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
-    if res.returncode != 0:
-        sys.stderr.write(res.stdout)
-        raise RuntimeError("nvcc failed building libmuon_transport.so")
+    bdir = os.path.join(HERE, "build")
+    os.makedirs(bdir, exist_ok=True)
+    tag = ".%d" % os.getpid()
+    base = [_nvcc(), *NVCC_FLAGS, *["-D" + d for d in defines], "-I", INCLUDE]
+
+    def compile_one(src):
+        obj = os.path.join(bdir, src[:-3] + tag + ".o")
+        cmd = base + ["-c", os.path.join(CSRC, src), "-o", obj]
+        res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+        return obj, cmd, res
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as pool:
+        done = list(pool.map(compile_one, SOURCES))
+    log = []
+    objs = []
+    try:
+        for obj, cmd, res in done:
+            log.append(" ".join(cmd) + "\n" + res.stdout)
+            objs.append(obj)
+            if res.returncode != 0:
+                sys.stderr.write(res.stdout)
+                raise RuntimeError("nvcc failed compiling " + cmd[-3])
+        tmp = LIB + ".tmp" + tag
+        link = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + objs
+        res = subprocess.run(link, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+        log.append(" ".join(link) + "\n" + res.stdout)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout)
+            raise RuntimeError("nvcc failed linking libmuon_transport.so")
+        os.replace(tmp, LIB)
+    finally:
+        for obj in objs:
+            if os.path.exists(obj):
+                os.remove(obj)
+        with open(os.path.join(bdir, "ptxas.log"), "w") as f:
+            f.write("\n".join(log))
     if verbose:
-        print(res.stdout)
-    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
-    with open(os.path.join(HERE, "build", "ptxas.log"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + res.stdout)
-    os.replace(tmp, LIB)
+        print("\n".join(log))
     return LIB
 
 

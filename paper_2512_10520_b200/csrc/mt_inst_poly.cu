@@ -1,0 +1,6 @@
+// mt_inst_poly.cu — transport-kernel instantiations for convex polyhedra (MT_GEOM_POLY): every table kind and schedule, field frozen or per stage.
+#include "mt_kernels.cuh"
+
+mt_kernel_fn mt_pick_poly(const MtLaunchCfg& cfg) {
+  return (cfg.field & 2) ? pick_tables<2, 2>(cfg) : pick_tables<2, 0>(cfg);
+}

@@ -1,190 +1,12 @@
-// mt_kernels.cu — the transport kernels and their launchers (sm_100a).
-//
-// Algorithm 1 runs under three schedules; the per-step arithmetic is
-// mt_step.cuh and results do not depend on the schedule:
-//   STATIC     one lane per muon for its whole life (the paper's own mapping, L59, L174);
-//   REFILL     persistent warps; lanes whose muon has terminated take new muons from a global counter;
-//   WAVEFRONT  one pass per z-slab over the live muons, which are re-sorted by xy cell between passes
-//              (counting sort of record indices: wave_bin / wave_scan / wave_perm).  A warp then holds 32 muons of the same
-//              cell column at the same z, so its eight field-corner gathers fall into one or two cache lines
-//              instead of 32, and the slab's few z-layers of the 1.9 GB grid stay L1/L2-resident.
+// mt_kernels.cu — the helper kernels (index sort of the WAVEFRONT schedule, grid repack, test hooks), the choice of the
+// transport kernel for a launch configuration, and all launchers (sm_100a).  The transport kernels themselves are the
+// templates of mt_kernels.cuh, instantiated in the mt_inst_*.cu files.
 #include <cuda_runtime.h>
 #include <algorithm>
 #include <stdint.h>
-#include "mt_launch.h"
-#include "mt_step.cuh"
+#include "mt_kernels.cuh"
 
 namespace {
-
-using namespace mt;
-
-enum { SCHED_STATIC = 1, SCHED_REFILL = 2, SCHED_WAVEFRONT = 3 };
-constexpr int kInnerSteps = 8;        // REFILL: steps between two refill checks
-constexpr unsigned kFull = 0xFFFFFFFFu;
-
-extern __shared__ __align__(16) unsigned char mt_smem[];
-
-template <int PACK, bool TAB_SMEM>
-MT_DEV View<PACK> stage_view(const MtParams& P) {
-  // const blob (edges, step lengths, axes, regions) -> shared memory, then the hot prefix of the packed tables
-  float* sblob = reinterpret_cast<float*>(mt_smem);
-  for (int i = threadIdx.x; i < P.bl.n_words; i += blockDim.x) sblob[i] = __ldg(P.blob + i);
-  View<PACK> V;
-  V.edges = sblob;
-  V.edges_open = sblob + P.bl.off_edges_open;
-  V.steps = sblob + P.bl.off_steps;
-  V.axes = reinterpret_cast<const float4*>(sblob + P.bl.off_axes);
-  V.zlo = sblob + P.bl.off_zlo;
-  V.regions = reinterpret_cast<const MtRegionDev*>(sblob + P.bl.off_regions);
-  V.blocks = reinterpret_cast<const MtBlockDev*>(sblob + P.bl.off_blocks);
-  const uint32_t* gtab = (PACK == 32) ? P.tab32 : reinterpret_cast<const uint32_t*>(P.tab64);
-  V.tab = reinterpret_cast<const typename Tab<PACK>::cell_t*>(gtab);
-  uint4* stab = reinterpret_cast<uint4*>(sblob + ((P.bl.n_words + 3) & ~3));
-  V.hot = reinterpret_cast<const typename Tab<PACK>::cell_t*>(stab);
-  if (TAB_SMEM) {
-    const uint32_t n16 = (P.hot_cells * (PACK / 8) + 15u) / 16u;          // the device array is padded to 16 bytes
-    const uint4* src = reinterpret_cast<const uint4*>(gtab);
-    for (uint32_t i = threadIdx.x; i < n16; i += blockDim.x) stab[i] = __ldg(src + i);
-  }
-  __syncthreads();
-  return V;
-}
-
-// per-lane tallies of a call, reduced per warp and added to the caller's counters at kernel end
-struct Tally {
-  unsigned long long steps = 0;
-  unsigned f1 = 0, f2 = 0, f3 = 0, f4 = 0;
-  MT_DEV void count(int flag) { f1 += (flag == 1); f2 += (flag == 2); f3 += (flag == 3); f4 += (flag == 4); }
-  MT_DEV void flush(unsigned long long* counters, unsigned lane) {
-    if (!counters) return;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) steps += __shfl_xor_sync(kFull, steps, o);
-    f1 = __reduce_add_sync(kFull, f1); f2 = __reduce_add_sync(kFull, f2);
-    f3 = __reduce_add_sync(kFull, f3); f4 = __reduce_add_sync(kFull, f4);
-    if (lane == 0) {
-      if (steps) atomicAdd(counters + 0, steps);
-      if (f1) atomicAdd(counters + 1, (unsigned long long)f1);
-      if (f2) atomicAdd(counters + 2, (unsigned long long)f2);
-      if (f3) atomicAdd(counters + 3, (unsigned long long)f3);
-      if (f4) atomicAdd(counters + 4, (unsigned long long)f4);
-    }
-  }
-};
-
-// final state of a terminated muon -> dense outputs; exit-plane hits also go to the compact list through one
-// atomic per warp (north_star subsystem 6).  Called by all 32 lanes; `flag` is 0 on lanes with nothing to write.
-MT_DEV void write_final(const MtParams& P, const Muon& m, uint32_t idx, int flag, unsigned lane) {
-  if (flag) {
-    P.out_pos_flag[idx] = make_float4(m.x, m.y, m.z, __int_as_float(flag));
-    P.out_mom_steps[idx] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
-  }
-  if (P.exit_rec) {
-    const bool ex = (flag == 2);
-    const unsigned em = __ballot_sync(kFull, ex);
-    if (em) {
-      const int leader = __ffs(em) - 1;
-      unsigned base = 0;
-      if ((int)lane == leader) base = atomicAdd(P.exit_count, (unsigned)__popc(em));
-      base = __shfl_sync(kFull, base, leader);
-      if (ex) {
-        const unsigned slot = base + (unsigned)__popc(em & ((1u << lane) - 1u));
-        if (slot < P.exit_capacity) {
-          P.exit_rec[2 * (size_t)slot] = make_float4(m.x, m.y, m.z, __uint_as_float(idx));
-          P.exit_rec[2 * (size_t)slot + 1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
-        }
-      }
-    }
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// STATIC and REFILL
-// ------------------------------------------------------------------------------------------------
-template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD, int SCHED>
-__global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
-transport_kernel(const __grid_constant__ MtParams P) {
-  const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
-  const unsigned lane = threadIdx.x & 31u;
-  const unsigned lt_mask = (1u << lane) - 1u;
-  const uint64_t n_items = P.n;
-
-  Muon m;
-  m.x = m.y = m.z = m.q = m.px = m.py = m.pz = 0.0f;
-  m.step = 0;
-  uint32_t idx = 0;              // muon index within this call
-  bool active = false;
-  bool exhausted = false;        // warp-uniform: the work counter has run past n_items
-  Tally tally;
-
-  auto load = [&](uint64_t item) {
-    idx = (uint32_t)item;
-    const float4 a = __ldg(P.in_pos_q + idx), b = __ldg(P.in_mom + idx);
-    m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z; m.step = 0;
-    active = true;
-  };
-
-  if (SCHED == SCHED_STATIC) {
-    const uint64_t item = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (item < n_items) load(item);
-    exhausted = true;
-  }
-
-  for (;;) {
-    // ---- refill idle lanes from the global work counter (warp-aggregated: one atomic per warp)
-    if (SCHED != SCHED_STATIC && !exhausted) {
-      const unsigned idle = __ballot_sync(kFull, !active);
-      const int n_idle = __popc(idle);
-      if (n_idle >= P.refill_min_idle || idle == kFull) {
-        unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(P.work_counter, (unsigned long long)n_idle);
-        base = __shfl_sync(kFull, base, 0);
-        if (!active) {
-          const uint64_t item = base + (unsigned)__popc(idle & lt_mask);
-          if (item < n_items) load(item);
-        }
-        if (base + (unsigned)n_idle >= n_items) exhausted = true;
-      }
-    }
-    if (!__any_sync(kFull, active)) {
-      if (exhausted) break;
-      continue;
-    }
-
-    // ---- a few steps for every active lane; the loop itself stays warp-uniform
-#pragma unroll 1
-    for (int k = 0; k < kInnerSteps; ++k) {
-      int flag = 0;
-      if (active) {
-        const uint64_t id = P.id_base + idx;
-        flag = step_once<GEOM, PACK, TAB_SMEM, false, JOINT, FIELD>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
-        if (flag == 0) tally.steps += 1;
-      }
-      write_final(P, m, idx, flag, lane);
-      if (flag) {
-        tally.count(flag);
-        active = false;
-      }
-      if (!__any_sync(kFull, active)) break;
-    }
-    if (SCHED == SCHED_STATIC && !__any_sync(kFull, active)) break;
-  }
-  tally.flush(P.counters, lane);
-}
-
-// ------------------------------------------------------------------------------------------------
-// WAVEFRONT: sorted z-slab passes
-// ------------------------------------------------------------------------------------------------
-MT_DEV uint32_t sort_key(const MtParams& P, float x, float y, float px, float py, float pz) {
-  // any mapping works (the order never changes results); NaN and far-away positions land in a border cell.
-  // The key is the xy cell the muon will be in after key_look metres of z on a straight line (about mid-slab), so
-  // that the muons of a warp fan out around a common cell instead of away from it.
-  const float t = __fdividef(P.key_look, fmaxf(pz, 0.05f));
-  x = fmaf(px, t, x);
-  y = fmaf(py, t, y);
-  const float fx = fminf(fmaxf((x - P.key_x0) * P.key_inv, 0.0f), (float)(P.key_nx - 1));
-  const float fy = fminf(fmaxf((y - P.key_y0) * P.key_inv, 0.0f), (float)(P.key_ny - 1));
-  return (uint32_t)((int)fy * P.key_nx + (int)fx);
-}
 
 // pass "-1": key and rank of every input muon (the first transport pass reads the state from the caller's arrays)
 __global__ void __launch_bounds__(256) wave_bin_kernel(const __grid_constant__ MtParams P) {
@@ -254,84 +76,6 @@ __global__ void __launch_bounds__(256) wave_perm_kernel(const __grid_constant__ 
     const uint2 k = P.sort_key[i];
     P.perm[P.key_offset[k.x] + k.y] = i;
   }
-}
-
-template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD, bool LEAN = false>
-__global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
-wave_transport_kernel(const __grid_constant__ MtParams P) {
-  const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
-  const unsigned lane = threadIdx.x & 31u;
-  const unsigned lt_mask = (1u << lane) - 1u;
-  const uint32_t n_items = *P.live_in_count;
-  Tally tally;
-
-  for (;;) {
-    // ---- the warp takes the next 32 muons of the sorted list
-    unsigned long long base = 0;
-    if (lane == 0) base = atomicAdd(P.work_counter, 32ull);
-    base = __shfl_sync(kFull, base, 0);
-    if (base >= n_items) break;
-    const uint32_t item = (uint32_t)base + lane;
-    Muon m;
-    uint32_t idx = 0;
-    int flag = -1;                                    // -1: no muon on this lane
-    m.x = m.y = m.z = m.q = m.px = m.py = m.pz = 0.0f;
-    m.step = 0;
-    if (item < n_items) {
-      const uint32_t rec = P.perm[item];
-      float4 a, b;
-      if (P.first_pass) {
-        a = __ldg(P.in_pos_q + rec); b = __ldg(P.in_mom + rec);
-        b.w = __int_as_float(0);
-        idx = rec;
-      } else {
-        const float4* r = P.rec_in + 3 * (size_t)rec;
-        a = __ldg(r); b = __ldg(r + 1);
-        idx = __ldg(reinterpret_cast<const uint32_t*>(r + 2));
-      }
-      m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z;
-      m.step = __float_as_int(b.w);
-      flag = 0;
-    }
-    const uint64_t id = P.id_base + idx;
-    const uint32_t id_lo = (uint32_t)id, id_hi = (uint32_t)(id >> 32);
-    const int step_in = m.step;
-
-    // ---- step until every lane has terminated or reached the end of the slab
-    for (;;) {
-      if (flag == 0) flag = step_once<GEOM, PACK, TAB_SMEM, true, JOINT, FIELD, true, LEAN>(P, V, m, id_lo, id_hi, P.slab_z_end);
-      if (!__any_sync(kFull, flag == 0)) break;
-    }
-    tally.steps += (unsigned)(m.step - step_in);
-
-    // ---- terminated muons: final state; parked muons: state, sort key and rank for the next pass
-    const int fin = (flag >= 1 && flag <= 4) ? flag : 0;
-    write_final(P, m, idx, fin, lane);
-    tally.count(fin);
-    const bool parked = (flag == MT_PARK);
-    const unsigned pm = __ballot_sync(kFull, parked);
-    if (pm) {
-      const int leader = __ffs(pm) - 1;
-      unsigned slot0 = 0;
-      if ((int)lane == leader) slot0 = atomicAdd(P.live_out_count, (unsigned)__popc(pm));
-      slot0 = __shfl_sync(kFull, slot0, leader);
-      if (parked) {
-        const uint32_t key = sort_key(P, m.x, m.y, m.px, m.py, m.pz);
-        const unsigned peers = __match_any_sync(pm, key);
-        const int pl = __ffs(peers) - 1;
-        unsigned r0 = 0;
-        if ((int)lane == pl) r0 = atomicAdd(P.hist + key, (unsigned)__popc(peers));
-        r0 = __shfl_sync(peers, r0, pl);
-        const unsigned slot = slot0 + (unsigned)__popc(pm & lt_mask);
-        float4* r = P.rec_out + 3 * (size_t)slot;                       // a warp's records are contiguous: full sectors
-        r[0] = make_float4(m.x, m.y, m.z, m.q);
-        r[1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
-        r[2] = make_float4(__uint_as_float(idx), 0.0f, 0.0f, 0.0f);
-        P.sort_key[slot] = make_uint2(key, r0 + (unsigned)__popc(peers & lt_mask));
-      }
-    }
-  }
-  tally.flush(P.counters, lane);
 }
 
 // ---- voxel repack: {material u8, field f32x3} -> one 32-byte record {cell x, cell x+1} per cell of a grid with a
@@ -410,51 +154,11 @@ __global__ void __launch_bounds__(256) debug_lookup_kernel(const __grid_constant
   }
 }
 
-typedef void (*kernel_fn)(const MtParams);
-
-// Instantiated combinations: geometry x table kind {pack32, pack32 + shared prefix, pack64, pack64 + shared prefix,
-// joint (pack64)} x field mode {trilinear / region, per-stage; voxel only: nearest, nearest per-stage} x schedule.
-template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD>
-kernel_fn pick_sched(int sched) {
-  switch (sched) {
-    case SCHED_STATIC: return transport_kernel<GEOM, PACK, TAB_SMEM, JOINT, FIELD, SCHED_STATIC>;
-    case SCHED_REFILL: return transport_kernel<GEOM, PACK, TAB_SMEM, JOINT, FIELD, SCHED_REFILL>;
-    default: return wave_transport_kernel<GEOM, PACK, TAB_SMEM, JOINT, FIELD>;
-  }
-}
-template <int GEOM, int FIELD>
-kernel_fn pick_tables(const MtLaunchCfg& cfg) {
-  if (cfg.joint) return pick_sched<GEOM, 64, false, true, FIELD>(cfg.sched);
-  if (cfg.pack == 32) return cfg.tab_smem ? pick_sched<GEOM, 32, true, false, FIELD>(cfg.sched)
-                                          : pick_sched<GEOM, 32, false, false, FIELD>(cfg.sched);
-  return cfg.tab_smem ? pick_sched<GEOM, 64, true, false, FIELD>(cfg.sched)
-                      : pick_sched<GEOM, 64, false, false, FIELD>(cfg.sched);
-}
-kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
-  if (cfg.lean && mt_has_lean(mode, cfg)) {
-    switch ((cfg.field & 3) | (cfg.joint ? 8 : (cfg.pack == 32 ? 0 : 4))) {
-      case 0: return wave_transport_kernel<1, 32, false, false, 0, true>;
-      case 1: return wave_transport_kernel<1, 32, false, false, 1, true>;
-      case 2: return wave_transport_kernel<1, 32, false, false, 2, true>;
-      case 3: return wave_transport_kernel<1, 32, false, false, 3, true>;
-      case 4: return wave_transport_kernel<1, 64, false, false, 0, true>;
-      case 5: return wave_transport_kernel<1, 64, false, false, 1, true>;
-      case 6: return wave_transport_kernel<1, 64, false, false, 2, true>;
-      case 7: return wave_transport_kernel<1, 64, false, false, 3, true>;
-      case 8: return wave_transport_kernel<1, 64, false, true, 0, true>;
-      case 9: return wave_transport_kernel<1, 64, false, true, 1, true>;
-      case 10: return wave_transport_kernel<1, 64, false, true, 2, true>;
-      default: return wave_transport_kernel<1, 64, false, true, 3, true>;
-    }
-  }
-  if (mode == 0) return (cfg.field & 2) ? pick_tables<0, 2>(cfg) : pick_tables<0, 0>(cfg);
-  if (mode == 2) return (cfg.field & 2) ? pick_tables<2, 2>(cfg) : pick_tables<2, 0>(cfg);
-  switch (cfg.field & 3) {
-    case 1: return pick_tables<1, 1>(cfg);
-    case 2: return pick_tables<1, 2>(cfg);
-    case 3: return pick_tables<1, 3>(cfg);
-    default: return pick_tables<1, 0>(cfg);
-  }
+mt_kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
+  if (cfg.lean && mt_has_lean(mode, cfg)) return mt_pick_lean(cfg);
+  if (mode == 0) return mt_pick_regions(cfg);
+  if (mode == 2) return mt_pick_poly(cfg);
+  return (cfg.field & 2) ? mt_pick_voxel_b(cfg) : mt_pick_voxel_a(cfg);
 }
 
 }  // namespace
@@ -467,7 +171,7 @@ bool mt_has_lean(int mode, const MtLaunchCfg& cfg) {
 // launchers (called from mt_lib.cu)
 // ------------------------------------------------------------------------------------------------
 cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream) {
-  kernel_fn fn = pick_kernel(P.mode, cfg);
+  mt_kernel_fn fn = pick_kernel(P.mode, cfg);
   cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
   if (e != cudaSuccess) return e;
   void* args[] = {(void*)&P};
@@ -475,7 +179,7 @@ cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaS
 }
 
 cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm) {
-  kernel_fn fn = pick_kernel(P.mode, cfg);
+  mt_kernel_fn fn = pick_kernel(P.mode, cfg);
   cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
   if (e != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, (const void*)fn, cfg.block, cfg.smem_bytes);

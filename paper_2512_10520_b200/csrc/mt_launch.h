@@ -25,6 +25,14 @@ struct MtLaunchCfg {
 // field mode, marginal or joint tables)
 bool mt_has_lean(int mode, const MtLaunchCfg& cfg);
 
+// the transport kernel for a launch configuration; each picker lives in the translation unit that instantiates its kernels
+typedef void (*mt_kernel_fn)(const MtParams);
+mt_kernel_fn mt_pick_regions(const MtLaunchCfg& cfg);
+mt_kernel_fn mt_pick_poly(const MtLaunchCfg& cfg);
+mt_kernel_fn mt_pick_voxel_a(const MtLaunchCfg& cfg);   // field frozen over the step
+mt_kernel_fn mt_pick_voxel_b(const MtLaunchCfg& cfg);   // field at every Runge-Kutta stage
+mt_kernel_fn mt_pick_lean(const MtLaunchCfg& cfg);      // only where mt_has_lean() holds
+
 cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream);
 cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm);
 // WAVEFRONT helpers: key + rank of the input muons; scan of the key histogram followed by the permutation that
