@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(256) wave_perm_kernel(const __grid_constant__ 
   }
 }
 
-// ---- voxel repack: {material u8, field f32x3} -> one 32-byte record {cell x, cell x+1} per cell of a grid with a
+// ---- voxel repack: {material u8, field f32x3} -> one 32-byte record {cell x, cell x+1 minus cell x} per cell of a grid with a
 // one-cell border that replicates the faces (so the clamped corner indices of DESIGN.md §3.3 need no clamps in
 // the step loop and an x-pair of corners is one load); also counts the cells of each material
 __global__ void repack_kernel(const uint8_t* __restrict__ mat, const float* __restrict__ fld, MtCellPair* __restrict__ out,
@@ -96,7 +96,10 @@ __global__ void repack_kernel(const uint8_t* __restrict__ mat, const float* __re
     const size_t s0 = row + sx, s1 = row + sx1;
     MtCellPair r;
     r.a = make_float4(fld[3 * s0], fld[3 * s0 + 1], fld[3 * s0 + 2], __int_as_float((int)mat[s0]));
-    r.b = make_float4(fld[3 * s1], fld[3 * s1 + 1], fld[3 * s1 + 2], __int_as_float((int)mat[s1]));
+    // .b holds the x-difference of §3.3's first lerp, v(x+1) - v(x) rounded once — the very subtraction the contract
+    // asks for, done here once per cell instead of once per step (0 at the replicated faces)
+    r.b = make_float4(__fsub_rn(fld[3 * s1], r.a.x), __fsub_rn(fld[3 * s1 + 1], r.a.y), __fsub_rn(fld[3 * s1 + 2], r.a.z),
+                      __int_as_float((int)mat[s1]));
     out[i] = r;
     if (x >= 1 && x <= nx && y >= 1 && y <= ny && z >= 1 && z <= nz) atomicAdd(&hist[mat[s0]], 1u);
   }

@@ -33,7 +33,8 @@ struct __align__(16) MtBlockDev {
 };
 
 // Two x-neighbours of the padded field grid in one 32-byte record, so that the x-pair of a trilinear corner set
-// is one 256-bit load.  a = cell x, b = cell x+1; .w = material id (int bits).
+// is one 256-bit load.  a = field of cell x; b = field of cell x+1 MINUS that of cell x, each component
+// rounded once (the subtraction of §3.3's x-lerp, precomputed); .w = material id of cell x / x+1 (int bits).
 struct __align__(32) MtCellPair {
   float4 a, b;
 };
