@@ -31,8 +31,8 @@ if ROOT not in sys.path:
 ALG_OPS_PER_STEP = {"voxel": 383, "regions": 308, "poly": 349}
 ALG_GATHER_BYTES_PER_STEP = {"voxel": 168, "regions": 40, "poly": 50}
 # DRAM bytes (read + written) of ONE launch of the dominant kernel, from the `ncu --set full` capture summarised in
-# profiles/r1h_transport_kernel_full.csv (mean of the three captured z-slab passes of config 3)
-NCU_DRAM_BYTES_PER_LAUNCH = {"voxel": 0.757e9, "regions": None, "poly": None}
+# profiles/r1i_transport_kernel_full.csv (mean of the three captured z-slab passes of config 3)
+NCU_DRAM_BYTES_PER_LAUNCH = {"voxel": 0.960e9, "regions": None, "poly": None}
 SM_COUNT, LANES_PER_SM = 148, 128          # B200: 4 SMSPs x 32 lanes issue one warp instruction per clock
 
 
@@ -299,7 +299,7 @@ def run_ours(args, rank, world, local_rank):
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "T thread-ops/s",
                      "frac": achieved / alu_peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH[mode],
-                     "traffic_unit": "DRAM bytes per launch of the kernel (ncu, profiles/r1h_transport_kernel_full.csv)",
+                     "traffic_unit": "DRAM bytes per launch of the kernel (ncu, profiles/r1i_transport_kernel_full.csv)",
                      "kernel": ("wave_transport_kernel: %d z-slab passes among the %d launches of a step (the rest sort the "
                                 "live list)" % ((launches_per_step - 1) // 3, launches_per_step)) if launches_per_step > 1
                      else "transport_kernel (1 launch per step)",

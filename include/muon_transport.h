@@ -160,8 +160,9 @@ typedef struct {
   const mt_poly_block* blocks; /* HOST, copied.  The library bins their bounding boxes into a uniform grid  */
                              /* over the world box (the spatial hash of L120) and tests only a cell's candidates */
 } mt_geometry;
-/* VOXEL mode repacks both grids into one library-owned 16-byte-per-cell grid {Bx,By,Bz,material}
- * (DESIGN.md §6), so the caller may free d_material / d_field after the call returns. */
+/* VOXEL mode repacks both grids into one library-owned grid of 32-byte records (field and material of a cell, and the
+ * field difference to its +x neighbour), so the caller may free d_material / d_field after the call
+ * returns.  The library's copy takes 32 bytes per cell of the grid padded by one cell on every side. */
 int mt_set_geometry(mt_ctx* ctx, const mt_geometry* geom);
 
 /* Muon state, SoA of 16-byte records (north_star subsystem 3). */

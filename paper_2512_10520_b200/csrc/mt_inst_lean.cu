@@ -1,7 +1,8 @@
-// mt_inst_lean.cu — transport-kernel instantiations for the LEAN variants: WAVEFRONT schedule on a voxel grid, tables gathered from L2.
+// mt_inst_lean.cu — transport-kernel instantiations for the LEAN variants: WAVEFRONT schedule on a voxel grid, tables gathered from L2 (and, for the default mode, staged in shared memory).
 #include "mt_kernels.cuh"
 
 mt_kernel_fn mt_pick_lean(const MtLaunchCfg& cfg) {
+  if (cfg.tab_smem) return wave_transport_kernel<1, 32, true, false, 0, true>;   // 4-byte cells, trilinear frozen only
   switch ((cfg.field & 3) | (cfg.joint ? 8 : (cfg.pack == 32 ? 0 : 4))) {
     case 0: return wave_transport_kernel<1, 32, false, false, 0, true>;
     case 1: return wave_transport_kernel<1, 32, false, false, 1, true>;

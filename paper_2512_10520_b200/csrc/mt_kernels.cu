@@ -167,7 +167,7 @@ mt_kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
 }  // namespace
 
 bool mt_has_lean(int mode, const MtLaunchCfg& cfg) {
-  return mode == 1 && cfg.sched == SCHED_WAVEFRONT && !cfg.tab_smem;
+  return mode == 1 && cfg.sched == SCHED_WAVEFRONT && (!cfg.tab_smem || (cfg.pack == 32 && !cfg.joint && (cfg.field & 3) == 0));
 }
 
 // ------------------------------------------------------------------------------------------------

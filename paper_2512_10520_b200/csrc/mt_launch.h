@@ -22,7 +22,8 @@ struct MtLaunchCfg {
   bool lean;       // P.lean == MT_LEAN_ALL and a LEAN kernel exists for this combination (mt_has_lean)
 };
 // LEAN variants are compiled for the WAVEFRONT schedule on a voxel geometry with the tables gathered from L2 (every
-// field mode, marginal or joint tables)
+// field mode, marginal or joint tables) and, for marginal 4-byte cells with the trilinear frozen field, staged in
+// shared memory
 bool mt_has_lean(int mode, const MtLaunchCfg& cfg);
 
 // the transport kernel for a launch configuration; each picker lives in the translation unit that instantiates its kernels
