@@ -2,5 +2,6 @@
 #include "mt_kernels.cuh"
 
 mt_kernel_fn mt_pick_regions(const MtLaunchCfg& cfg) {
+  if (cfg.lean) return (cfg.field & 2) ? pick_tables_lean<0, 2>(cfg) : pick_tables_lean<0, 0>(cfg);
   return (cfg.field & 2) ? pick_tables<0, 2>(cfg) : pick_tables<0, 0>(cfg);
 }

@@ -158,16 +158,20 @@ __global__ void __launch_bounds__(256) debug_lookup_kernel(const __grid_constant
 }
 
 mt_kernel_fn pick_kernel(int mode, const MtLaunchCfg& cfg) {
-  if (cfg.lean && mt_has_lean(mode, cfg)) return mt_pick_lean(cfg);
-  if (mode == 0) return mt_pick_regions(cfg);
-  if (mode == 2) return mt_pick_poly(cfg);
+  MtLaunchCfg c = cfg;
+  c.lean = cfg.lean && mt_has_lean(mode, cfg);
+  if (mode == 1 && c.lean) return mt_pick_lean(c);
+  if (mode == 0) return mt_pick_regions(c);
+  if (mode == 2) return mt_pick_poly(c);
   return (cfg.field & 2) ? mt_pick_voxel_b(cfg) : mt_pick_voxel_a(cfg);
 }
 
 }  // namespace
 
 bool mt_has_lean(int mode, const MtLaunchCfg& cfg) {
-  return mode == 1 && cfg.sched == SCHED_WAVEFRONT && (!cfg.tab_smem || (cfg.pack == 32 && !cfg.joint && (cfg.field & 3) == 0));
+  const bool staged_ok = !cfg.tab_smem || (cfg.pack == 32 && !cfg.joint);
+  if (mode == 1) return cfg.sched == SCHED_WAVEFRONT && staged_ok && (!cfg.tab_smem || (cfg.field & 3) == 0);
+  return (cfg.sched == SCHED_REFILL || cfg.sched == SCHED_WAVEFRONT) && staged_ok;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -102,7 +102,7 @@ MT_DEV void write_final(const MtParams& P, const Muon& m, uint32_t idx, int flag
 // ------------------------------------------------------------------------------------------------
 // STATIC and REFILL
 // ------------------------------------------------------------------------------------------------
-template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD, int SCHED>
+template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD, int SCHED, bool LEAN = false>
 __global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
 transport_kernel(const __grid_constant__ MtParams P) {
   const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
@@ -158,7 +158,7 @@ transport_kernel(const __grid_constant__ MtParams P) {
       int flag = 0;
       if (active) {
         const uint64_t id = P.id_base + idx;
-        flag = step_once<GEOM, PACK, TAB_SMEM, false, JOINT, FIELD>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
+        flag = step_once<GEOM, PACK, TAB_SMEM, false, JOINT, FIELD, true, LEAN>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
         if (flag == 0) tally.steps += 1;
       }
       write_final(P, m, idx, flag, lane);
@@ -283,6 +283,20 @@ mt_kernel_fn pick_tables(const MtLaunchCfg& cfg) {
                                           : pick_sched<GEOM, 32, false, false, FIELD>(cfg.sched);
   return cfg.tab_smem ? pick_sched<GEOM, 64, true, false, FIELD>(cfg.sched)
                       : pick_sched<GEOM, 64, false, false, FIELD>(cfg.sched);
+}
+// LEAN variants of a region / polyhedra geometry (MT_LEAN_AXES only): REFILL and WAVEFRONT; joint, 8-byte or 4-byte
+// cells from L2, 4-byte cells staged in shared memory (mt_has_lean)
+template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD>
+mt_kernel_fn pick_sched_lean(int sched) {
+  if (sched == SCHED_REFILL) return transport_kernel<GEOM, PACK, TAB_SMEM, JOINT, FIELD, SCHED_REFILL, true>;
+  return wave_transport_kernel<GEOM, PACK, TAB_SMEM, JOINT, FIELD, true>;
+}
+template <int GEOM, int FIELD>
+mt_kernel_fn pick_tables_lean(const MtLaunchCfg& cfg) {
+  if (cfg.joint) return pick_sched_lean<GEOM, 64, false, true, FIELD>(cfg.sched);
+  if (cfg.pack == 32) return cfg.tab_smem ? pick_sched_lean<GEOM, 32, true, false, FIELD>(cfg.sched)
+                                          : pick_sched_lean<GEOM, 32, false, false, FIELD>(cfg.sched);
+  return pick_sched_lean<GEOM, 64, false, false, FIELD>(cfg.sched);
 }
 
 }  // namespace

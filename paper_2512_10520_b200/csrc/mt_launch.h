@@ -21,9 +21,9 @@ struct MtLaunchCfg {
   int field;       // MT_FIELD_* of the geometry
   bool lean;       // P.lean == MT_LEAN_ALL and a LEAN kernel exists for this combination (mt_has_lean)
 };
-// LEAN variants are compiled for the WAVEFRONT schedule on a voxel geometry with the tables gathered from L2 (every
-// field mode, marginal or joint tables) and, for marginal 4-byte cells with the trilinear frozen field, staged in
-// shared memory
+// LEAN variants exist for: voxel grids under WAVEFRONT (every field mode, marginal or joint tables from L2; marginal
+// 4-byte cells staged in shared memory with the trilinear frozen field); regions and polyhedra under REFILL and WAVEFRONT
+// (tables from L2, or 4-byte cells staged in shared memory)
 bool mt_has_lean(int mode, const MtLaunchCfg& cfg);
 
 // the transport kernel for a launch configuration; each picker lives in the translation unit that instantiates its kernels

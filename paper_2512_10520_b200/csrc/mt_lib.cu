@@ -719,7 +719,9 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   }
   P.hot_cells = (uint32_t)(hot_blocks * block_cells);
   cfg.tab_smem = hot_blocks > 0;
-  cfg.lean = !c->opt_no_lean && P.lean == MT_LEAN_ALL && mt_has_lean(c->geom.mode, cfg);
+  // voxel grids need both facts (the lean kernel has no inside-grid test), regions and polyhedra the axes fact only
+  const bool facts = (c->geom.mode == MT_GEOM_VOXEL) ? (P.lean == MT_LEAN_ALL) : ((P.lean & MT_LEAN_AXES) != 0);
+  cfg.lean = !c->opt_no_lean && facts && mt_has_lean(c->geom.mode, cfg);
   c->last_lean = cfg.lean; c->last_sched = sched;
   cfg.smem_bytes = blob_b + ((hot_blocks * block_cells * cell_b + 15) & ~(size_t)15) + 16;
 

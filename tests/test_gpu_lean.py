@@ -117,3 +117,32 @@ def test_lean_variants_of_the_other_voxel_modes(mt, oracle, joint, field_mode):
     for got in (lean, gen):
         c = compare(got, ref)
         assert c["bit_exact"] == 1.0 and c["matched"] >= 0.999
+
+
+@pytest.mark.parametrize("which,sched", [("config1", 0), ("config2", 0), ("config2", 3), ("config2p", 0), ("config2p", 2),
+                                         ("config2_joint", 0), ("config2p_per_stage", 0)])
+def test_lean_variants_of_regions_and_polyhedra(mt, oracle, which, sched):
+    # regions and polyhedra take the lean kernels on the table facts alone (clamps, caps, theta < pi/4): REFILL and
+    # WAVEFRONT, tables from L2 or (config 1: 38 KB) staged in shared memory
+    import torch
+    from paper_2512_10520_b200 import workloads as w
+    b = mt.binding
+    wl = {"config1": lambda: w.config1(n=20_000, n_draws=100_000),
+          "config2": lambda: w.config2(n=40_000, n_draws=100_000, n_cells=4),
+          "config2p": lambda: w.config2p(n=40_000, n_draws=100_000, n_cells=4),
+          "config2_joint": lambda: w.config2(n=20_000, n_draws=100_000, n_cells=2, joint=True, table_shape=(20, 32, 16)),
+          "config2p_per_stage": lambda: w.config2p(n=20_000, n_draws=100_000, n_cells=2, field_mode=w.FIELD_PER_STAGE)}[which]()
+    ref = oracle_transport(oracle, wl)
+    for no_lean in (0, 1):
+        h = b.MuonTransport(0).setup(wl.hist, wl.geom)
+        try:
+            h.set_option(b.MT_OPT_NO_LEAN, no_lean).set_option(b.MT_OPT_SCHEDULE, sched)
+            out = h.transport(torch.from_numpy(wl.muons.pos_q).cuda(), torch.from_numpy(wl.muons.mom).cuda(), wl.seed)
+            torch.cuda.synchronize()
+            assert b.mt_get_info(h.ctx, b.MT_INFO_LEAN_FACTS) & 1
+            assert b.mt_get_info(h.ctx, b.MT_INFO_LAST_LEAN) == 1 - no_lean
+            got = unpack(out["pos_flag"].cpu().numpy(), out["mom_steps"].cpu().numpy())
+        finally:
+            h.close()
+        c = compare(got, ref)
+        assert c["bit_exact"] == 1.0 and c["matched"] >= 0.999
