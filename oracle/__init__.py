@@ -297,6 +297,17 @@ def transport(tables, geom, pos_q, mom, seed, id_base=0, ids=None, dtype=np.floa
     return dict(pos=out_pos, mom=out_mom, flag=flag, steps=steps)
 
 
+def exit_project(pos, mom, z_exit, dtype=np.float32):
+    """positions [n,3] of EXITED muons projected back onto the plane z = z_exit along mom [n,3]."""
+    pos = np.array(_c(pos, dtype).reshape(-1, 3), copy=True)
+    mom = _c(mom, dtype).reshape(-1, 3)
+    if dtype == np.float64:
+        lib().orc_exit_project_f64(_p(pos), _p(mom), C.c_uint64(len(pos)), C.c_double(z_exit))
+    else:
+        lib().orc_exit_project_f32(_p(pos), _p(mom), C.c_uint64(len(pos)), C.c_float(z_exit))
+    return pos
+
+
 def trace(tables, geom, pos_q, mom, seed, muon_id, cap=20000):
     """one muon in float32 with its per-step (material, pbin, cell_dp, cell_th) record"""
     og = geom if isinstance(geom, OracleGeometry) else OracleGeometry(geom)

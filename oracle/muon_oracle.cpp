@@ -18,6 +18,7 @@
 //   termination ............... L65, L149
 //   joint 2D histogram mode ... L77 (§3), Fig. 3 L95, L163
 //   nearest-neighbour field ... L133 (§4.3); per-stage field evaluation: Eq. 4 integrated by RK4 proper
+//   exit record on the plane .. L182: straight-line projection of an EXITED muon back onto z_exit
 //   convex-polyhedra lookup ... L109-120 (§4.1), Eq. 2; the spatial hash of L120 only prunes, so the
 //                               oracle scans every block
 //
@@ -32,7 +33,8 @@
 // Rodrigues (Eq. 3) in double; trilinear on affine fields; region lookup vs brute force;
 // exp2/sin/cos polynomials vs libm; two-word alias draw vs the exact pmf of the table; joint-mode kick vs its
 // geometry; nearest field vs the stored cell values; per-stage push vs h^4 convergence in a field gradient;
-// polyhedra containment vs scipy's convex hull of the eight vertices, the prismatoid volume, and the box regions.  Physics fidelity vs Geant4 (Figs. 5, 7): parity unpinned
+// polyhedra containment vs scipy's convex hull of the eight vertices, the prismatoid volume, and the box regions;
+// exit projection vs the exact plane crossing of a straight line and the sagitta bound in a uniform field.  Physics fidelity vs Geant4 (Figs. 5, 7): parity unpinned
 // (needs Geant4 histograms, not available).
 
 #include <cmath>
@@ -553,6 +555,15 @@ int transport_many(const Tables& T, const Geometry& g, uint64_t seed, uint64_t i
   return 0;
 }
 
+// the exit record of an EXITED muon moved back onto the plane z = z_exit along its final direction
+template <class R> void exit_project(R r[3], const R p[3], R z_exit) {
+  if (!(p[2] > (R)0)) return;
+  const R s = (r[2] - z_exit) / p[2];
+  r[0] = std::fma(-s, p[0], r[0]);
+  r[1] = std::fma(-s, p[1], r[1]);
+  r[2] = z_exit;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------
@@ -675,6 +686,13 @@ int orc_trace_f32(const Tables* T, const Geometry* g, uint64_t seed, uint64_t id
                        reinterpret_cast<StepTrace*>(trace), cap);
   for (int i = 0; i < 3; ++i) { out_pos[i] = r[i]; out_mom[i] = p[i]; }
   return 0;
+}
+
+void orc_exit_project_f32(float* pos, const float* mom, uint64_t n, float z_exit) {
+  for (uint64_t i = 0; i < n; ++i) exit_project<float>(pos + 3 * i, mom + 3 * i, z_exit);
+}
+void orc_exit_project_f64(double* pos, const double* mom, uint64_t n, double z_exit) {
+  for (uint64_t i = 0; i < n; ++i) exit_project<double>(pos + 3 * i, mom + 3 * i, z_exit);
 }
 
 int orc_max_threads(void) {
