@@ -59,6 +59,12 @@ enum {
   MT_FIELD_PER_STAGE = 2   /* flag: B looked up at every Runge-Kutta stage position instead of once per step       */
 };
 
+/* where the compact exit list records an EXITED muon (mt_geometry.exit_mode) */
+enum {
+  MT_EXIT_AT_BREAK = 0,    /* its state at the break of Algorithm 1: up to one step length behind the exit plane (default) */
+  MT_EXIT_PROJECT = 1      /* moved back onto the plane z = z_exit along its final direction; momentum unchanged.  The  */
+};                         /* dense outputs pos_flag / mom_steps are never changed by this                              */
+
 /* alias-table placement (north_star subsystem 1) */
 enum { MT_PLACE_AUTO = 0, MT_PLACE_SMEM = 1, MT_PLACE_L2 = 2 };
 
@@ -159,6 +165,7 @@ typedef struct {
   int32_t n_blocks;          /* POLY mode: 0..1024                                                           */
   const mt_poly_block* blocks; /* HOST, copied.  The library bins their bounding boxes into a uniform grid  */
                              /* over the world box (the spatial hash of L120) and tests only a cell's candidates */
+  int32_t exit_mode;         /* MT_EXIT_AT_BREAK | MT_EXIT_PROJECT: what mt_muons_out.exit_rec holds         */
 } mt_geometry;
 /* VOXEL mode repacks both grids into one library-owned grid of 32-byte records (field and material of a cell, and the
  * field difference to its +x neighbour), so the caller may free d_material / d_field after the call
@@ -174,7 +181,8 @@ typedef struct {
 typedef struct {
   float* pos_flag;         /* [n][4] = final x, y, z, flag (int32 bits in the 4th float)                   */
   float* mom_steps;        /* [n][4] = final px, py, pz, step count (int32 bits)                           */
-  float* exit_rec;         /* optional [exit_capacity][8]: x,y,z,index(uint32 bits),px,py,pz,steps(int32)  */
+  float* exit_rec;         /* optional [exit_capacity][8]: x,y,z,index(uint32 bits),px,py,pz,steps(int32);  */
+                           /* x,y,z per mt_geometry.exit_mode                                              */
   uint32_t* exit_count;    /* optional, one counter; ADDED to (caller zeroes it); may exceed the capacity  */
   uint32_t exit_capacity;
   uint64_t* counters;      /* optional [8], ADDED to: [0] total steps, [1..4] muons per flag               */

@@ -19,6 +19,7 @@ MT_SCHED_AUTO, MT_SCHED_STATIC, MT_SCHED_REFILL, MT_SCHED_WAVEFRONT = 0, 1, 2, 3
 MT_OPT_SCHEDULE, MT_OPT_BLOCK_THREADS, MT_OPT_BLOCKS_PER_SM, MT_OPT_SLAB_CELLS, MT_OPT_REFILL_MIN_IDLE = 1, 2, 3, 4, 5
 MT_OPT_KEY_LOOKAHEAD, MT_OPT_HASH_NXY, MT_OPT_HASH_NZ, MT_OPT_NO_LEAN = 6, 7, 8, 9
 MT_HIST_MARGINAL, MT_HIST_JOINT = 0, 1
+MT_EXIT_AT_BREAK, MT_EXIT_PROJECT = 0, 1
 MT_INFO_LEAN_FACTS, MT_INFO_LAST_LEAN, MT_INFO_LAST_SCHEDULE = 1, 2, 3
 MT_FIELD_TRILINEAR, MT_FIELD_NEAREST, MT_FIELD_PER_STAGE = 0, 1, 2
 
@@ -55,7 +56,7 @@ class mt_geometry(C.Structure):
                 ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("ox", C.c_float), ("oy", C.c_float), ("oz", C.c_float), ("cell", C.c_float),
                 ("d_material", C.c_void_p), ("d_field", C.c_void_p), ("field_mode", C.c_int32),
-                ("n_blocks", C.c_int32), ("blocks", C.c_void_p)]
+                ("n_blocks", C.c_int32), ("blocks", C.c_void_p), ("exit_mode", C.c_int32)]
 
 
 class mt_muons_in(C.Structure):
@@ -181,6 +182,7 @@ def mt_set_geometry(ctx, geom):
     g.x_min, g.x_max, g.y_min, g.y_max, g.z_min, g.z_exit = geom.x_min, geom.x_max, geom.y_min, geom.y_max, geom.z_min, geom.z_exit
     g.p_min, g.max_steps, g.world_material = geom.p_min, geom.max_steps, geom.world_material
     g.field_mode = int(getattr(geom, "field_mode", 0))
+    g.exit_mode = int(getattr(geom, "exit_mode", 0))
     keep = None
     if geom.mode == MT_GEOM_REGIONS:
         regs = np.ascontiguousarray(geom.regions) if geom.regions is not None else np.zeros(0, np.uint8)

@@ -91,7 +91,13 @@ MT_DEV void write_final(const MtParams& P, const Muon& m, uint32_t idx, int flag
       if (ex) {
         const unsigned slot = base + (unsigned)__popc(em & ((1u << lane) - 1u));
         if (slot < P.exit_capacity) {
-          P.exit_rec[2 * (size_t)slot] = make_float4(m.x, m.y, m.z, __uint_as_float(idx));
+          float ex = m.x, ey = m.y, ez = m.z;
+          if (P.exit_mode == 1 && m.pz > 0.0f) {
+            // §3.13: back onto the plane along the final direction (one IEEE division, two fma)
+            const float s = __fdiv_rn(mt::sub(m.z, P.z_exit), m.pz);
+            ex = mt::fma(-s, m.px, m.x); ey = mt::fma(-s, m.py, m.y); ez = P.z_exit;
+          }
+          P.exit_rec[2 * (size_t)slot] = make_float4(ex, ey, ez, __uint_as_float(idx));
           P.exit_rec[2 * (size_t)slot + 1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
         }
       }

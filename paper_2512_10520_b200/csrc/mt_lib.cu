@@ -520,6 +520,7 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
     return fail(c, MT_ERR_INVALID_ARG, "empty world box");
   if (gm->max_steps < 0 || gm->world_material < 0 || gm->world_material > c->n_materials)
     return fail(c, MT_ERR_INVALID_ARG, "bad max_steps or world_material");
+  if (gm->exit_mode != MT_EXIT_AT_BREAK && gm->exit_mode != MT_EXIT_PROJECT) return fail(c, MT_ERR_INVALID_ARG, "bad exit_mode");
   if (gm->field_mode < 0 || gm->field_mode > (MT_FIELD_NEAREST | MT_FIELD_PER_STAGE))
     return fail(c, MT_ERR_INVALID_ARG, "bad field_mode");
   if ((gm->field_mode & MT_FIELD_NEAREST) && gm->mode != MT_GEOM_VOXEL)
@@ -651,6 +652,7 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.cells_per_bin = joint ? P.n_joint : (uint32_t)(c->n_dp + c->n_th);
   P.nth_magic = (uint32_t)((((uint64_t)1 << 32) + (uint64_t)c->n_th - 1) / (uint64_t)c->n_th);   // n_th = 1 wraps to 0: unused then
   P.field_mode = g.field_mode;
+  P.exit_mode = g.exit_mode;
   P.n_blocks = g.n_blocks;
   P.hash_cells = (const uint2*)c->d_hash.p;
   P.hash_list = (const uint16_t*)((const char*)c->d_hash.p + c->hash_list_off);

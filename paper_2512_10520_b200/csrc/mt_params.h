@@ -78,6 +78,7 @@ struct MtParams {
   uint32_t n_joint;              // JOINT mode: n_dp * n_th cells per table, pack64 cells
   uint32_t nth_magic;            // ceil(2^32 / n_th): cell / n_th == umulhi(cell, nth_magic) for cell * n_th < 2^32
   int32_t field_mode;            // MT_FIELD_*
+  int32_t exit_mode;             // MT_EXIT_* (DESIGN.md §3.13): what the compact exit list records
   // ---- POLY mode: spatial hash over the world box; a cell lists, in ascending order, the blocks whose
   //      padded bounding box meets it
   int32_t n_blocks;

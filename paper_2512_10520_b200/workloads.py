@@ -71,6 +71,7 @@ class Geometry:
     field: object = None                # float32 [nz][ny][nx][3]
     field_mode: int = 0                 # FIELD_NEAREST | FIELD_PER_STAGE; 0 = trilinear, frozen
     blocks: np.ndarray = None           # POLY_DTYPE (MODE_POLY); the first block that contains a point wins
+    exit_mode: int = 0                  # 1: the compact exit list is projected back onto the exit plane
 
 
 @dataclass

@@ -30,7 +30,7 @@ def test_struct_layouts_match_the_header(mt):
     assert ctypes.sizeof(b.mt_region) == 40
     assert ctypes.sizeof(b.mt_hist_desc) == 24 + 5 * 8 + 8 and b.mt_hist_desc.hist_mode.offset == 64
     assert b.mt_geometry.regions.offset == 48 and b.mt_geometry.d_material.offset == 88
-    assert ctypes.sizeof(b.mt_geometry) == 120 and b.mt_geometry.field_mode.offset == 104
+    assert ctypes.sizeof(b.mt_geometry) == 128 and b.mt_geometry.field_mode.offset == 104 and b.mt_geometry.exit_mode.offset == 120
     assert b.mt_geometry.n_blocks.offset == 108 and b.mt_geometry.blocks.offset == 112
     assert ctypes.sizeof(b.mt_poly_block) == 88 and b.mt_poly_block.xy_hi.offset == 40 and b.mt_poly_block.material.offset == 72
     from paper_2512_10520_b200.workloads import POLY_DTYPE, REGION_DTYPE

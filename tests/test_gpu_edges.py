@@ -123,6 +123,32 @@ def test_exit_records_and_counters(mt, wl1, ref1):
     assert np.array_equal(g["counters"][1:5], np.bincount(ref1["flag"], minlength=5)[1:5])
 
 
+@pytest.mark.parametrize("sched", [1, 2, 3])
+def test_exit_records_projected_onto_the_plane(mt, oracle, wl1, ref1, sched):
+    # with MT_EXIT_PROJECT the compact list holds the oracle's projection of every EXITED muon, bit for
+    # bit; the dense outputs stay the state at the break
+    import copy
+    wl = copy.copy(wl1)
+    wl.geom = copy.copy(wl1.geom)
+    wl.geom.exit_mode = 1
+    n = len(ref1["flag"])
+    hit = np.nonzero(ref1["flag"] == 2)[0]
+    g = gpu_transport(mt, wl, sched=sched, exit_capacity=n)
+    assert g["exit_count"] == len(hit)
+    for k in ("pos", "mom", "flag", "steps"):
+        assert np.array_equal(g[k], ref1[k]), k
+    rec = g["exit_rec"][:len(hit)]
+    idx = rec[:, 3].copy().view(np.uint32)
+    assert np.array_equal(np.sort(idx), hit)
+    want = oracle.exit_project(ref1["pos"][idx], ref1["mom"][idx], wl.geom.z_exit, dtype=np.float32)
+    assert np.array_equal(rec[:, :3].view(np.uint32), want.view(np.uint32))
+    assert np.all(rec[:, 2] == np.float32(wl.geom.z_exit)) and np.any(ref1["pos"][idx][:, 2] > wl.geom.z_exit)
+    assert np.array_equal(rec[:, 4:7], ref1["mom"][idx])
+    # the projection moved the points by up to a step's worth of transverse travel
+    moved = np.abs(rec[:, :2] - ref1["pos"][idx][:, :2]).max()
+    assert 1e-5 < moved < 0.02
+
+
 def test_host_buffer_call(mt, wl1, ref1):
     import torch
     b = mt.binding
