@@ -10,7 +10,9 @@
  *
  * Conventions.  Units: metres, GeV/c, tesla.  Every function returns an int status: MT_OK (0) or a
  * negative MT_ERR_* code; nothing throws or aborts across this boundary; mt_last_error() gives a text for
- * the last failure on a context.  A context belongs to one CUDA device and is not thread-safe.  "HOST"
+ * the last failure on a context.  A context belongs to one CUDA device and is not thread-safe; its transports share
+ * library-owned scratch, so successive mt_transport calls on one context must be ordered on the device (same stream, or
+ * streams synchronised by the caller).  "HOST"
  * pointers are ordinary host memory, read during the call and never retained.  "DEVICE" pointers are
  * CUDA device memory on the context's device; the caller owns them (the library never frees them), and
  * those marked "borrowed" must stay valid and unchanged until the context is destroyed or the geometry is
