@@ -58,7 +58,7 @@ def lib():
         _lib.orc_rk4_f32.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_float, C.c_int]
         _lib.orc_make_edges.argtypes = [C.c_double, C.c_double, C.c_int, C.c_void_p]
         _lib.orc_muon_words.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_void_p]
-        for name in ("orc_transport_f32", "orc_transport_f64"):
+        for name in ("orc_transport_f32", "orc_transport_f64", "orc_transport_libm_f32", "orc_transport_libm_f64"):
             getattr(_lib, name).argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_void_p,
                                             C.c_uint64] + [C.c_void_p] * 6 + [C.c_int]
         _lib.orc_trace_f32.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64] + [C.c_void_p] * 7 + [C.c_int32]
@@ -279,9 +279,11 @@ class OracleTables:
         return make_edges(self.struct.p_lo, self.struct.p_hi, self.h.n_pbins)
 
 
-def transport(tables, geom, pos_q, mom, seed, id_base=0, ids=None, dtype=np.float32, threads=1):
+def transport(tables, geom, pos_q, mom, seed, id_base=0, ids=None, dtype=np.float32, threads=1, libm=False):
     """Algorithm 1 for every muon.  pos_q [n,4] = x,y,z,q; mom [n,4] = px,py,pz,-.
 
+    libm=True: the witness mode — the C library's exp2 / sin / cos in place of the fixed polynomials of DESIGN.md
+    §3.6 (not the parity reference: used to exercise north_star's tolerance against the plain definitions).
     Returns dict(pos [n,3], mom [n,3], flag [n] int32, steps [n] int32) in `dtype`."""
     og = geom if isinstance(geom, OracleGeometry) else OracleGeometry(geom)
     pos_q, mom = _c(pos_q, dtype).reshape(-1, 4), _c(mom, dtype).reshape(-1, 4)
@@ -289,7 +291,7 @@ def transport(tables, geom, pos_q, mom, seed, id_base=0, ids=None, dtype=np.floa
     out_pos, out_mom = np.empty((n, 3), dtype), np.empty((n, 3), dtype)
     flag, steps = np.empty(n, np.int32), np.empty(n, np.int32)
     ids_arr = _c(ids, np.uint64) if ids is not None else None
-    fn = lib().orc_transport_f64 if dtype == np.float64 else lib().orc_transport_f32
+    fn = getattr(lib(), "orc_transport_%s%s" % ("libm_" if libm else "", "f64" if dtype == np.float64 else "f32"))
     rc = fn(C.byref(tables.struct), C.byref(og.struct), seed, id_base,
             _p(ids_arr) if ids_arr is not None else None, n,
             _p(pos_q), _p(mom), _p(out_pos), _p(out_mom), _p(flag), _p(steps), int(threads))

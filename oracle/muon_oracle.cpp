@@ -210,6 +210,24 @@ template <class R> void sincos_polar(R theta, R* sn, R* cs) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// The libm witness (R-21, §9): the plain definitions that the fixed polynomials of §3.6 stand for —
+// 2^y, sin and cos from the C library in Real, the azimuth as phi = 2 pi u.  ELEM_LIBM runs Algorithm 1 with these in
+// place of exp2c / sincos_polar / sincos_azimuth and nothing else changed; it is not the parity reference (its last
+// bits are the C library's), it is the second witness against which north_star's real tolerance (>= 99.9 % of muons
+// within 1e-5 relative in |p| and 1e-5 m, KS on the rest) is exercised.
+// ------------------------------------------------------------------------------------------------
+enum { ELEM_CONTRACT = 0, ELEM_LIBM = 1 };
+template <class R> R exp2_libm(R y) { return std::exp2(y); }
+template <class R> void sincos_polar_libm(R theta, R* sn, R* cs) {
+  theta = std::min(theta, (R)0x1.921fb6p+1f);          // the same cap at pi as §3.6c
+  *sn = std::sin(theta); *cs = std::cos(theta);
+}
+template <class R> void sincos_azimuth_libm(uint32_t k24, R* sn, R* cs) {
+  const R phi = (R)6.283185307179586 * ((R)k24 * (R)0x1p-24f);       // phi = 2 pi u (L161)
+  *sn = std::sin(phi); *cs = std::cos(phi);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Geometry.  DESIGN.md §3.2, §3.8.
 // ------------------------------------------------------------------------------------------------
 struct Region { float z_lo, z_hi, x_lo, x_hi, y_lo, y_hi; int32_t material; float bx, by, bz; };
@@ -465,7 +483,7 @@ enum { FLAG_STOPPED = 1, FLAG_EXITED = 2, FLAG_ESCAPED = 3, FLAG_MAXSTEPS = 4 };
 
 struct StepTrace { int32_t material, pbin, cell_dp, cell_th; };
 
-template <class R>
+template <class R, int ELEM = ELEM_CONTRACT>
 void transport_one(const Tables& T, const float* edges, const Geometry& g, uint64_t seed, uint64_t id,
                    R r[3], R p[3], R q, int32_t* flag_out, int32_t* steps_out,
                    StepTrace* trace, int32_t trace_cap) {
@@ -510,16 +528,20 @@ void transport_one(const Tables& T, const float* edges, const Geometry& g, uint6
       const R yd = rfma<R>((R)cd + ud, (R)T.axis_dp[2 * t + 1], (R)T.axis_dp[2 * t]);
       const R yt = rfma<R>((R)ct + ut, (R)T.axis_th[2 * t + 1], (R)T.axis_th[2 * t]);
       R sphi, cphi;
-      sincos_azimuth<R>(w[3] >> 8, &sphi, &cphi);
+      if (ELEM == ELEM_LIBM) sincos_azimuth_libm<R>(w[3] >> 8, &sphi, &cphi);
+      else sincos_azimuth<R>(w[3] >> 8, &sphi, &cphi);
+      const R vd = (ELEM == ELEM_LIBM) ? exp2_libm<R>(yd) : exp2c<R>(yd);
+      const R vt = (ELEM == ELEM_LIBM) ? exp2_libm<R>(yt) : exp2c<R>(yt);
       if (T.joint) {
-        const R fz = std::min(exp2c<R>(yd), F_MAX);
-        const R ft = exp2c<R>(yt);
+        const R fz = std::min(vd, F_MAX);
+        const R ft = vt;
         Pn = kick_joint<R>(p, P, fz, ft, sphi, cphi);
       } else {
-        const R f = std::min(exp2c<R>(yd), F_MAX);
-        const R theta = exp2c<R>(yt);
+        const R f = std::min(vd, F_MAX);
+        const R theta = vt;
         R st, ctv;
-        sincos_polar<R>(theta, &st, &ctv);
+        if (ELEM == ELEM_LIBM) sincos_polar_libm<R>(theta, &st, &ctv);
+        else sincos_polar<R>(theta, &st, &ctv);
         // l.10-11 kick in the muon's frame, rotated to the lab (Eq. 3)
         Pn = kick<R>(p, P, f, st, ctv, sphi, cphi);
       }
@@ -534,7 +556,7 @@ void transport_one(const Tables& T, const float* edges, const Geometry& g, uint6
   *steps_out = step;
 }
 
-template <class R>
+template <class R, int ELEM = ELEM_CONTRACT>
 int transport_many(const Tables& T, const Geometry& g, uint64_t seed, uint64_t id_base,
                    const uint64_t* ids, uint64_t n, const R* pos_q, const R* mom,
                    R* out_pos, R* out_mom, int32_t* out_flag, int32_t* out_steps, int threads) {
@@ -549,7 +571,7 @@ int transport_many(const Tables& T, const Geometry& g, uint64_t seed, uint64_t i
     R p[3] = {mom[4 * k], mom[4 * k + 1], mom[4 * k + 2]};
     const R q = pos_q[4 * k + 3];
     const uint64_t id = ids ? ids[k] : id_base + (uint64_t)k;
-    transport_one<R>(T, edges.data(), g, seed, id, r, p, q, &out_flag[k], &out_steps[k], nullptr, 0);
+    transport_one<R, ELEM>(T, edges.data(), g, seed, id, r, p, q, &out_flag[k], &out_steps[k], nullptr, 0);
     for (int i = 0; i < 3; ++i) { out_pos[3 * k + i] = r[i]; out_mom[3 * k + i] = p[i]; }
   }
   return 0;
@@ -673,6 +695,18 @@ int orc_transport_f64(const Tables* T, const Geometry* g, uint64_t seed, uint64_
                       uint64_t n, const double* pos_q, const double* mom, double* out_pos, double* out_mom,
                       int32_t* out_flag, int32_t* out_steps, int threads) {
   return transport_many<double>(*T, *g, seed, id_base, ids, n, pos_q, mom, out_pos, out_mom, out_flag, out_steps, threads);
+}
+
+// the libm witness (ELEM_LIBM): same loop, C-library 2^y / sin / cos instead of the polynomials of DESIGN.md §3.6
+int orc_transport_libm_f32(const Tables* T, const Geometry* g, uint64_t seed, uint64_t id_base, const uint64_t* ids,
+                           uint64_t n, const float* pos_q, const float* mom, float* out_pos, float* out_mom,
+                           int32_t* out_flag, int32_t* out_steps, int threads) {
+  return transport_many<float, ELEM_LIBM>(*T, *g, seed, id_base, ids, n, pos_q, mom, out_pos, out_mom, out_flag, out_steps, threads);
+}
+int orc_transport_libm_f64(const Tables* T, const Geometry* g, uint64_t seed, uint64_t id_base, const uint64_t* ids,
+                           uint64_t n, const double* pos_q, const double* mom, double* out_pos, double* out_mom,
+                           int32_t* out_flag, int32_t* out_steps, int threads) {
+  return transport_many<double, ELEM_LIBM>(*T, *g, seed, id_base, ids, n, pos_q, mom, out_pos, out_mom, out_flag, out_steps, threads);
 }
 
 // one muon, float32, with the per-step (material, pbin, cells) record
