@@ -100,20 +100,20 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ workload
-def make_workload(config, n_muons, device, rank, joint=False, field_mode=0, poly=False):
+def make_workload(config, n_muons, device, rank, joint=False, field_mode=0, poly=False, n_draws=1_000_000):
     """BASELINE.json configs[config] with this rank's batch of muons (generator batch = rank)."""
     from paper_2512_10520_b200 import workloads as w
     t0 = time.time()
     if config == 3:
-        wl = w.config3(n=8, device=device, joint=joint, field_mode=field_mode)   # histograms + voxel grids (made on the GPU)
+        wl = w.config3(n=8, device=device, joint=joint, field_mode=field_mode, n_draws=n_draws)   # histograms + voxel grids (made on the GPU)
         wl.muons = w.spectrum_muons(3, n_muons, "square", batch=rank)
     elif config == 2:
         # --poly: config 2's muons and tables in the tapered-magnet polyhedra geometry (DESIGN.md §3.12)
-        wl = w.config2p(n=8, joint=joint) if poly else w.config2(n=8, joint=joint)
+        wl = w.config2p(n=8, joint=joint, n_draws=n_draws) if poly else w.config2(n=8, joint=joint, n_draws=n_draws)
         wl.geom.field_mode = field_mode & 2
         wl.muons = w.spectrum_muons(2, n_muons, "square", batch=rank)
     elif config == 1:
-        wl = w.config1(n=8, joint=joint)
+        wl = w.config1(n=8, joint=joint, n_draws=n_draws)
         wl.geom.field_mode = field_mode & 2
         wl.muons = w.spectrum_muons(1, n_muons, "gauss", batch=rank)
     else:
@@ -147,12 +147,16 @@ def oracle_sample(wl, n_muons, id_base, target_seconds, threads=None):
 
 # --------------------------------------------------------------------------------------- reference arm
 def run_reference(args, rank, world):
-    """The CPU oracle on host cores, same config / metric / unit; rank 0 only."""
+    """The CPU oracle on host cores, same config / metric / unit; rank 0 alone works and prints, the other ranks only
+    join the (gloo) process group so that the line's n_gpus is the number of ranks that really ran."""
+    dist, joined = join_ranks(args, rank, world, 0, "gloo")
     if rank != 0:
+        dist.barrier()
+        dist.destroy_process_group()
         return
     import torch
     dev = "cuda" if torch.cuda.is_available() else "cpu"          # the grid generator may use the GPU; the timed code never does
-    wl = make_workload(args.config, args.muons, dev, 0, args.joint, args.field_mode, args.poly)
+    wl = make_workload(args.config, args.muons, dev, 0, args.joint, args.field_mode, args.poly, args.draws)
     cores, desc, runner = oracle_sample(wl, args.muons, 0, args.ref_seconds)
     for _ in range(args.warmup):
         runner()
@@ -163,7 +167,7 @@ def run_reference(args, rank, world):
     value = s_tot / t_tot
     line = {
         "impl": "reference", "metric": "muon_steps_per_s", "value": value, "unit": "muon-steps/s",
-        "muons_per_s": m_tot / t_tot, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "muons_per_s": m_tot / t_tot, "n_gpus": joined, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": wl.name, "muons_per_step": m_tot // max(args.steps, 1), "sample": desc},
@@ -172,6 +176,9 @@ def run_reference(args, rank, world):
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
 
 
 # --------------------------------------------------------------------------------------------- our arm
@@ -186,15 +193,15 @@ def run_ours(args, rank, world, local_rank):
     dev = torch.device("cuda", local_rank)
     if rank == 0:
         lib_build.build()
+    _, joined = join_ranks(args, rank, world, local_rank, "nccl")
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
         dist.barrier()
     b.lib()
 
-    from paper_2512_10520_b200.sharding import reduce_job, weak_shard
+    from paper_2512_10520_b200.sharding import gather_ranges, reduce_job, weak_shard
     shard = weak_shard(args.muons, rank, world)               # own batch, own id range, no collective
     n, id_base = shard.n, shard.id_base
-    wl = make_workload(args.config, n, dev, rank, args.joint, args.field_mode, args.poly)
+    wl = make_workload(args.config, n, dev, rank, args.joint, args.field_mode, args.poly, args.draws)
     mode = {0: "regions", 1: "voxel", 2: "poly"}[wl.geom.mode]
     h = b.MuonTransport(local_rank).setup(wl.hist, wl.geom, args.placement)
     h.set_option(b.MT_OPT_SCHEDULE, args.sched).set_option(b.MT_OPT_BLOCK_THREADS, args.block)
@@ -268,6 +275,7 @@ def run_ours(args, rank, world, local_rank):
     # ---- max over ranks, totals over ranks
     (t_dev_max, t_e2e_max, wall_max), (steps_all, muons_all) = reduce_job(
         [t_dev, t_e2e, wall], [steps_per_call, n], dist if world > 1 else None, dev)
+    id_ranges = gather_ranges(shard, dist if world > 1 else None, dev)
     h.close()
     if rank != 0:
         return
@@ -284,12 +292,13 @@ def run_ours(args, rank, world, local_rank):
     line = {
         "metric": "muon_steps_per_s", "value": value, "unit": "muon-steps/s",
         "muons_per_s": muons_all * args.steps / t_dev_max,
-        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_dev_max / args.steps,
+        "n_gpus": joined, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_dev_max / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": wl.name + ("+joint2d" if args.joint else "") + ("+field_mode%d" % args.field_mode if args.field_mode else ""),
                    "muons_per_gpu": n, "muon_steps_per_gpu_step": steps_per_call,
                    "schedule": args.sched, "placement": args.placement, "block": args.block, "slab_cells": args.slab,
                    "parallelism": "id-range sharding x%d, replicated tables and grids, no collective" % world,
+                   "id_ranges": id_ranges,
                    "l2": "inputs larger than L2 (320 MB muon state, 1.9 GB field grid per step)",
                    "flags_rank0": {"stopped": int(flags[0]), "exited": int(flags[1]), "escaped": int(flags[2]),
                                    "maxsteps": int(flags[3])}},
@@ -394,6 +403,45 @@ def run_sweep(args):
             h.close()
 
 
+def self_launch(n_gpus):
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start the N ranks ourselves, one process per
+    GPU, exactly as the driver's own command line would (torch.distributed.run, 127.0.0.1 rendezvous), and pass the
+    ranks' output through.  Rank 0 prints the JSON line."""
+    import socket
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    env = dict(os.environ)
+    # leave the communicator log on (the ranks that joined can be counted from it) but keep stdout to the one JSON line
+    env.setdefault("NCCL_DEBUG", "INFO")
+    env.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+    env["MT_BENCH_SELF_LAUNCHED"] = "1"
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n_gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    log("[bench] --gpus %d without a torchrun environment: launching %s" % (n_gpus, " ".join(cmd)))
+    raise SystemExit(subprocess.call(cmd, env=env))
+
+
+def join_ranks(args, rank, world, local_rank, backend):
+    """Process group of the job; returns (dist or None, ranks that actually joined).  The line's n_gpus is that count,
+    and a count that differs from --gpus is refused rather than printed."""
+    if world == 1:
+        return None, 1
+    import torch
+    import torch.distributed as dist
+    if backend == "nccl":
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        one = torch.ones(1, dtype=torch.int64, device=torch.device("cuda", local_rank))
+    else:
+        dist.init_process_group("gloo")
+        one = torch.ones(1, dtype=torch.int64)
+    dist.all_reduce(one)
+    joined = int(one.item())
+    if joined != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but %d ranks joined the process group" % (args.gpus, joined))
+    return dist, joined
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -416,14 +464,25 @@ def main():
     ap.add_argument("--no-lean", action="store_true", help="MT_OPT_NO_LEAN: general kernels even where the lean variant applies")
     ap.add_argument("--poly", action="store_true", help="with --config 2: the convex-polyhedra shield (DESIGN.md 3.12)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
+    ap.add_argument("--draws", type=int, default=1_000_000, help="draws per generated histogram (BASELINE.json: 10^6)")
     ap.add_argument("--sweep-batches", type=int, default=10)
     ap.add_argument("--sweep-draws", type=int, default=1_000_000, help="draws per generated histogram")
     args = ap.parse_args()
     if args.warmup < 1:
         args.warmup = 1
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be at least 1")
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not args.sweep:
+        self_launch(args.gpus)                                   # does not return
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus and not args.sweep:
+        # one rank per GPU or nothing: a line that says n_gpus = N must come from N ranks
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d (launch with --nproc-per-node %d, or drop the torchrun "
+                         "environment and let bench.py start the ranks)" % (args.gpus, world, args.gpus))
+    # every rank generates its own inputs: share the host cores instead of fighting for them
+    os.environ.setdefault("MT_GEN_WORKERS", str(max(1, (os.cpu_count() or 1) // max(world, 1))))
     if args.sweep:
         if rank == 0:
             run_sweep(args)

@@ -81,7 +81,8 @@ enum {
 /* integer options for mt_set_option */
 enum {
   MT_OPT_SCHEDULE = 1,       /* MT_SCHED_*                                                                 */
-  MT_OPT_BLOCK_THREADS = 2,  /* 0 = library default; else a multiple of 32 in [32, 1024]                   */
+  MT_OPT_BLOCK_THREADS = 2,  /* 0 = library default; else a multiple of 32 in [32, 768] (the largest block  */
+                             /* the transport kernels are compiled for)                                    */
   MT_OPT_BLOCKS_PER_SM = 3,  /* 0 = library default (persistent kernels)                                   */
   MT_OPT_SLAB_CELLS = 4,     /* wavefront: slab thickness along z, in units of 1 cm; 0 = default           */
   MT_OPT_REFILL_MIN_IDLE = 5,/* refill: lanes of a warp that must be idle before it refills; 0 = default   */
@@ -171,7 +172,11 @@ typedef struct {
 } mt_geometry;
 /* VOXEL mode repacks both grids into one library-owned grid of 32-byte records (field and material of a cell, and the
  * field difference to its +x neighbour), so the caller may free d_material / d_field after the call
- * returns.  The library's copy takes 32 bytes per cell of the grid padded by one cell on every side. */
+ * returns.  The library's copy takes 32 bytes per cell of the grid padded by one cell on every side.
+ * On failure: an argument error found before anything is touched leaves the previous geometry in place; a failure
+ * after the library's grid has been overwritten (a material id above n_materials in d_material, a CUDA error) leaves
+ * the context WITHOUT a geometry, and mt_transport then returns MT_ERR_STATE until mt_set_geometry succeeds.
+ * mt_load_histograms invalidates the tables and the geometry; mt_build_alias keeps a geometry that is set. */
 int mt_set_geometry(mt_ctx* ctx, const mt_geometry* geom);
 
 /* Muon state, SoA of 16-byte records (north_star subsystem 3). */
@@ -185,7 +190,8 @@ typedef struct {
   float* mom_steps;        /* [n][4] = final px, py, pz, step count (int32 bits)                           */
   float* exit_rec;         /* optional [exit_capacity][8]: x,y,z,index(uint32 bits),px,py,pz,steps(int32);  */
                            /* x,y,z per mt_geometry.exit_mode                                              */
-  uint32_t* exit_count;    /* optional, one counter; ADDED to (caller zeroes it); may exceed the capacity  */
+  uint32_t* exit_count;    /* optional, one counter; ADDED to (caller zeroes it): one per EXITED muon, so it */
+                           /* may exceed the capacity; may be given WITHOUT exit_rec to count hits only     */
   uint32_t exit_capacity;
   uint64_t* counters;      /* optional [8], ADDED to: [0] total steps, [1..4] muons per flag               */
 } mt_muons_out;
@@ -193,7 +199,10 @@ typedef struct {
 /* Transport n muons (ids id_base .. id_base+n-1) until each meets a break condition.  All buffers DEVICE.
  * Asynchronous: kernels are enqueued on `cuda_stream` (a cudaStream_t; NULL = default stream) and the call
  * returns; outputs are complete when the stream reaches that point.  Outputs are a function of (inputs,
- * seed, id) only — not of launch shape, schedule, batch split or refill order. */
+ * seed, id) only — not of launch shape, schedule, batch split or refill order.  The library's scratch grows to the
+ * largest batch seen: the first call at a larger n than any before it allocates (cudaMalloc, which synchronises the
+ * device) before it enqueues; calls at the same or a smaller n do not.  MT_ERR_STATE unless mt_build_alias and
+ * mt_set_geometry have both succeeded since the last mt_load_histograms. */
 int mt_transport(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
                  const mt_muons_out* out, void* cuda_stream);
 

@@ -125,6 +125,16 @@ def _stream_ptr(stream):
     return C.c_void_p(getattr(stream, "cuda_stream", stream))
 
 
+def _torch_stream(stream):
+    """the torch view of `stream` (None = current stream, a torch stream, or a raw cudaStream_t value)"""
+    import torch
+    if stream is None:
+        return torch.cuda.current_stream()
+    if isinstance(stream, torch.cuda.Stream):
+        return stream
+    return torch.cuda.ExternalStream(int(stream))
+
+
 # ------------------------------------------------------------------------------- the C calls, one to one
 def mt_create(device=0):
     ctx = C.c_void_p()
@@ -213,9 +223,11 @@ def mt_set_geometry(ctx, geom):
     del keep
 
 
-def mt_transport(ctx, pos_q, mom, seed, id_base=0, out=None, exit_capacity=0, counters=True, stream=None):
+def mt_transport(ctx, pos_q, mom, seed, id_base=0, out=None, exit_capacity=0, counters=True, stream=None,
+                 count_exits=False):
     """pos_q, mom: CUDA float32 tensors [n,4].  Returns dict of CUDA tensors (asynchronous on the stream):
-    pos_flag [n,4], mom_steps [n,4], and optionally exit_rec [cap,8], exit_count [1], counters [8]."""
+    pos_flag [n,4], mom_steps [n,4], and optionally exit_rec [cap,8], exit_count [1], counters [8].
+    count_exits=True passes exit_count without a list (exit-plane hits are counted, no records written)."""
     import torch
     assert pos_q.is_cuda and mom.is_cuda and pos_q.dtype == torch.float32 and mom.dtype == torch.float32
     pos_q, mom = pos_q.contiguous(), mom.contiguous()
@@ -224,19 +236,23 @@ def mt_transport(ctx, pos_q, mom, seed, id_base=0, out=None, exit_capacity=0, co
     dev = pos_q.device
     if out is None:
         out = {}
-    if "pos_flag" not in out:
-        out["pos_flag"] = torch.empty((n, 4), dtype=torch.float32, device=dev)
-        out["mom_steps"] = torch.empty((n, 4), dtype=torch.float32, device=dev)
-    if exit_capacity and "exit_rec" not in out:
-        out["exit_rec"] = torch.zeros((exit_capacity, 8), dtype=torch.float32, device=dev)
-    if "exit_rec" in out:
-        out["exit_count"] = torch.zeros(1, dtype=torch.int32, device=dev)
-    if counters:
-        out["counters"] = torch.zeros(8, dtype=torch.int64, device=dev)
+    # the zero-fills below must be ordered before the kernels: they are enqueued on the stream the kernels run on
+    with torch.cuda.stream(_torch_stream(stream)):
+        if "pos_flag" not in out:
+            out["pos_flag"] = torch.empty((n, 4), dtype=torch.float32, device=dev)
+            out["mom_steps"] = torch.empty((n, 4), dtype=torch.float32, device=dev)
+        if exit_capacity and "exit_rec" not in out:
+            out["exit_rec"] = torch.zeros((exit_capacity, 8), dtype=torch.float32, device=dev)
+        if "exit_rec" in out or count_exits:
+            out["exit_count"] = torch.zeros(1, dtype=torch.int32, device=dev)
+        if counters:
+            out["counters"] = torch.zeros(8, dtype=torch.int64, device=dev)
     o = mt_muons_out()
     o.pos_flag, o.mom_steps = out["pos_flag"].data_ptr(), out["mom_steps"].data_ptr()
     if "exit_rec" in out:
         o.exit_rec, o.exit_count, o.exit_capacity = out["exit_rec"].data_ptr(), out["exit_count"].data_ptr(), out["exit_rec"].shape[0]
+    elif count_exits:
+        o.exit_count = out["exit_count"].data_ptr()
     if counters:
         o.counters = out["counters"].data_ptr()
     i = mt_muons_in(pos_q.data_ptr(), mom.data_ptr())

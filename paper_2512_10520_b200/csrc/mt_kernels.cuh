@@ -80,26 +80,26 @@ MT_DEV void write_final(const MtParams& P, const Muon& m, uint32_t idx, int flag
     P.out_pos_flag[idx] = make_float4(m.x, m.y, m.z, __int_as_float(flag));
     P.out_mom_steps[idx] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
   }
-  if (P.exit_rec) {
-    const bool ex = (flag == 2);
-    const unsigned em = __ballot_sync(kFull, ex);
+  if (P.exit_count) {
+    // the counter advances for every exit-plane hit (a caller may pass exit_count alone to count them); records are
+    // written while there is a list and room in it
+    const bool hit = (flag == 2);
+    const unsigned em = __ballot_sync(kFull, hit);
     if (em) {
       const int leader = __ffs(em) - 1;
       unsigned base = 0;
       if ((int)lane == leader) base = atomicAdd(P.exit_count, (unsigned)__popc(em));
       base = __shfl_sync(kFull, base, leader);
-      if (ex) {
-        const unsigned slot = base + (unsigned)__popc(em & ((1u << lane) - 1u));
-        if (slot < P.exit_capacity) {
-          float ex = m.x, ey = m.y, ez = m.z;
-          if (P.exit_mode == 1 && m.pz > 0.0f) {
-            // §3.13: back onto the plane along the final direction (one IEEE division, two fma)
-            const float s = __fdiv_rn(mt::sub(m.z, P.z_exit), m.pz);
-            ex = mt::fma(-s, m.px, m.x); ey = mt::fma(-s, m.py, m.y); ez = P.z_exit;
-          }
-          P.exit_rec[2 * (size_t)slot] = make_float4(ex, ey, ez, __uint_as_float(idx));
-          P.exit_rec[2 * (size_t)slot + 1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
+      const unsigned slot = base + (unsigned)__popc(em & ((1u << lane) - 1u));
+      if (hit && P.exit_rec && slot < P.exit_capacity) {
+        float ex = m.x, ey = m.y, ez = m.z;
+        if (P.exit_mode == 1 && m.pz > 0.0f) {
+          // §3.13: back onto the plane along the final direction (one IEEE division, two fma)
+          const float s = __fdiv_rn(mt::sub(m.z, P.z_exit), m.pz);
+          ex = mt::fma(-s, m.px, m.x); ey = mt::fma(-s, m.py, m.y); ez = P.z_exit;
         }
+        P.exit_rec[2 * (size_t)slot] = make_float4(ex, ey, ez, __uint_as_float(idx));
+        P.exit_rec[2 * (size_t)slot + 1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
       }
     }
   }

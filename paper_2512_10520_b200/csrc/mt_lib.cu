@@ -262,6 +262,8 @@ int build_hash(mt_ctx* c, const mt_geometry* gm, const std::vector<mt_poly_block
   const double w_lo[3] = {gm->x_min, gm->y_min, gm->z_min};
   const double w_ext[3] = {(double)gm->x_max - gm->x_min, (double)gm->y_max - gm->y_min, (double)gm->z_exit - gm->z_min};
   const int hn[3] = {hnx, hny, hnz};
+  if ((uint64_t)hnx * hny * hnz > ((uint64_t)1 << 24))
+    return fail(c, MT_ERR_UNSUPPORTED, "spatial hash of %d x %d x %d cells: at most 2^24 cells", hnx, hny, hnz);
   float inv[3];
   for (int a = 0; a < 3; ++a) inv[a] = (float)((double)hn[a] / w_ext[a]);
   double world = w_ext[0] * w_ext[1] * w_ext[2];
@@ -320,6 +322,11 @@ int build_hash(mt_ctx* c, const mt_geometry* gm, const std::vector<mt_poly_block
   }
   weight[gm->world_material] += std::max(world, 0.0);
   const size_t n_cells = (size_t)hnx * hny * hnz;
+  uint64_t n_list64 = 0;                                     // 2^24 cells x 1024 blocks does not fit 32 bits
+  for (size_t k = 0; k < n_cells; ++k) n_list64 += count[k];
+  if (n_list64 >= ((uint64_t)1 << 28))
+    return fail(c, MT_ERR_UNSUPPORTED, "spatial hash candidate lists hold %llu entries (limit 2^28): use a coarser hash",
+                (unsigned long long)n_list64);
   std::vector<uint32_t> first(n_cells + 1, 0u);
   for (size_t k = 0; k < n_cells; ++k) first[k + 1] = first[k] + count[k];
   const size_t n_list = first[n_cells];
@@ -339,6 +346,19 @@ int build_hash(mt_ctx* c, const mt_geometry* gm, const std::vector<mt_poly_block
   c->h_inv[0] = inv[0]; c->h_inv[1] = inv[1]; c->h_inv[2] = inv[2];
   c->hash_list_off = list_off;
   return MT_OK;
+}
+
+// the header promises that nothing throws across the C boundary: host allocations of the setup calls (std::vector,
+// std::string) are the only throwing code in this file
+template <class F> int guarded(mt_ctx* c, F&& body) {
+  try {
+    return body();
+  } catch (const std::bad_alloc&) {
+    if (c) { try { c->last_error = "host allocation failed"; } catch (...) {} }
+    return MT_ERR_NOMEM;
+  } catch (...) {
+    return MT_ERR_INVALID_ARG;
+  }
 }
 
 }  // namespace
@@ -424,7 +444,7 @@ int mt_set_option(mt_ctx* c, int option, int64_t value) {
   }
 }
 
-int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) {
+static int load_histograms_impl(mt_ctx* c, const mt_hist_desc* d) {
   if (!c || !d) return MT_ERR_INVALID_ARG;
   if (d->hist_mode != MT_HIST_MARGINAL && d->hist_mode != MT_HIST_JOINT) return fail(c, MT_ERR_INVALID_ARG, "bad hist_mode");
   const bool joint = (d->hist_mode == MT_HIST_JOINT);
@@ -466,11 +486,12 @@ int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) {
   c->axis_th.assign(d->axis_th, d->axis_th + nt * 2);
   c->step_m.assign(d->step_m, d->step_m + d->n_materials + 1);
   c->have_hist = true;
-  c->have_tables = false;
+  c->have_tables = false;        // the tables AND the geometry (its material ids, table offsets and shared-memory blob
+  c->have_geom = false;          // follow the histogram shape) must be set again: anything else is MT_ERR_STATE
   return MT_OK;
 }
 
-int mt_build_alias(mt_ctx* c, int placement) {
+static int build_alias_impl(mt_ctx* c, int placement) {
   if (!c) return MT_ERR_INVALID_ARG;
   if (!c->have_hist) return fail(c, MT_ERR_STATE, "mt_build_alias before mt_load_histograms");
   if (placement < MT_PLACE_AUTO || placement > MT_PLACE_L2) return fail(c, MT_ERR_INVALID_ARG, "bad placement");
@@ -511,7 +532,7 @@ int mt_get_alias(const mt_ctx* c, float* prob_dp, uint32_t* alias_dp, float* pro
   return MT_OK;
 }
 
-int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
+static int set_geometry_impl(mt_ctx* c, const mt_geometry* gm) {
   if (!c || !gm) return MT_ERR_INVALID_ARG;
   if (!c->have_tables) return fail(c, MT_ERR_STATE, "mt_set_geometry before mt_build_alias");
   if (gm->mode != MT_GEOM_REGIONS && gm->mode != MT_GEOM_VOXEL && gm->mode != MT_GEOM_POLY)
@@ -562,6 +583,9 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
       return fail(c, MT_ERR_UNSUPPORTED, "voxel grid above 2^20 cells along an axis");
     const size_t n_cells = (size_t)(gm->nx + 2) * (gm->ny + 2) * (gm->nz + 2);       // with the replicated border
     if (n_cells >= ((size_t)1 << 31)) return fail(c, MT_ERR_UNSUPPORTED, "voxel grid above 2^31 cells");
+    // from here on the library's grid is overwritten: a failure below leaves the context WITHOUT a geometry (never with
+    // the previous geometry's parameters over the new grid's data)
+    c->have_geom = false;
     MT_CUDA(c, c->d_grid.reserve(n_cells * sizeof(MtCellPair)));
     MT_CUDA(c, c->d_scratch.reserve(4096));
     MT_CUDA(c, cudaMemset(c->d_scratch.p, 0, 256 * sizeof(unsigned long long)));
@@ -609,6 +633,9 @@ int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) {
   return rebuild_blob(c);
 }
 
+int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) { return guarded(c, [&] { return load_histograms_impl(c, d); }); }
+int mt_build_alias(mt_ctx* c, int placement) { return guarded(c, [&] { return build_alias_impl(c, placement); }); }
+int mt_set_geometry(mt_ctx* c, const mt_geometry* gm) { return guarded(c, [&] { return set_geometry_impl(c, gm); }); }
 int64_t mt_launch_count(const mt_ctx* c) { return c ? c->launches : 0; }
 
 int mt_get_info(const mt_ctx* c, int what, int64_t* value) {
@@ -668,7 +695,8 @@ void fill_params(const mt_ctx* c, MtParams& P) {
 
 int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
                   const mt_muons_out* out, cudaStream_t stream) {
-  if (!c->have_geom) return fail(c, MT_ERR_STATE, "mt_transport before mt_set_geometry");
+  if (!c->have_tables || !c->have_geom)
+    return fail(c, MT_ERR_STATE, "mt_transport needs mt_build_alias and mt_set_geometry after the last mt_load_histograms");
   if (n == 0) return MT_OK;
   if (!in->pos_q || !in->mom || !out->pos_flag || !out->mom_steps) return fail(c, MT_ERR_INVALID_ARG, "null muon buffer");
   if (n >= ((uint64_t)1 << 32)) return fail(c, MT_ERR_UNSUPPORTED, "at most 2^32 - 1 muons per call");
@@ -842,6 +870,9 @@ int mt_transport_host(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_
   if (!c || !in || !out) return MT_ERR_INVALID_ARG;
   if (n == 0) return MT_OK;
   if (!in->pos_q || !in->mom || !out->pos_flag || !out->mom_steps) return fail(c, MT_ERR_INVALID_ARG, "null muon buffer");
+  if (out->exit_rec && !out->exit_count) return fail(c, MT_ERR_INVALID_ARG, "exit_rec without exit_count");
+  if (!c->have_tables || !c->have_geom)
+    return fail(c, MT_ERR_STATE, "mt_transport needs mt_build_alias and mt_set_geometry after the last mt_load_histograms");
   DeviceGuard g(c->device);
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   const size_t rec = n * 4 * sizeof(float);
@@ -861,9 +892,8 @@ int mt_transport_host(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_
   dout.pos_flag = (float*)d_out;
   dout.mom_steps = (float*)(d_out + rec);
   dout.counters = out->counters ? (uint64_t*)d_misc : nullptr;            // 8 x u64 at offset 0
+  if (out->exit_count) dout.exit_count = (uint32_t*)(d_misc + 64);
   if (out->exit_rec) {
-    if (!out->exit_count) return fail(c, MT_ERR_INVALID_ARG, "exit_rec without exit_count");
-    dout.exit_count = (uint32_t*)(d_misc + 64);
     dout.exit_rec = (float*)(d_misc + 128);
     dout.exit_capacity = out->exit_capacity;
   }
@@ -872,10 +902,8 @@ int mt_transport_host(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_
   MT_CUDA(c, cudaMemcpyAsync(out->pos_flag, d_out, rec, cudaMemcpyDeviceToHost, stream));
   MT_CUDA(c, cudaMemcpyAsync(out->mom_steps, d_out + rec, rec, cudaMemcpyDeviceToHost, stream));
   if (out->counters) MT_CUDA(c, cudaMemcpyAsync(out->counters, d_misc, 64, cudaMemcpyDeviceToHost, stream));
-  if (out->exit_rec) {
-    MT_CUDA(c, cudaMemcpyAsync(out->exit_count, d_misc + 64, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
-    MT_CUDA(c, cudaMemcpyAsync(out->exit_rec, d_misc + 128, exit_b, cudaMemcpyDeviceToHost, stream));
-  }
+  if (out->exit_count) MT_CUDA(c, cudaMemcpyAsync(out->exit_count, d_misc + 64, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
+  if (out->exit_rec) MT_CUDA(c, cudaMemcpyAsync(out->exit_rec, d_misc + 128, exit_b, cudaMemcpyDeviceToHost, stream));
   MT_CUDA(c, cudaStreamSynchronize(stream));
   return MT_OK;
 }
@@ -901,7 +929,7 @@ int mt_debug_sample(mt_ctx* c, int material, int pbin, int which, const uint32_t
 int mt_debug_lookup(mt_ctx* c, const float* d_xyz, uint64_t n, int32_t* d_material_out, float* d_field_out,
                     void* cuda_stream) {
   if (!c || !d_xyz || !d_material_out || !d_field_out) return MT_ERR_INVALID_ARG;
-  if (!c->have_geom) return fail(c, MT_ERR_STATE, "mt_debug_lookup before mt_set_geometry");
+  if (!c->have_tables || !c->have_geom) return fail(c, MT_ERR_STATE, "mt_debug_lookup before mt_set_geometry");
   DeviceGuard g(c->device);
   MtParams P;
   fill_params(c, P);

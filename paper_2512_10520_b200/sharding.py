@@ -41,3 +41,14 @@ def reduce_job(times_s, totals, dist=None, device=None):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dist.all_reduce(s, op=dist.ReduceOp.SUM)
     return t.tolist(), s.tolist()
+
+
+def gather_ranges(shard, dist=None, device=None):
+    """[[first id, one past the last id]] of every rank, in rank order, as the ranks themselves report them."""
+    import torch
+    mine = torch.tensor([shard.id_base, shard.id_base + shard.n], dtype=torch.int64, device=device)
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return [mine.tolist()]
+    parts = [torch.zeros_like(mine) for _ in range(dist.get_world_size())]
+    dist.all_gather(parts, mine)
+    return [p.tolist() for p in parts]

@@ -144,7 +144,8 @@ def make_histograms(config, materials, steps_cm, n_pbins, p_lo, p_hi, n_dp, n_th
         rho, x0 = MATERIALS[name]
         for i in range(n_pbins):
             jobs.append((config, m * 4096 + i, rho, x0, step_cm, edges[i], edges[i + 1], n_dp, n_th, n_draws, joint))
-    workers = workers or min(32, os.cpu_count() or 1)
+    # MT_GEN_WORKERS: set by launchers that run several generating processes on one host (bench.py --gpus N)
+    workers = workers or int(os.environ.get("MT_GEN_WORKERS", 0)) or min(32, os.cpu_count() or 1)
     with ThreadPoolExecutor(workers) as ex:
         res = list(ex.map(_one_histogram, jobs))
     counts_dp = np.stack([r[0][0] for r in res]).reshape((M, n_pbins, n_dp, n_th) if joint else (M, n_pbins, n_dp))

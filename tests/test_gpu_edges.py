@@ -201,3 +201,89 @@ def test_error_behaviour(mt, workloads):
         b.mt_destroy(ctx)
     with pytest.raises(b.MtError):
         b.mt_create(9999)
+
+
+def test_reloading_histograms_invalidates_tables_and_geometry(mt, oracle, workloads):
+    """load -> build -> set_geometry -> load(new shape) must not transport against the old tables / blob."""
+    import torch
+    b = mt.binding
+    wl = workloads.config1(n=512, n_draws=30_000)
+    other = workloads.make_histograms(0, ["iron", "concrete"], [2.0, 2.0], 20, 1.0, 300.0, 32, 16, 20_000)
+    dq, dm = torch.from_numpy(wl.muons.pos_q).cuda(), torch.from_numpy(wl.muons.mom).cuda()
+    h = b.MuonTransport(0).setup(wl.hist, wl.geom)
+    try:
+        h.transport(dq, dm, wl.seed)
+        b.mt_load_histograms(h.ctx, other)                       # new shape: 2 materials, 20 bins, 32 + 16 cells
+        for call in (lambda: h.transport(dq, dm, wl.seed),
+                     lambda: h.transport_host(wl.muons.pos_q, wl.muons.mom, wl.seed),
+                     lambda: b.mt_debug_lookup(h.ctx, torch.zeros((4, 3), device="cuda"))):
+            with pytest.raises(b.MtError) as e:
+                call()
+            assert e.value.code == b.MT_ERR_STATE
+        b.mt_build_alias(h.ctx)
+        with pytest.raises(b.MtError) as e:                      # tables rebuilt, geometry still missing
+            h.transport(dq, dm, wl.seed)
+        assert e.value.code == b.MT_ERR_STATE
+        b.mt_set_geometry(h.ctx, wl.geom)
+        wl2 = workloads.Workload("reloaded", other, wl.geom, wl.muons, seed=wl.seed)
+        out = h.transport(dq, dm, wl.seed)
+        torch.cuda.synchronize()
+        g = unpack(out["pos_flag"].cpu().numpy(), out["mom_steps"].cpu().numpy())
+        assert compare(g, oracle_transport(oracle, wl2))["bit_exact"] == 1.0
+        # mt_build_alias again with a geometry in place keeps it (and the results)
+        b.mt_build_alias(h.ctx, b.MT_PLACE_L2)
+        out = h.transport(dq, dm, wl.seed)
+        torch.cuda.synchronize()
+        assert compare(unpack(out["pos_flag"].cpu().numpy(), out["mom_steps"].cpu().numpy()), g)["bit_exact"] == 1.0
+    finally:
+        h.close()
+
+
+def test_failed_voxel_geometry_leaves_no_geometry(mt, workloads):
+    """mt_set_geometry(VOXEL) overwrites the library's grid before it can validate the material ids; on
+    failure the context must not keep transporting with the old parameters over the new data."""
+    import copy
+    import torch
+    b = mt.binding
+    wl = workloads.config3(n=256, n_draws=20_000, n_cells=1, half_width_cells=16, device="cuda")
+    dq, dm = torch.from_numpy(wl.muons.pos_q).cuda(), torch.from_numpy(wl.muons.mom).cuda()
+    h = b.MuonTransport(0).setup(wl.hist, wl.geom)
+    try:
+        h.transport(dq, dm, wl.seed)
+        bad = copy.copy(wl.geom)
+        bad.material = wl.geom.material.clone()
+        bad.material[3, 3, 3] = 9                                # > n_materials = 3
+        with pytest.raises(b.MtError) as e:
+            b.mt_set_geometry(h.ctx, bad)
+        assert e.value.code == b.MT_ERR_INVALID_ARG
+        with pytest.raises(b.MtError) as e:
+            h.transport(dq, dm, wl.seed)
+        assert e.value.code == b.MT_ERR_STATE
+        # an argument error caught before the grid is touched keeps a geometry that is set
+        b.mt_set_geometry(h.ctx, wl.geom)
+        bad2 = copy.copy(wl.geom)
+        bad2.cell = -1.0
+        with pytest.raises(b.MtError):
+            b.mt_set_geometry(h.ctx, bad2)
+        h.transport(dq, dm, wl.seed)
+        torch.cuda.synchronize()
+    finally:
+        h.close()
+
+
+def test_exit_count_without_a_list(mt, wl1, ref1):
+    """include/muon_transport.h: exit_count may be given alone; it counts every EXITED muon."""
+    import torch
+    b = mt.binding
+    h = b.MuonTransport(0).setup(wl1.hist, wl1.geom)
+    try:
+        dq, dm = torch.from_numpy(wl1.muons.pos_q).cuda(), torch.from_numpy(wl1.muons.mom).cuda()
+        for sched in (1, 2, 3):
+            h.set_option(b.MT_OPT_SCHEDULE, sched)
+            side = torch.cuda.Stream()                           # zero-fills and kernels on a non-current stream
+            out = h.transport(dq, dm, wl1.seed, count_exits=True, stream=side)
+            side.synchronize()
+            assert "exit_rec" not in out and int(out["exit_count"].item()) == int((ref1["flag"] == 2).sum())
+            assert int(out["counters"][0].item()) == int(ref1["steps"].sum())
+    finally:
+        h.close()
