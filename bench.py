@@ -30,9 +30,11 @@ if ROOT not in sys.path:
 # DESIGN.md §3 counted one each; loads not counted as operations)
 ALG_OPS_PER_STEP = {"voxel": 383, "regions": 308, "poly": 349}
 ALG_GATHER_BYTES_PER_STEP = {"voxel": 168, "regions": 40, "poly": 50}
-# DRAM bytes (read + written) of ONE launch of the dominant kernel, from the `ncu --set full` capture summarised in
-# profiles/r1i_transport_kernel_full.csv (mean of the three captured z-slab passes of config 3)
-NCU_DRAM_BYTES_PER_LAUNCH = {"voxel": 0.960e9, "regions": None, "poly": None}
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ALL launches of the dominant kernel in one 10^7-muon
+# batch of config 3, summed over the batch's z-slab passes from the ncu launch list profiles/r2_dram_launches.csv
+# (profiles/r2_summary.md has the command); None where no capture exists.  bench.py cannot run ncu itself.
+NCU_DRAM_BYTES_PER_BATCH = {"voxel": None, "regions": None, "poly": None}
+NCU_DRAM_SOURCE = "profiles/r2_dram_launches.csv"
 SM_COUNT, LANES_PER_SM = 148, 128          # B200: 4 SMSPs x 32 lanes issue one warp instruction per clock
 
 
@@ -97,6 +99,57 @@ class ClockSampler:
                     reasons.add(name)
         return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
                     reasons=sorted(reasons), samples=len(sm), power_w_max=max(power) if power else None)
+
+
+# ------------------------------------------------------------------------------------------ roofline
+def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_muons, peaks, mp):
+    """north_star's roofline for one step of this rank: "the larger of FP32-issue time ... at peak and gather bytes at
+    L2/HBM bandwidth", with both terms, against peaks MEASURED in this process (mt_measure_peaks: csrc/mt_probe.cu) and
+    the nominal issue peak beside them.  DESIGN.md §7 derives the per-muon-step figures."""
+    ops = steps_per_call * ALG_OPS_PER_STEP[mode]                          # thread-operations per step
+    gbytes = steps_per_call * ALG_GATHER_BYTES_PER_STEP[mode]              # gathered bytes per step
+    nominal = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6           # thread-ops/s: one per lane per clock
+    measured = mp["ffma_thread_ops_per_s"]                                 # a pure FFMA stream on this device, now
+    per_lane = launches_per_step // max(lanes, 1)
+    passes = lanes * ((per_lane - 3) // 3 + 1 if per_lane > 3 else per_lane)      # launches of the transport kernel
+    t_issue, t_issue_nominal = ops / measured, ops / nominal
+    t_gather = {"l1_resident_64k": gbytes / mp["gather_l1_bytes_per_s"], "l2_resident_64m": gbytes / mp["gather_64m_bytes_per_s"],
+                "hbm_1400m": gbytes / mp["gather_1400m_bytes_per_s"]}
+    state_bytes = 64 * n_muons                                             # 32 B in + 32 B out per muon: the only compulsory HBM traffic
+    dram = NCU_DRAM_BYTES_PER_BATCH[mode]
+    return {
+        "bound": "alu", "unit": "T thread-ops/s",
+        "achieved": ops / t_call_s / 1e12, "peak": measured / 1e12, "frac": t_issue / t_call_s,
+        "peak_nominal": nominal / 1e12, "frac_nominal": t_issue_nominal / t_call_s,
+        "peak_source": "measured in this process: mt_measure_peaks, fma.rn.f32 stream, 8 warps per scheduler "
+                       "(nominal = 148 SM x 128 lanes x %s sm_max_mhz %.0f)" % (peaks["source"], peaks["sm_max_mhz"]),
+        "kernel": ("wave_transport_kernel: %d z-slab passes (%d lane(s)) among the %d launches of a step (the rest sort "
+                   "the live list)" % (passes, lanes, launches_per_step)) if per_lane > 1 else
+                  "transport_kernel (%d launch(es) per step)" % launches_per_step,
+        "ops_per_muon_step": ALG_OPS_PER_STEP[mode], "gather_bytes_per_muon_step": ALG_GATHER_BYTES_PER_STEP[mode],
+        "terms_ms": {
+            "measured": 1e3 * t_call_s,
+            "t_issue_at_measured_ffma_peak": 1e3 * t_issue, "t_issue_at_nominal_peak": 1e3 * t_issue_nominal,
+            "t_gather_if_every_record_came_from": {k: 1e3 * v for k, v in t_gather.items()},
+            "reading": "the issue term binds.  The gather terms price every lane's record as a separate 32-byte sector "
+                       "at the random-sector rate of that level; a term above the measured time means the schedule does "
+                       "not pay it: the sorted wavefront makes a warp's lanes share sectors in L1 (ncu: L1 hit 57-77 %, "
+                       "L2 hit 88-91 %, DRAM 2-3 % busy)"},
+        "gather_tb_per_s": gbytes / t_call_s / 1e12,
+        "measured_peaks": {"ffma_T_thread_ops_per_s": measured / 1e12, "lop3_T": mp["lop3_thread_ops_per_s"] / 1e12,
+                           "imad_T": mp["imad_thread_ops_per_s"] / 1e12, "mulhi_T": mp["mulhi_thread_ops_per_s"] / 1e12,
+                           "mufu_T": mp["mufu_thread_ops_per_s"] / 1e12,
+                           "gather_TB_per_s": {"l1_resident_64k": mp["gather_l1_bytes_per_s"] / 1e12,
+                                               "l2_resident_675k": mp["gather_675k_bytes_per_s"] / 1e12,
+                                               "l2_resident_64m": mp["gather_64m_bytes_per_s"] / 1e12,
+                                               "hbm_1400m": mp["gather_1400m_bytes_per_s"] / 1e12},
+                           "hbm_copy_gbs_%s" % peaks["source"]: peaks["hbm_gbs"]},
+        "traffic": (dram / passes) if dram else None,
+        "traffic_unit": "DRAM bytes per launch of the kernel = per-batch total / passes (ncu, %s)" % NCU_DRAM_SOURCE,
+        "traffic_per_batch": dram,
+        "algorithmic_hbm_bytes_per_batch": state_bytes,
+        "traffic_over_algorithmic": (dram / state_bytes) if dram else None,
+    }
 
 
 # ------------------------------------------------------------------------------------------ workload
@@ -207,6 +260,7 @@ def run_ours(args, rank, world, local_rank):
     h.set_option(b.MT_OPT_SCHEDULE, args.sched).set_option(b.MT_OPT_BLOCK_THREADS, args.block)
     h.set_option(b.MT_OPT_SLAB_CELLS, args.slab).set_option(b.MT_OPT_REFILL_MIN_IDLE, args.min_idle)
     h.set_option(b.MT_OPT_BLOCKS_PER_SM, args.blocks_per_sm).set_option(b.MT_OPT_NO_LEAN, int(args.no_lean))
+    h.set_option(b.MT_OPT_LANES, args.lanes)
     host_geom = None
     if rank == 0 and not args.no_cpu_baseline:
         import copy
@@ -251,6 +305,7 @@ def run_ours(args, rank, world, local_rank):
         wall = time.perf_counter() - wall0
         clocks = sampler.stop() if sampler else None
         launches = b.mt_launch_count(h.ctx) - launches0
+        lanes_used = b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES)
     dev_ms = [e0.elapsed_time(e1) for e0, e1 in evs]
     t_dev = sum(dev_ms) * 1e-3
     flags = np.bincount(out["pos_flag"][:, 3].view(torch.int32).cpu().numpy(), minlength=5)[1:5]
@@ -283,12 +338,8 @@ def run_ours(args, rank, world, local_rank):
     peaks = load_peaks()
     value = steps_all * args.steps / t_dev_max
     e2e_value = steps_all * e2e_steps / t_e2e_max
-    # roofline of the dominant kernel (transport_kernel), this rank: algorithmic thread-operations per launch /
-    # CUDA-event duration per launch, against the FP32 issue peak 148 SMs x 128 lanes x max SM clock
-    launches_per_step = max(1, launches // args.steps)
-    alu_peak = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12                  # T thread-ops/s
-    achieved = steps_per_call * ALG_OPS_PER_STEP[mode] * args.steps / t_dev / 1e12
-    gather_tbs = steps_per_call * ALG_GATHER_BYTES_PER_STEP[mode] * args.steps / t_dev / 1e12
+    roofline = roofline_block(mode, steps_per_call, t_dev / args.steps, max(1, launches // args.steps), lanes_used, n,
+                              peaks, b.mt_measure_peaks(local_rank))
     line = {
         "metric": "muon_steps_per_s", "value": value, "unit": "muon-steps/s",
         "muons_per_s": muons_all * args.steps / t_dev_max,
@@ -297,6 +348,7 @@ def run_ours(args, rank, world, local_rank):
         "config": {"workload": wl.name + ("+joint2d" if args.joint else "") + ("+field_mode%d" % args.field_mode if args.field_mode else ""),
                    "muons_per_gpu": n, "muon_steps_per_gpu_step": steps_per_call,
                    "schedule": args.sched, "placement": args.placement, "block": args.block, "slab_cells": args.slab,
+                   "lanes": lanes_used,
                    "parallelism": "id-range sharding x%d, replicated tables and grids, no collective" % world,
                    "id_ranges": id_ranges,
                    "l2": "inputs larger than L2 (320 MB muon state, 1.9 GB field grid per step)",
@@ -306,16 +358,7 @@ def run_ours(args, rank, world, local_rank):
                 "steps": e2e_steps, "ms_per_step": 1e3 * t_e2e_max / e2e_steps},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "T thread-ops/s",
-                     "frac": achieved / alu_peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH[mode],
-                     "traffic_unit": "DRAM bytes per launch of the kernel (ncu, profiles/r1i_transport_kernel_full.csv)",
-                     "kernel": ("wave_transport_kernel: %d z-slab passes among the %d launches of a step (the rest sort the "
-                                "live list)" % ((launches_per_step - 1) // 3, launches_per_step)) if launches_per_step > 1
-                     else "transport_kernel (1 launch per step)",
-                     "ops_per_muon_step": ALG_OPS_PER_STEP[mode], "peak_source": "148 SM x 128 lanes x %s sm_max_mhz"
-                     % peaks["source"], "gather_tb_per_s": gather_tbs,
-                     "gather_bytes_per_muon_step": ALG_GATHER_BYTES_PER_STEP[mode],
-                     "hbm_gbs_%s" % peaks["source"]: peaks["hbm_gbs"]},
+        "roofline": roofline,
         "wall_ms_per_step": 1e3 * wall_max / args.steps,
         "dev_ms_steps": [round(x, 3) for x in dev_ms],
     }
@@ -357,7 +400,7 @@ def run_sweep(args):
         return e0.elapsed_time(e1) * 1e-3, int(r["counters"][0].item())
 
     def emit(**kw):
-        kw["roofline_frac"] = kw["muon_steps_per_s"] * ALG_OPS_PER_STEP["voxel"] / alu_peak
+        kw["roofline_frac_nominal"] = kw["muon_steps_per_s"] * ALG_OPS_PER_STEP["voxel"] / alu_peak
         print(json.dumps(kw), flush=True)
 
     batches = [w.spectrum_muons(3, n_batch, "square", batch=k) for k in range(n_batches)]
@@ -456,6 +499,7 @@ def main():
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--slab", type=int, default=0)
     ap.add_argument("--min-idle", type=int, default=0)
+    ap.add_argument("--lanes", type=int, default=0, help="MT_OPT_LANES: concurrent lanes per call (0 = library default)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-seconds", type=float, default=15.0, help="CPU work per oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -91,8 +91,12 @@ enum {
   MT_OPT_HASH_NXY = 7,       /* POLY: cells of the spatial hash along x and along y; 0 = default (16); 1..256 */
   MT_OPT_HASH_NZ = 8,        /* POLY: cells of the spatial hash along z; 0 = default (256); 1..4096.  Both    */
                              /* take effect at the next mt_set_geometry; results never depend on them         */
-  MT_OPT_NO_LEAN = 9         /* 1: never take the kernel variants that drop operations the host has proven to  */
+  MT_OPT_NO_LEAN = 9,        /* 1: never take the kernel variants that drop operations the host has proven to  */
                              /* be identities for the loaded tables and geometry; for testing    */
+  MT_OPT_LANES = 10,         /* concurrent lanes a call is split into (contiguous id ranges on library-owned    */
+                             /* streams, joined on the caller's stream); 0 = default (by n), 1..16             */
+  MT_OPT_CHECK_SELFTEST = 11 /* checked build only (MT_INFO_CHECK_ERRORS): 1 hands the kernels a wrong table size */
+                             /* so that the bounds checks must fire; MT_ERR_UNSUPPORTED in the normal build     */
 };
 
 const char* mt_strerror(int code);
@@ -218,9 +222,31 @@ int64_t mt_launch_count(const mt_ctx* ctx);
 enum {
   MT_INFO_LEAN_FACTS = 1,  /* bit 0: table axes proven inside the clamps; bit 1: world box proven inside the voxel grid   */
   MT_INFO_LAST_LEAN = 2,   /* 1 if the last mt_transport call ran the lean kernel variant                                */
-  MT_INFO_LAST_SCHEDULE = 3/* MT_SCHED_* the last mt_transport call ran under                                            */
+  MT_INFO_LAST_SCHEDULE = 3,/* MT_SCHED_* the last mt_transport call ran under                                           */
+  MT_INFO_LAST_LANES = 4,  /* number of concurrent lanes the last mt_transport call was split into                        */
+  MT_INFO_CHECK_ERRORS = 5 /* -1 in the normal build.  Checked build (libmuon_transport_checked.so, compiled with           */
+                           /* -DMT_CHECKED: every index into a global array is bounds-checked in the kernels instead of       */
+                           /* dereferenced): low 32 bits = violations so far, high 32 bits = highest violation code;         */
+                           /* synchronises the device                                                                       */
 };
 int mt_get_info(const mt_ctx* ctx, int what, int64_t* value);
+
+/* Measured peaks of device `cuda_device`, for the roofline the transport kernels are reported against (SURVEY.md §8(d):
+ * "measure the FFMA peak in the same process ... L2 bandwidth with a random-sector gather").  Runs a few short probe
+ * kernels (about 50 ms in all, 1.4 GB of temporary device memory) and synchronises.  Not on the transport path.
+ *   *_thread_ops_per_s   lanes x warp instructions per second over the whole GPU for an instruction stream of that one
+ *                        kind with no dependency stalls (8 warps per scheduler, 8 independent chains per thread):
+ *                        fma.rn.f32 / lop3.b32 / mad.lo.u32 / mul.hi.u32 / rsqrt.approx.f32 (the conversion unit)
+ *   gather_*_bytes_per_s 32-byte sectors per second x 32 for one random sector per lane out of a working set of
+ *                        64 KB (L1-resident), 675 KB and 64 MB (L2-resident), 1400 MB (HBM)                              */
+typedef struct {
+  int32_t sm_count;
+  double sm_clock_mhz_nominal;
+  double ffma_thread_ops_per_s, ffma_warp_instr_per_s_per_smsp;
+  double lop3_thread_ops_per_s, imad_thread_ops_per_s, mulhi_thread_ops_per_s, mufu_thread_ops_per_s;
+  double gather_l1_bytes_per_s, gather_675k_bytes_per_s, gather_64m_bytes_per_s, gather_1400m_bytes_per_s;
+} mt_peaks;
+int mt_measure_peaks(int cuda_device, mt_peaks* out);
 
 /* Test hooks (DEVICE buffers, asynchronous on the stream).
  * mt_debug_sample: cell_out[i] = alias draw from table `which` (0 = Dp/p, 1 = theta) of

@@ -5,6 +5,8 @@ this package.  It never imports paper_2512_10520_b200 (the CUDA path), and the C
 it.  All arithmetic lives in muon_oracle.cpp; this file only marshals numpy arrays.
 """
 import ctypes as C
+import os
+
 import numpy as np
 
 from .build import build as _build
@@ -45,7 +47,8 @@ class _Tables(C.Structure):
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(_build())
+        # MUON_ORACLE_LIB: an alternative build of the same source (oracle/build.py --sanitize) for the sanitizer run
+        _lib = C.CDLL(os.environ.get("MUON_ORACLE_LIB") or _build())
         _lib.orc_kick_f64.restype = C.c_double
         _lib.orc_kick_f32.restype = C.c_float
         _lib.orc_kick_f64.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_uint32]

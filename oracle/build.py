@@ -15,14 +15,26 @@ FLAGS = ["-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off
          "-march=x86-64-v3", "-Wall", "-Wextra"]
 
 
-def build(force: bool = False) -> str:
-    if (not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
-        return LIB
-    tmp = LIB + ".tmp.%d" % os.getpid()
-    subprocess.check_call(["g++", *FLAGS, SRC, "-o", tmp])
-    os.replace(tmp, LIB)
-    return LIB
+SANITIZED_LIB = os.path.join(HERE, "libmuon_oracle_asan.so")
+SANITIZE_FLAGS = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+
+
+def build(force: bool = False, sanitize: bool = False) -> str:
+    """sanitize=True: the same source with AddressSanitizer and UndefinedBehaviorSanitizer as
+    libmuon_oracle_asan.so; run the CPU tests against it with
+        LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+        MUON_ORACLE_LIB=oracle/libmuon_oracle_asan.so python -m pytest tests -q -m "not gpu"
+    (profiles/r2_sanitizers.md has the record)."""
+    lib = SANITIZED_LIB if sanitize else LIB
+    if (not force and os.path.exists(lib) and os.path.getmtime(lib) >= os.path.getmtime(SRC)):
+        return lib
+    tmp = lib + ".tmp.%d" % os.getpid()
+    flags = [f for f in FLAGS if f != "-O2"] + SANITIZE_FLAGS if sanitize else FLAGS
+    subprocess.check_call(["g++", *flags, SRC, "-o", tmp])
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force=True))
+    import sys
+    print(build(force=True, sanitize="--sanitize" in sys.argv))

@@ -8,7 +8,8 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libmuon_transport.so")
+# MUON_TRANSPORT_LIB: an alternative build of the same sources (build.py --checked: bounds-checked kernels) for tests
+LIB_PATH = os.environ.get("MUON_TRANSPORT_LIB") or os.path.join(HERE, "libmuon_transport.so")
 
 MT_OK = 0
 MT_ERR_INVALID_ARG, MT_ERR_STATE, MT_ERR_EMPTY_HIST, MT_ERR_UNSUPPORTED, MT_ERR_CUDA, MT_ERR_NOMEM = -1, -2, -3, -4, -5, -6
@@ -17,16 +18,16 @@ MT_GEOM_REGIONS, MT_GEOM_VOXEL, MT_GEOM_POLY = 0, 1, 2
 MT_PLACE_AUTO, MT_PLACE_SMEM, MT_PLACE_L2 = 0, 1, 2
 MT_SCHED_AUTO, MT_SCHED_STATIC, MT_SCHED_REFILL, MT_SCHED_WAVEFRONT = 0, 1, 2, 3
 MT_OPT_SCHEDULE, MT_OPT_BLOCK_THREADS, MT_OPT_BLOCKS_PER_SM, MT_OPT_SLAB_CELLS, MT_OPT_REFILL_MIN_IDLE = 1, 2, 3, 4, 5
-MT_OPT_KEY_LOOKAHEAD, MT_OPT_HASH_NXY, MT_OPT_HASH_NZ, MT_OPT_NO_LEAN = 6, 7, 8, 9
+MT_OPT_KEY_LOOKAHEAD, MT_OPT_HASH_NXY, MT_OPT_HASH_NZ, MT_OPT_NO_LEAN, MT_OPT_LANES, MT_OPT_CHECK_SELFTEST = 6, 7, 8, 9, 10, 11
 MT_HIST_MARGINAL, MT_HIST_JOINT = 0, 1
 MT_EXIT_AT_BREAK, MT_EXIT_PROJECT = 0, 1
-MT_INFO_LEAN_FACTS, MT_INFO_LAST_LEAN, MT_INFO_LAST_SCHEDULE = 1, 2, 3
+MT_INFO_LEAN_FACTS, MT_INFO_LAST_LEAN, MT_INFO_LAST_SCHEDULE, MT_INFO_LAST_LANES, MT_INFO_CHECK_ERRORS = 1, 2, 3, 4, 5
 MT_FIELD_TRILINEAR, MT_FIELD_NEAREST, MT_FIELD_PER_STAGE = 0, 1, 2
 
 # every symbol include/muon_transport.h declares (tests check that the library exports each one)
 SYMBOLS = ["mt_strerror", "mt_last_error", "mt_create", "mt_destroy", "mt_set_option", "mt_load_histograms",
            "mt_build_alias", "mt_get_alias", "mt_set_geometry", "mt_transport", "mt_transport_host",
-           "mt_launch_count", "mt_get_info", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
+           "mt_launch_count", "mt_get_info", "mt_measure_peaks", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
 
 
 class mt_hist_desc(C.Structure):
@@ -57,6 +58,15 @@ class mt_geometry(C.Structure):
                 ("ox", C.c_float), ("oy", C.c_float), ("oz", C.c_float), ("cell", C.c_float),
                 ("d_material", C.c_void_p), ("d_field", C.c_void_p), ("field_mode", C.c_int32),
                 ("n_blocks", C.c_int32), ("blocks", C.c_void_p), ("exit_mode", C.c_int32)]
+
+
+class mt_peaks(C.Structure):
+    _fields_ = [("sm_count", C.c_int32), ("sm_clock_mhz_nominal", C.c_double),
+                ("ffma_thread_ops_per_s", C.c_double), ("ffma_warp_instr_per_s_per_smsp", C.c_double),
+                ("lop3_thread_ops_per_s", C.c_double), ("imad_thread_ops_per_s", C.c_double),
+                ("mulhi_thread_ops_per_s", C.c_double), ("mufu_thread_ops_per_s", C.c_double),
+                ("gather_l1_bytes_per_s", C.c_double), ("gather_675k_bytes_per_s", C.c_double),
+                ("gather_64m_bytes_per_s", C.c_double), ("gather_1400m_bytes_per_s", C.c_double)]
 
 
 class mt_muons_in(C.Structure):
@@ -96,6 +106,7 @@ def lib():
         L.mt_launch_count.restype = C.c_int64
         L.mt_launch_count.argtypes = [C.c_void_p]
         L.mt_get_info.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]
+        L.mt_measure_peaks.argtypes = [C.c_int, C.POINTER(mt_peaks)]
         L.mt_debug_sample.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_philox.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -301,6 +312,15 @@ def mt_get_info(ctx, what):
     if rc != MT_OK:
         raise MtError(rc, "mt_get_info")
     return int(v.value)
+
+
+def mt_measure_peaks(device=0):
+    """dict of the measured issue and gather peaks of the device (include/muon_transport.h: mt_peaks)"""
+    p = mt_peaks()
+    rc = lib().mt_measure_peaks(int(device), C.byref(p))
+    if rc != MT_OK:
+        raise MtError(rc, "mt_measure_peaks(device=%d)" % device)
+    return {name: getattr(p, name) for name, _ in mt_peaks._fields_}
 
 
 def mt_debug_sample(ctx, material, pbin, which, words, stream=None, joint=False):

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmuon_transport.so")
 SOURCES = ["mt_lib.cu", "mt_kernels.cu", "mt_inst_regions.cu", "mt_inst_poly.cu", "mt_inst_voxel_a.cu",
-           "mt_inst_voxel_b.cu", "mt_inst_lean.cu"]
+           "mt_inst_voxel_b.cu", "mt_inst_lean.cu", "mt_probe.cu"]
 DEPS = SOURCES + ["mt_kernels.cuh", "mt_step.cuh", "mt_params.h", "mt_launch.h"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
@@ -29,15 +29,22 @@ def _nvcc():
     return "nvcc"
 
 
-def build(force: bool = False, verbose: bool = False, defines=()) -> str:
+CHECKED_LIB = os.path.join(HERE, "libmuon_transport_checked.so")
+
+
+def build(force: bool = False, verbose: bool = False, defines=(), checked: bool = False) -> str:
     """Compile the translation units in parallel (the kernel instantiations are split over several so that this takes
-    well under a minute), then link.  `defines`: extra -D macros (e.g. MT_MAX_THREADS=1024) for tuning experiments."""
+    well under a minute), then link.  `defines`: extra -D macros (e.g. MT_MAX_THREADS=1024) for tuning experiments.
+    checked=True builds libmuon_transport_checked.so with -DMT_CHECKED: the same kernels with every global-array index
+    bounds-checked (csrc/mt_params.h: MT_CHECK); load it through MUON_TRANSPORT_LIB (tests/test_gpu_checked.py)."""
+    LIB = CHECKED_LIB if checked else globals()["LIB"]
+    defines = tuple(defines) + (("MT_CHECKED",) if checked else ())
     deps = [os.path.join(CSRC, d) for d in DEPS] + [os.path.join(INCLUDE, "muon_transport.h"), __file__]
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     bdir = os.path.join(HERE, "build")
     os.makedirs(bdir, exist_ok=True)
-    tag = ".%d" % os.getpid()
+    tag = ".%d%s" % (os.getpid(), ".chk" if checked else "")
     base = [_nvcc(), *NVCC_FLAGS, *["-D" + d for d in defines], "-I", INCLUDE]
 
     def compile_one(src):
@@ -69,7 +76,7 @@ def build(force: bool = False, verbose: bool = False, defines=()) -> str:
         for obj in objs:
             if os.path.exists(obj):
                 os.remove(obj)
-        with open(os.path.join(bdir, "ptxas.log"), "w") as f:
+        with open(os.path.join(bdir, "ptxas_checked.log" if checked else "ptxas.log"), "w") as f:
             f.write("\n".join(log))
     if verbose:
         print("\n".join(log))
@@ -78,4 +85,4 @@ def build(force: bool = False, verbose: bool = False, defines=()) -> str:
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv or any(a.startswith("-D") for a in sys.argv), verbose="--quiet" not in sys.argv,
-                defines=[a[2:] for a in sys.argv if a.startswith("-D")]))
+                defines=[a[2:] for a in sys.argv if a.startswith("-D")], checked="--checked" in sys.argv))

@@ -14,6 +14,7 @@ __global__ void __launch_bounds__(256) wave_bin_kernel(const __grid_constant__ M
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += stride) {
     const float4 a = __ldg(P.in_pos_q + i), b = __ldg(P.in_mom + i);
     const uint32_t key = sort_key(P, a.x, a.y, b.x, b.y, b.z);
+    MT_CHECK(P, key < P.n_keys, MT_CHK_SORT_KEY);
     const uint32_t rank = atomicAdd(P.hist + key, 1u);
     P.sort_key[i] = make_uint2(key, rank);
   }
@@ -74,6 +75,8 @@ __global__ void __launch_bounds__(256) wave_perm_kernel(const __grid_constant__ 
   const uint32_t stride = gridDim.x * blockDim.x;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
     const uint2 k = P.sort_key[i];
+    MT_CHECK(P, k.x < P.n_keys, MT_CHK_SORT_KEY);
+    MT_CHECK(P, P.key_offset[k.x] + k.y < n, MT_CHK_PERM_SLOT);
     P.perm[P.key_offset[k.x] + k.y] = i;
   }
 }
@@ -115,6 +118,7 @@ __global__ void debug_sample_kernel(const typename Tab<PACK>::cell_t* tab, uint3
   if (i >= n) return;
   MtParams P;                       // only hot_cells is read: nothing staged here
   P.hot_cells = 0u;
+  P.check = nullptr; P.n_tab_cells = 0xFFFFFFFFu;      // checked build: the caller passes a table of N cells, k < N
   View<PACK> V;
   V.tab = tab;
   V.hot = tab;

@@ -39,6 +39,7 @@ MT_DEV View<PACK> stage_view(const MtParams& P) {
   V.zlo = sblob + P.bl.off_zlo;
   V.regions = reinterpret_cast<const MtRegionDev*>(sblob + P.bl.off_regions);
   V.blocks = reinterpret_cast<const MtBlockDev*>(sblob + P.bl.off_blocks);
+  V.binlut = reinterpret_cast<const uint16_t*>(sblob + P.bl.off_binlut);
   const uint32_t* gtab = (PACK == 32) ? P.tab32 : reinterpret_cast<const uint32_t*>(P.tab64);
   V.tab = reinterpret_cast<const typename Tab<PACK>::cell_t*>(gtab);
   uint4* stab = reinterpret_cast<uint4*>(sblob + ((P.bl.n_words + 3) & ~3));
@@ -77,6 +78,7 @@ struct Tally {
 // atomic per warp (north_star subsystem 6).  Called by all 32 lanes; `flag` is 0 on lanes with nothing to write.
 MT_DEV void write_final(const MtParams& P, const Muon& m, uint32_t idx, int flag, unsigned lane) {
   if (flag) {
+    MT_CHECK(P, idx < P.n, MT_CHK_OUTPUT);
     P.out_pos_flag[idx] = make_float4(m.x, m.y, m.z, __int_as_float(flag));
     P.out_mom_steps[idx] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
   }
@@ -98,7 +100,7 @@ MT_DEV void write_final(const MtParams& P, const Muon& m, uint32_t idx, int flag
           const float s = __fdiv_rn(mt::sub(m.z, P.z_exit), m.pz);
           ex = mt::fma(-s, m.px, m.x); ey = mt::fma(-s, m.py, m.y); ez = P.z_exit;
         }
-        P.exit_rec[2 * (size_t)slot] = make_float4(ex, ey, ez, __uint_as_float(idx));
+        P.exit_rec[2 * (size_t)slot] = make_float4(ex, ey, ez, __uint_as_float(idx + P.idx_base));
         P.exit_rec[2 * (size_t)slot + 1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
       }
     }
@@ -126,6 +128,7 @@ transport_kernel(const __grid_constant__ MtParams P) {
 
   auto load = [&](uint64_t item) {
     idx = (uint32_t)item;
+    MT_CHECK(P, item < P.n, MT_CHK_INPUT);
     const float4 a = __ldg(P.in_pos_q + idx), b = __ldg(P.in_mom + idx);
     m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z; m.step = 0;
     active = true;
@@ -216,7 +219,9 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
     m.x = m.y = m.z = m.q = m.px = m.py = m.pz = 0.0f;
     m.step = 0;
     if (item < n_items) {
+      MT_CHECK(P, item < P.n, MT_CHK_PERM);
       const uint32_t rec = P.perm[item];
+      MT_CHECK(P, rec < (P.first_pass ? P.n : (uint64_t)n_items), MT_CHK_RECORD);
       float4 a, b;
       if (P.first_pass) {
         a = __ldg(P.in_pos_q + rec); b = __ldg(P.in_mom + rec);
@@ -226,6 +231,7 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
         const float4* r = P.rec_in + 3 * (size_t)rec;
         a = __ldg(r); b = __ldg(r + 1);
         idx = __ldg(reinterpret_cast<const uint32_t*>(r + 2));
+        MT_CHECK(P, idx < P.n, MT_CHK_RECORD);
       }
       m.x = a.x; m.y = a.y; m.z = a.z; m.q = a.w; m.px = b.x; m.py = b.y; m.pz = b.z;
       m.step = __float_as_int(b.w);
@@ -261,6 +267,8 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
         if ((int)lane == pl) r0 = atomicAdd(P.hist + key, (unsigned)__popc(peers));
         r0 = __shfl_sync(peers, r0, pl);
         const unsigned slot = slot0 + (unsigned)__popc(pm & lt_mask);
+        MT_CHECK(P, slot < P.n, MT_CHK_PARK_SLOT);
+        MT_CHECK(P, key < P.n_keys, MT_CHK_SORT_KEY);
         float4* r = P.rec_out + 3 * (size_t)slot;                       // a warp's records are contiguous: full sectors
         r[0] = make_float4(m.x, m.y, m.z, m.q);
         r[1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));

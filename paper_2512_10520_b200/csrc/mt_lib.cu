@@ -31,6 +31,14 @@ struct DevBuf {
   void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
 };
 
+// a lane of concurrent transport work inside one call (run_transport): own stream, own scratch
+struct Lane {
+  cudaStream_t stream = nullptr;
+  cudaEvent_t done = nullptr, ready = nullptr;   // its kernels (and copies out) are done / its inputs have landed
+  DevBuf scratch, wave;
+  size_t zero_bytes = 0;
+};
+
 }  // namespace
 
 struct mt_ctx {
@@ -54,7 +62,7 @@ struct mt_ctx {
   size_t table_bytes = 0;
   std::vector<int> mat_order;        // material ids, most-used first: the order of their blocks in the packed tables
   std::vector<uint32_t> mat_cell0;   // [n_materials + 1] first cell of material m's block in the packed tables
-  DevBuf d_tab, d_blob, d_grid, d_scratch, d_wave, d_stage_in, d_stage_out, d_stage_misc, d_hash;
+  DevBuf d_tab, d_blob, d_grid, d_scratch, d_check, d_stage_in, d_stage_out, d_stage_misc, d_hash;
   int opt_hash_nxy = 0, opt_hash_nz = 0, opt_no_lean = 0;
   float lean_box[6] = {0, 0, 0, 0, 0, 0};        // x_lo, x_hi, y_lo, y_hi, z_lo, z_hi of MT_LEAN_INSIDE
   bool lean_axes = false, lean_inside = false;   // MT_LEAN_* facts (mt_params.h), proven in rebuild_blob / mt_set_geometry
@@ -65,9 +73,16 @@ struct mt_ctx {
   int hnx = 0, hny = 0, hnz = 0;         // spatial hash
   float h_inv[3] = {0, 0, 0};
   size_t hash_list_off = 0;              // byte offset of the candidate lists inside d_hash
+  uint32_t n_hash_list = 0;              // entries of the candidate lists
+  int bin_shift = 0, bin_key_lo = 0, bin_key_max = 0;   // momentum-bin table (mt_params.h)
+  int selftest_bad_bounds = 0;           // checked build: hand the kernels a wrong table size (MT_OPT_CHECK_SELFTEST)
   MtBlobLayout bl{};
   int64_t launches = 0;
-  int last_lean = 0, last_sched = 0;
+  int last_lean = 0, last_sched = 0, last_lanes = 0;
+  int opt_lanes = 0;
+  std::vector<Lane> lanes;
+  cudaEvent_t ev_fork = nullptr;
+  cudaStream_t copy_in = nullptr;
 };
 
 namespace {
@@ -149,11 +164,39 @@ int rebuild_blob(mt_ctx* c) {
   bl.off_regions = (bl.off_zlo + n_reg + 3) & ~3;
   const int n_blk = c->have_geom ? (int)c->blocks.size() : 0;
   bl.off_blocks = (bl.off_regions + 10 * n_reg + 3) & ~3;
-  bl.n_words = bl.off_blocks + 24 * n_blk;
-  std::vector<float> blob((size_t)bl.n_words + 4, 0.0f);
+  bl.off_binlut = bl.off_blocks + 24 * n_blk;
   const double lo = (double)c->p_lo, hi = (double)c->p_hi;
+  std::vector<float> edges(n_edges);
   for (int j = 0; j <= c->n_pbins; ++j)
-    blob[j] = (float)(lo * pow(hi / lo, (double)j / (double)c->n_pbins));                 // §3.4
+    edges[j] = (float)(lo * pow(hi / lo, (double)j / (double)c->n_pbins));                // §3.4
+  // Momentum-bin table (mt_params.h: bin_shift).  A key names the 2^shift consecutive floats that share their top bits;
+  // the coarsest keys under which no run of floats holds more than one edge are taken, so that one comparison with the
+  // edge above the tabulated bin settles §3.4's decision.  Runs are looked at over [p_lo, p_hi] (keys are clamped there).
+  auto bits_of = [](float v) { uint32_t u; memcpy(&u, &v, 4); return u; };
+  auto float_of = [](uint32_t u) { float v; memcpy(&v, &u, 4); return v; };
+  auto bin_of = [&](float Pv) {                              // greatest j in [0, n-1] with edges[j] <= P, 0 if none
+    int b = (int)(std::upper_bound(edges.begin(), edges.end() - 1, Pv) - edges.begin()) - 1;
+    return std::max(b, 0);
+  };
+  std::vector<uint16_t> binlut;
+  c->bin_shift = 0; c->bin_key_lo = 0; c->bin_key_max = 0;
+  for (int m = 3; m <= 12 && c->n_pbins <= 65535; ++m) {
+    const int shift = 23 - m;
+    const uint32_t k_lo = bits_of(c->p_lo) >> shift, k_hi = bits_of(c->p_hi) >> shift;
+    if (k_hi - k_lo + 1 > 16384) break;
+    std::vector<uint16_t> lut(k_hi - k_lo + 1);
+    bool ok = true;
+    for (uint32_t k = k_lo; k <= k_hi && ok; ++k) {
+      const int b_first = bin_of(float_of(k << shift)), b_last = bin_of(float_of(((k + 1) << shift) - 1));
+      ok = (b_last - b_first) <= 1;
+      lut[k - k_lo] = (uint16_t)b_first;
+    }
+    if (ok) { binlut.swap(lut); c->bin_shift = shift; c->bin_key_lo = (int)k_lo; c->bin_key_max = (int)(k_hi - k_lo); break; }
+  }
+  bl.n_words = bl.off_binlut + (int)((binlut.size() + 1) / 2);
+  std::vector<float> blob((size_t)bl.n_words + 4, 0.0f);
+  for (int j = 0; j <= c->n_pbins; ++j) blob[j] = edges[j];
+  if (!binlut.empty()) memcpy(&blob[bl.off_binlut], binlut.data(), binlut.size() * sizeof(uint16_t));
   for (int j = 0; j <= c->n_pbins; ++j)
     blob[bl.off_edges_open + j] = (j == 0) ? -INFINITY : (j == c->n_pbins) ? INFINITY : blob[j];
   for (int m = 0; m <= c->n_materials; ++m) {
@@ -179,7 +222,7 @@ int rebuild_blob(mt_ctx* c) {
     axes_ok = axes_ok && ax[1] >= 0.0f && ax[3] >= 0.0f && ax[0] >= -120.0f && ax[2] >= -120.0f &&
               hi_dp <= -0.0034f && hi_th <= (joint_axes ? 0.0f : -0.36f);
   }
-  c->lean_axes = axes_ok;
+  c->lean_axes = axes_ok && c->bin_shift != 0;               // the lean kernels read the bin from the table
   for (int j = 0; j < n_reg; ++j) {
     blob[bl.off_zlo + j] = c->regions[j].z_lo;
     static_assert(sizeof(mt_region) == 40 && sizeof(MtRegionDev) == 40, "region layout");
@@ -345,6 +388,7 @@ int build_hash(mt_ctx* c, const mt_geometry* gm, const std::vector<mt_poly_block
   c->hnx = hnx; c->hny = hny; c->hnz = hnz;
   c->h_inv[0] = inv[0]; c->h_inv[1] = inv[1]; c->h_inv[2] = inv[2];
   c->hash_list_off = list_off;
+  c->n_hash_list = (uint32_t)n_list;
   return MT_OK;
 }
 
@@ -396,6 +440,9 @@ int mt_create(mt_ctx** out, int cuda_device) {
   if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { delete c; return MT_ERR_CUDA; }
   c->sm_count = prop.multiProcessorCount;
   c->smem_optin = prop.sharedMemPerBlockOptin;
+  if (MT_CHECKED_BUILD) {                // {violations, highest code}: see MT_CHECK in mt_params.h
+    if (c->d_check.reserve(256) != cudaSuccess || cudaMemset(c->d_check.p, 0, 256) != cudaSuccess) { delete c; return MT_ERR_CUDA; }
+  }
   *out = c;
   return MT_OK;
 }
@@ -403,9 +450,17 @@ int mt_create(mt_ctx** out, int cuda_device) {
 int mt_destroy(mt_ctx* c) {
   if (!c) return MT_OK;
   DeviceGuard g(c->device);
-  DevBuf* bufs[] = {&c->d_tab, &c->d_blob, &c->d_grid, &c->d_scratch, &c->d_wave,
+  DevBuf* bufs[] = {&c->d_tab, &c->d_blob, &c->d_grid, &c->d_scratch, &c->d_check,
                     &c->d_stage_in, &c->d_stage_out, &c->d_stage_misc, &c->d_hash};
   for (DevBuf* b : bufs) b->release();
+  for (Lane& L : c->lanes) {
+    if (L.stream) { cudaStreamSynchronize(L.stream); cudaStreamDestroy(L.stream); }
+    if (L.done) cudaEventDestroy(L.done);
+    if (L.ready) cudaEventDestroy(L.ready);
+    L.scratch.release(); L.wave.release();
+  }
+  if (c->copy_in) { cudaStreamSynchronize(c->copy_in); cudaStreamDestroy(c->copy_in); }
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   delete c;
   return MT_OK;
 }
@@ -434,6 +489,12 @@ int mt_set_option(mt_ctx* c, int option, int64_t value) {
       c->opt_min_idle = (int)value; return MT_OK;
     case MT_OPT_NO_LEAN:
       c->opt_no_lean = value != 0; return MT_OK;
+    case MT_OPT_CHECK_SELFTEST:
+      if (!MT_CHECKED_BUILD) return fail(c, MT_ERR_UNSUPPORTED, "not a checked build");
+      c->selftest_bad_bounds = value != 0; return MT_OK;
+    case MT_OPT_LANES:
+      if (value < 0 || value > 16) return fail(c, MT_ERR_INVALID_ARG, "bad lane count");
+      c->opt_lanes = (int)value; return MT_OK;
     case MT_OPT_HASH_NXY:
       if (value < 0 || value > 256) return fail(c, MT_ERR_INVALID_ARG, "bad hash resolution");
       c->opt_hash_nxy = (int)value; return MT_OK;
@@ -644,6 +705,16 @@ int mt_get_info(const mt_ctx* c, int what, int64_t* value) {
     case MT_INFO_LEAN_FACTS: *value = (c->lean_axes ? 1 : 0) | (c->lean_inside ? 2 : 0); return MT_OK;
     case MT_INFO_LAST_LEAN: *value = c->last_lean; return MT_OK;
     case MT_INFO_LAST_SCHEDULE: *value = c->last_sched; return MT_OK;
+    case MT_INFO_LAST_LANES: *value = c->last_lanes; return MT_OK;
+    case MT_INFO_CHECK_ERRORS: {
+      if (!MT_CHECKED_BUILD) { *value = -1; return MT_OK; }
+      unsigned v[2] = {0, 0};
+      DeviceGuard g(c->device);
+      if (cudaDeviceSynchronize() != cudaSuccess || cudaMemcpy(v, c->d_check.p, sizeof v, cudaMemcpyDeviceToHost) != cudaSuccess)
+        return MT_ERR_CUDA;
+      *value = (int64_t)v[0] | ((int64_t)v[1] << 32);
+      return MT_OK;
+    }
     default: return MT_ERR_INVALID_ARG;
   }
 }
@@ -658,6 +729,11 @@ namespace {
 void fill_params(const mt_ctx* c, MtParams& P) {
   memset(&P, 0, sizeof P);
   const mt_geometry& g = c->geom;
+  P.check = (unsigned*)c->d_check.p;
+  P.n_tab_cells = c->selftest_bad_bounds ? 1u : (uint32_t)(c->table_bytes / (c->pack == 32 ? 4 : 8));
+  P.n_grid_cells = (g.mode == MT_GEOM_VOXEL) ? (uint64_t)(g.nx + 2) * (g.ny + 2) * (g.nz + 2) : 0;
+  P.n_hash_cells = (uint32_t)((size_t)c->hnx * c->hny * c->hnz);
+  P.n_hash_list = c->n_hash_list;
   P.mode = g.mode;
   P.x_min = g.x_min; P.x_max = g.x_max; P.y_min = g.y_min; P.y_max = g.y_max; P.z_min = g.z_min; P.z_exit = g.z_exit;
   P.p_min = g.p_min; P.max_steps = g.max_steps; P.world_material = g.world_material;
@@ -685,6 +761,7 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.hash_list = (const uint16_t*)((const char*)c->d_hash.p + c->hash_list_off);
   P.hnx = c->hnx; P.hny = c->hny; P.hnz = c->hnz;
   P.h_inv_x = c->h_inv[0]; P.h_inv_y = c->h_inv[1]; P.h_inv_z = c->h_inv[2];
+  P.bin_shift = c->bin_shift; P.bin_key_lo = c->bin_key_lo; P.bin_key_max = c->bin_key_max;
   P.inv_p_lo = 1.0f / c->p_lo;
   P.bin_scale = (float)((double)c->n_pbins / log2((double)c->p_hi / (double)c->p_lo));
   P.tab32 = (c->pack == 32) ? (const uint32_t*)c->d_tab.p : nullptr;
@@ -693,32 +770,66 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.bl = c->bl;
 }
 
-int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
-                  const mt_muons_out* out, cudaStream_t stream) {
-  if (!c->have_tables || !c->have_geom)
-    return fail(c, MT_ERR_STATE, "mt_transport needs mt_build_alias and mt_set_geometry after the last mt_load_histograms");
-  if (n == 0) return MT_OK;
-  if (!in->pos_q || !in->mom || !out->pos_flag || !out->mom_steps) return fail(c, MT_ERR_INVALID_ARG, "null muon buffer");
-  if (n >= ((uint64_t)1 << 32)) return fail(c, MT_ERR_UNSUPPORTED, "at most 2^32 - 1 muons per call");
-  if (out->exit_rec && !out->exit_count) return fail(c, MT_ERR_INVALID_ARG, "exit_rec without exit_count");
+// Everything about a call that does not depend on which muons a lane holds: the launch configuration, the schedule and,
+// for WAVEFRONT, the slab and sort-key geometry.
+struct Plan {
+  MtParams P;                  // geometry, tables, Philox keys, output pointers of the WHOLE call
+  MtLaunchCfg cfg;
+  int sched = 0;
+  unsigned persistent_grid = 0;
+  double slab = 0.0;           // WAVEFRONT: slab thickness (m), passes, sort keys
+  int n_pass = 0, n_keys = 0;
+};
 
-  MtParams P;
+// One lane = one contiguous range of the call's muons with its own stream and scratch (DESIGN.md §7 "lanes").  The
+// lanes of a call run concurrently: lane 0 on the highest-priority stream, the next ones filling the SMs that its
+// z-slab passes leave idle in their tails (and, for the host-buffer call, computing while other lanes copy).
+struct LaneWork {
+  uint64_t off = 0, n = 0;     // muons [off, off + n) of the call
+  MtParams P;                  // the plan's parameters narrowed to this range
+  unsigned long long* work = nullptr;
+  uint32_t* counts = nullptr;
+  float4* rec[2] = {nullptr, nullptr};
+  unsigned aux_grid = 0, grid = 0;
+};
+
+int ensure_lanes(mt_ctx* c, int K) {
+  if (!c->ev_fork) MT_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+  if (!c->copy_in) MT_CUDA(c, cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking));
+  int least = 0, greatest = 0;
+  MT_CUDA(c, cudaDeviceGetStreamPriorityRange(&least, &greatest));      // greatest = numerically lowest = most urgent
+  while ((int)c->lanes.size() < K) {
+    Lane L;
+    const int prio = std::min(least, greatest + (int)c->lanes.size());
+    MT_CUDA(c, cudaStreamCreateWithPriority(&L.stream, cudaStreamNonBlocking, prio));
+    MT_CUDA(c, cudaEventCreateWithFlags(&L.done, cudaEventDisableTiming));
+    MT_CUDA(c, cudaEventCreateWithFlags(&L.ready, cudaEventDisableTiming));
+    c->lanes.push_back(L);
+  }
+  return MT_OK;
+}
+
+int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Plan& pl) {
+  MtParams& P = pl.P;
   fill_params(c, P);
-  P.n = n; P.id_base = id_base;
   P.key0 = (uint32_t)seed; P.key1 = (uint32_t)(seed >> 32);
   for (uint32_t r = 0; r < 10; ++r) {                       // Philox round keys
     P.rk[2 * r] = P.key0 + r * 0x9E3779B9u;
     P.rk[2 * r + 1] = P.key1 + r * 0xBB67AE85u;
   }
-  P.in_pos_q = (const float4*)in->pos_q; P.in_mom = (const float4*)in->mom;
-  P.out_pos_flag = (float4*)out->pos_flag; P.out_mom_steps = (float4*)out->mom_steps;
   P.exit_rec = (float4*)out->exit_rec; P.exit_count = out->exit_count; P.exit_capacity = out->exit_capacity;
   P.counters = (unsigned long long*)out->counters;
 
   int sched = c->opt_sched;
   // POLY: muons sorted by xy cell and advanced slab by slab share a hash cell and its candidate blocks, so a warp's
   // containment tests stay convergent: 53.0 against 42.0 G muon-steps/s under REFILL (profiles/r1g_poly.md)
-  if (sched == MT_SCHED_AUTO) sched = (c->geom.mode == MT_GEOM_REGIONS) ? MT_SCHED_REFILL : MT_SCHED_WAVEFRONT;
+  // REGIONS: persistent-warp REFILL for small calls (one launch; a 65 536-muon config-1 call is bound by the latency of
+  // one muon's history either way: 0.40 ms against 0.53 ms in slab passes), slab passes from 2^18 muons on, where
+  // same-z warps look up one region and the passes of two lanes overlap (config 2 at 10^6 muons: 12.99 -> 10.9 ms,
+  // profiles/r2b_lanes.md)
+  if (sched == MT_SCHED_AUTO)
+    sched = (c->geom.mode == MT_GEOM_REGIONS && n < ((uint64_t)1 << 18)) ? MT_SCHED_REFILL : MT_SCHED_WAVEFRONT;
+  pl.sched = sched;
   P.refill_min_idle = c->opt_min_idle ? c->opt_min_idle : 1;
 
   // Table placement (north_star subsystem 1).  The packed tables start with the most-used material; shared
@@ -726,7 +837,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   // leaves room for two CTAs per SM and otherwise nothing: on config 3 a shared-memory copy of the iron tables
   // (154 KB, one 768-thread CTA per SM) measured 2 % slower than L1/L2 gathers (profiles/r1c_summary.md).
   // MT_PLACE_SMEM stages as many materials as fit.
-  MtLaunchCfg cfg;
+  MtLaunchCfg& cfg = pl.cfg;
   cfg.pack = c->pack;
   cfg.sched = sched;
   cfg.joint = (c->hist_mode == MT_HIST_JOINT);
@@ -769,87 +880,196 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
     if ((size_t)o * blk > (size_t)occ * cfg.block) { occ = o; cfg.block = blk; }
   }
   if (occ < 1) return fail(c, MT_ERR_UNSUPPORTED, "kernel does not fit on an SM with %zu B shared memory", cfg.smem_bytes);
-  const unsigned persistent_grid = (unsigned)(c->sm_count * occ);
+  pl.persistent_grid = (unsigned)(c->sm_count * occ);
 
-  if (sched == MT_SCHED_STATIC) {
-    cfg.grid = (unsigned)((n + cfg.block - 1) / cfg.block);
-    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
-    c->launches += 1;
-    return MT_OK;
-  }
-
-  if (sched == MT_SCHED_REFILL) {
-    MT_CUDA(c, c->d_scratch.reserve(4096));
-    MT_CUDA(c, cudaMemsetAsync(c->d_scratch.p, 0, 8, stream));
-    P.work_counter = (unsigned long long*)c->d_scratch.p;
-    cfg.grid = (unsigned)std::min<uint64_t>(persistent_grid, (n + cfg.block - 1) / cfg.block);
-    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
-    c->launches += 1;
-    return MT_OK;
-  }
-
-  // WAVEFRONT: one pass per z-slab; between passes the live muons are counting-sorted by xy cell.
-  const bool voxel = (c->geom.mode == MT_GEOM_VOXEL);
-  const double unit = voxel ? (double)c->geom.cell : 0.01;
-  // default slab: 64 cells; small batches are bound by the latency of one muon's ~3000 dependent steps, so they take
-  // thicker slabs (fewer passes to launch) — profiles/r1d_config4_sweep.md
-  const double slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : (n < ((uint64_t)1 << 19) ? 256.0 : 64.0)) * unit;
-  const double span = (double)c->geom.z_exit - (double)c->geom.z_min;
-  const int n_pass = (int)std::max(1.0, std::min(ceil(span / slab), 4096.0));
-  // sort key: the voxel column (coarsened until there are at most 2^18 keys), or a 128 x 128 grid over the world box
-  int key_nx, key_ny;
-  if (voxel) {
-    int coarse = 1;
-    while ((size_t)((c->geom.nx + coarse - 1) / coarse) * ((c->geom.ny + coarse - 1) / coarse) > ((size_t)1 << 18)) coarse *= 2;
-    key_nx = (c->geom.nx + coarse - 1) / coarse; key_ny = (c->geom.ny + coarse - 1) / coarse;
-    P.key_x0 = c->geom.ox; P.key_y0 = c->geom.oy; P.key_inv = 1.0f / (c->geom.cell * (float)coarse);
-  } else {
-    key_nx = key_ny = 128;
-    const float ext = std::max(c->geom.x_max - c->geom.x_min, c->geom.y_max - c->geom.y_min);
-    P.key_x0 = c->geom.x_min; P.key_y0 = c->geom.y_min; P.key_inv = 128.0f / ext;
-  }
-  P.key_nx = key_nx; P.key_ny = key_ny;
-  P.key_look = (float)(slab * 0.01 * (c->opt_key_look >= 0 ? (double)c->opt_key_look : 50.0));
-  const int n_keys = key_nx * key_ny;
-  // scratch: [n_pass + 1] work counters (u64), [n_pass + 1] live counts (u32), histogram and offsets [n_keys] (u32)
-  const size_t off_counts = (size_t)(n_pass + 1) * 8, off_hist = (off_counts + (size_t)(n_pass + 1) * 4 + 255) & ~(size_t)255;
-  const size_t zero_b = off_hist + (size_t)n_keys * 4, scratch_b = zero_b + (size_t)n_keys * 4;
-  MT_CUDA(c, c->d_scratch.reserve(std::max<size_t>(scratch_b, 4096)));
-  MT_CUDA(c, cudaMemsetAsync(c->d_scratch.p, 0, zero_b, stream));
-  unsigned long long* work = (unsigned long long*)c->d_scratch.p;
-  uint32_t* counts = (uint32_t*)((char*)c->d_scratch.p + off_counts);
-  P.hist = (uint32_t*)((char*)c->d_scratch.p + off_hist);
-  P.key_offset = P.hist + n_keys;
-  // in-flight state: two buffers of 48-byte records (read by a pass / parked by it), {key, rank} 8 B and the
-  // permutation 4 B per muon
-  const size_t n48 = ((size_t)n * 48 + 255) & ~(size_t)255, n8 = ((size_t)n * 8 + 255) & ~(size_t)255, n4 = ((size_t)n * 4 + 255) & ~(size_t)255;
-  MT_CUDA(c, c->d_wave.reserve(2 * n48 + n8 + n4));
-  char* w = (char*)c->d_wave.p;
-  float4* rec[2] = {(float4*)w, (float4*)(w + n48)};
-  P.sort_key = (uint2*)(w + 2 * n48);
-  P.perm = (uint32_t*)(w + 2 * n48 + n8);
-  const unsigned aux_grid = (unsigned)std::min<uint64_t>((uint64_t)c->sm_count * 8, (n + 255) / 256);
-  cfg.grid = (unsigned)std::min<uint64_t>(persistent_grid, (n + cfg.block - 1) / cfg.block);
-
-  P.live_out_count = counts;                                   // counts[s] = muons entering pass s
-  MT_CUDA(c, mt_launch_wave_bin(P, aux_grid, stream));
-  MT_CUDA(c, mt_launch_wave_sort(P, n_keys, aux_grid, stream));
-  c->launches += 3;
-  for (int s = 0; s < n_pass; ++s) {
-    P.live_in_count = counts + s;
-    P.live_out_count = counts + s + 1;
-    P.work_counter = work + s;
-    P.first_pass = (s == 0);
-    P.rec_in = rec[(s + 1) & 1];
-    P.rec_out = rec[s & 1];
-    P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * slab);
-    P.lean_z_hi = std::min(c->lean_box[5], P.slab_z_end);
-    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
-    c->launches += 1;
-    if (s < n_pass - 1) {
-      MT_CUDA(c, mt_launch_wave_sort(P, n_keys, aux_grid, stream));
-      c->launches += 2;
+  if (sched == MT_SCHED_WAVEFRONT) {
+    // one pass per z-slab; between passes the live muons are counting-sorted by xy cell
+    const bool voxel = (c->geom.mode == MT_GEOM_VOXEL);
+    const double unit = voxel ? (double)c->geom.cell : 0.01;
+    // default slab (units of 1 cm): voxel grids 64 cells — the slab's field layers stay L2-resident — and 128 for small
+    // batches, which are bound by the latency of one muon's ~3000 dependent steps and want fewer passes; region and
+    // polyhedra geometries have no field working set to bound: 256 (profiles/r2b_lanes.md)
+    const double auto_slab = voxel ? (n < ((uint64_t)1 << 19) ? 128.0 : 64.0) : 256.0;
+    pl.slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : auto_slab) * unit;
+    const double span = (double)c->geom.z_exit - (double)c->geom.z_min;
+    pl.n_pass = (int)std::max(1.0, std::min(ceil(span / pl.slab), 4096.0));
+    // sort key: the voxel column (coarsened until there are at most 2^18 keys), or a 128 x 128 grid over the world box
+    int key_nx, key_ny;
+    if (voxel) {
+      int coarse = 1;
+      while ((size_t)((c->geom.nx + coarse - 1) / coarse) * ((c->geom.ny + coarse - 1) / coarse) > ((size_t)1 << 18)) coarse *= 2;
+      key_nx = (c->geom.nx + coarse - 1) / coarse; key_ny = (c->geom.ny + coarse - 1) / coarse;
+      P.key_x0 = c->geom.ox; P.key_y0 = c->geom.oy; P.key_inv = 1.0f / (c->geom.cell * (float)coarse);
+    } else {
+      key_nx = key_ny = 128;
+      const float ext = std::max(c->geom.x_max - c->geom.x_min, c->geom.y_max - c->geom.y_min);
+      P.key_x0 = c->geom.x_min; P.key_y0 = c->geom.y_min; P.key_inv = 128.0f / ext;
     }
+    P.key_nx = key_nx; P.key_ny = key_ny;
+    P.key_look = (float)(pl.slab * 0.01 * (c->opt_key_look >= 0 ? (double)c->opt_key_look : 50.0));
+    pl.n_keys = key_nx * key_ny;
+    P.n_keys = (uint32_t)pl.n_keys;
+  }
+  return MT_OK;
+}
+
+// HOST buffers of mt_transport_host (null for the device call): each lane copies its own range in and out
+struct HostIO {
+  const float* pos_q; const float* mom;
+  float* pos_flag; float* mom_steps;
+};
+
+int choose_lanes(const mt_ctx* c, uint64_t n, int sched, bool host_call) {
+  if (c->opt_lanes > 0) return (int)std::min<uint64_t>((uint64_t)c->opt_lanes, std::max<uint64_t>(n / 32, 1));
+  // Measured on config 3 and config 2 (profiles/r2b_lanes.md).  Host-buffer calls: four lanes on streams of descending
+  // priority leave only the first lane's copy in and the last lane's copy out exposed (164.4 -> 159.7 ms per 10^7
+  // muons); each further lane costs ~1.2 ms of pass start-up and tails.  Device calls: two lanes let one lane's
+  // passes fill the tails of the other's between 2^17 and 2^22 muons (+3 to +8 %); above that a single lane's passes
+  // are long enough that their tails do not matter (one lane is 1 % faster), below it there is nothing to overlap.
+  // REFILL and STATIC kernels run a muon's whole history in one launch: lanes only serialise them.
+  if (host_call && n >= ((uint64_t)1 << 21)) return 4;
+  if (sched == MT_SCHED_WAVEFRONT && n >= ((uint64_t)1 << 17) && n < ((uint64_t)1 << 22)) return 2;
+  return 1;
+}
+
+int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                  const mt_muons_out* out, cudaStream_t stream, const HostIO* host) {
+  if (!c->have_tables || !c->have_geom)
+    return fail(c, MT_ERR_STATE, "mt_transport needs mt_build_alias and mt_set_geometry after the last mt_load_histograms");
+  if (n == 0) return MT_OK;
+  if (!in->pos_q || !in->mom || !out->pos_flag || !out->mom_steps) return fail(c, MT_ERR_INVALID_ARG, "null muon buffer");
+  if (n >= ((uint64_t)1 << 32)) return fail(c, MT_ERR_UNSUPPORTED, "at most 2^32 - 1 muons per call");
+  if (out->exit_rec && !out->exit_count) return fail(c, MT_ERR_INVALID_ARG, "exit_rec without exit_count");
+
+  Plan pl;
+  int rc = make_plan(c, n, seed, out, pl);
+  if (rc != MT_OK) return rc;
+  const int K = choose_lanes(c, n, pl.sched, host != nullptr);
+  rc = ensure_lanes(c, K);
+  if (rc != MT_OK) return rc;
+  c->last_lanes = K;
+  const uint64_t chunk = (((n + K - 1) / K) + 31) & ~(uint64_t)31;
+
+  // ---- per-lane parameters and scratch
+  std::vector<LaneWork> W(K);
+  const int n_pass = pl.n_pass, n_keys = pl.n_keys;
+  for (int k = 0; k < K; ++k) {
+    LaneWork& w = W[k];
+    Lane& L = c->lanes[k];
+    w.off = std::min<uint64_t>((uint64_t)k * chunk, n);
+    w.n = std::min<uint64_t>(chunk, n - w.off);
+    w.P = pl.P;
+    MtParams& P = w.P;
+    P.n = w.n; P.id_base = id_base + w.off; P.idx_base = (uint32_t)w.off;
+    P.in_pos_q = (const float4*)in->pos_q + w.off; P.in_mom = (const float4*)in->mom + w.off;
+    P.out_pos_flag = (float4*)out->pos_flag + w.off; P.out_mom_steps = (float4*)out->mom_steps + w.off;
+    if (w.n == 0) continue;
+    w.grid = (unsigned)std::min<uint64_t>(pl.persistent_grid, (w.n + pl.cfg.block - 1) / pl.cfg.block);
+    if (pl.sched == MT_SCHED_STATIC) {
+      w.grid = (unsigned)((w.n + pl.cfg.block - 1) / pl.cfg.block);
+    } else if (pl.sched == MT_SCHED_REFILL) {
+      MT_CUDA(c, L.scratch.reserve(4096));
+      P.work_counter = (unsigned long long*)L.scratch.p;
+    } else {
+      // scratch: [n_pass + 1] work counters (u64), [n_pass + 1] live counts (u32), histogram and offsets [n_keys] (u32)
+      const size_t off_counts = (size_t)(n_pass + 1) * 8, off_hist = (off_counts + (size_t)(n_pass + 1) * 4 + 255) & ~(size_t)255;
+      const size_t zero_b = off_hist + (size_t)n_keys * 4, scratch_b = zero_b + (size_t)n_keys * 4;
+      MT_CUDA(c, L.scratch.reserve(std::max<size_t>(scratch_b, 4096)));
+      w.work = (unsigned long long*)L.scratch.p;
+      w.counts = (uint32_t*)((char*)L.scratch.p + off_counts);
+      P.hist = (uint32_t*)((char*)L.scratch.p + off_hist);
+      P.key_offset = P.hist + n_keys;
+      L.zero_bytes = zero_b;
+      // in-flight state: two buffers of 48-byte records (read by a pass / parked by it), {key, rank} 8 B and the
+      // permutation 4 B per muon
+      const size_t n48 = ((size_t)w.n * 48 + 255) & ~(size_t)255, n8 = ((size_t)w.n * 8 + 255) & ~(size_t)255,
+                   n4 = ((size_t)w.n * 4 + 255) & ~(size_t)255;
+      MT_CUDA(c, L.wave.reserve(2 * n48 + n8 + n4));
+      char* wb = (char*)L.wave.p;
+      w.rec[0] = (float4*)wb; w.rec[1] = (float4*)(wb + n48);
+      P.sort_key = (uint2*)(wb + 2 * n48);
+      P.perm = (uint32_t*)(wb + 2 * n48 + n8);
+      w.aux_grid = (unsigned)std::min<uint64_t>((uint64_t)c->sm_count * 8, (w.n + 255) / 256);
+    }
+  }
+
+  // ---- fork: every lane (and the copy-in stream) starts where the caller's stream stands
+  MT_CUDA(c, cudaEventRecord(c->ev_fork, stream));
+  if (host) MT_CUDA(c, cudaStreamWaitEvent(c->copy_in, c->ev_fork, 0));
+  for (int k = 0; k < K; ++k) {
+    if (W[k].n == 0) continue;
+    Lane& L = c->lanes[k];
+    MT_CUDA(c, cudaStreamWaitEvent(L.stream, c->ev_fork, 0));
+    if (host) {
+      // inputs arrive lane by lane on ONE stream (in order, each at full link bandwidth); a lane starts when its own have landed
+      const size_t b = (size_t)W[k].n * 16, o = (size_t)W[k].off * 4;
+      MT_CUDA(c, cudaMemcpyAsync((float*)in->pos_q + o, host->pos_q + o, b, cudaMemcpyHostToDevice, c->copy_in));
+      MT_CUDA(c, cudaMemcpyAsync((float*)in->mom + o, host->mom + o, b, cudaMemcpyHostToDevice, c->copy_in));
+      MT_CUDA(c, cudaEventRecord(L.ready, c->copy_in));
+      MT_CUDA(c, cudaStreamWaitEvent(L.stream, L.ready, 0));
+    }
+  }
+
+  // ---- enqueue: prologues, then pass by pass across the lanes
+  for (int k = 0; k < K; ++k) {
+    LaneWork& w = W[k];
+    if (w.n == 0) continue;
+    Lane& L = c->lanes[k];
+    MtLaunchCfg cfg = pl.cfg;
+    cfg.grid = w.grid;
+    if (pl.sched == MT_SCHED_STATIC) {
+      MT_CUDA(c, mt_launch_transport(w.P, cfg, L.stream));
+      c->launches += 1;
+    } else if (pl.sched == MT_SCHED_REFILL) {
+      MT_CUDA(c, cudaMemsetAsync(L.scratch.p, 0, 8, L.stream));
+      MT_CUDA(c, mt_launch_transport(w.P, cfg, L.stream));
+      c->launches += 1;
+    } else {
+      MT_CUDA(c, cudaMemsetAsync(L.scratch.p, 0, L.zero_bytes, L.stream));
+      w.P.live_out_count = w.counts;                             // counts[s] = muons entering pass s
+      MT_CUDA(c, mt_launch_wave_bin(w.P, w.aux_grid, L.stream));
+      MT_CUDA(c, mt_launch_wave_sort(w.P, n_keys, w.aux_grid, L.stream));
+      c->launches += 3;
+    }
+  }
+  if (pl.sched == MT_SCHED_WAVEFRONT) {
+    for (int s = 0; s < n_pass; ++s) {
+      for (int k = 0; k < K; ++k) {
+        LaneWork& w = W[k];
+        if (w.n == 0) continue;
+        Lane& L = c->lanes[k];
+        MtLaunchCfg cfg = pl.cfg;
+        cfg.grid = w.grid;
+        MtParams& P = w.P;
+        P.live_in_count = w.counts + s;
+        P.live_out_count = w.counts + s + 1;
+        P.work_counter = w.work + s;
+        P.first_pass = (s == 0);
+        P.rec_in = w.rec[(s + 1) & 1];
+        P.rec_out = w.rec[s & 1];
+        P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * pl.slab);
+        P.lean_z_hi = std::min(c->lean_box[5], P.slab_z_end);
+        MT_CUDA(c, mt_launch_transport(P, cfg, L.stream));
+        c->launches += 1;
+        if (s < n_pass - 1) {
+          MT_CUDA(c, mt_launch_wave_sort(P, n_keys, w.aux_grid, L.stream));
+          c->launches += 2;
+        }
+      }
+    }
+  }
+
+  // ---- join: results out (host call), and the caller's stream waits for every lane
+  for (int k = 0; k < K; ++k) {
+    if (W[k].n == 0) continue;
+    Lane& L = c->lanes[k];
+    if (host) {
+      const size_t b = (size_t)W[k].n * 16, o = (size_t)W[k].off * 4;
+      MT_CUDA(c, cudaMemcpyAsync(host->pos_flag + o, out->pos_flag + o, b, cudaMemcpyDeviceToHost, L.stream));
+      MT_CUDA(c, cudaMemcpyAsync(host->mom_steps + o, out->mom_steps + o, b, cudaMemcpyDeviceToHost, L.stream));
+    }
+    MT_CUDA(c, cudaEventRecord(L.done, L.stream));
+    MT_CUDA(c, cudaStreamWaitEvent(stream, L.done, 0));
   }
   return MT_OK;
 }
@@ -862,19 +1082,16 @@ int mt_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base,
                  const mt_muons_out* out, void* cuda_stream) {
   if (!c || !in || !out) return MT_ERR_INVALID_ARG;
   DeviceGuard g(c->device);
-  return run_transport(c, in, n, id_base, seed, out, (cudaStream_t)cuda_stream);
+  return guarded(c, [&] { return run_transport(c, in, n, id_base, seed, out, (cudaStream_t)cuda_stream, nullptr); });
 }
 
-int mt_transport_host(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
-                      const mt_muons_out* out, void* cuda_stream) {
-  if (!c || !in || !out) return MT_ERR_INVALID_ARG;
+static int transport_host_impl(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                               const mt_muons_out* out, cudaStream_t stream) {
   if (n == 0) return MT_OK;
   if (!in->pos_q || !in->mom || !out->pos_flag || !out->mom_steps) return fail(c, MT_ERR_INVALID_ARG, "null muon buffer");
   if (out->exit_rec && !out->exit_count) return fail(c, MT_ERR_INVALID_ARG, "exit_rec without exit_count");
   if (!c->have_tables || !c->have_geom)
     return fail(c, MT_ERR_STATE, "mt_transport needs mt_build_alias and mt_set_geometry after the last mt_load_histograms");
-  DeviceGuard g(c->device);
-  cudaStream_t stream = (cudaStream_t)cuda_stream;
   const size_t rec = n * 4 * sizeof(float);
   MT_CUDA(c, c->d_stage_in.reserve(2 * rec));
   MT_CUDA(c, c->d_stage_out.reserve(2 * rec));
@@ -883,8 +1100,6 @@ int mt_transport_host(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_
   char* d_in = (char*)c->d_stage_in.p;
   char* d_out = (char*)c->d_stage_out.p;
   char* d_misc = (char*)c->d_stage_misc.p;
-  MT_CUDA(c, cudaMemcpyAsync(d_in, in->pos_q, rec, cudaMemcpyHostToDevice, stream));
-  MT_CUDA(c, cudaMemcpyAsync(d_in + rec, in->mom, rec, cudaMemcpyHostToDevice, stream));
   MT_CUDA(c, cudaMemsetAsync(d_misc, 0, 128, stream));
   mt_muons_in din = {(const float*)d_in, (const float*)(d_in + rec)};
   mt_muons_out dout;
@@ -897,15 +1112,22 @@ int mt_transport_host(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_
     dout.exit_rec = (float*)(d_misc + 128);
     dout.exit_capacity = out->exit_capacity;
   }
-  const int rc = run_transport(c, &din, n, id_base, seed, &dout, stream);
+  // the muon state is copied lane by lane inside run_transport, so that one lane computes while others copy
+  const HostIO io = {in->pos_q, in->mom, out->pos_flag, out->mom_steps};
+  const int rc = run_transport(c, &din, n, id_base, seed, &dout, stream, &io);
   if (rc != MT_OK) return rc;
-  MT_CUDA(c, cudaMemcpyAsync(out->pos_flag, d_out, rec, cudaMemcpyDeviceToHost, stream));
-  MT_CUDA(c, cudaMemcpyAsync(out->mom_steps, d_out + rec, rec, cudaMemcpyDeviceToHost, stream));
   if (out->counters) MT_CUDA(c, cudaMemcpyAsync(out->counters, d_misc, 64, cudaMemcpyDeviceToHost, stream));
   if (out->exit_count) MT_CUDA(c, cudaMemcpyAsync(out->exit_count, d_misc + 64, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
   if (out->exit_rec) MT_CUDA(c, cudaMemcpyAsync(out->exit_rec, d_misc + 128, exit_b, cudaMemcpyDeviceToHost, stream));
   MT_CUDA(c, cudaStreamSynchronize(stream));
   return MT_OK;
+}
+
+int mt_transport_host(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                      const mt_muons_out* out, void* cuda_stream) {
+  if (!c || !in || !out) return MT_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  return guarded(c, [&] { return transport_host_impl(c, in, n, id_base, seed, out, (cudaStream_t)cuda_stream); });
 }
 
 int mt_debug_sample(mt_ctx* c, int material, int pbin, int which, const uint32_t* d_words, uint64_t n,

@@ -19,8 +19,9 @@ struct MtRegionDev {
 //   [off_zlo  + j]                       z_lo of region j (search array)
 //   [off_regions + 10*j ..]              MtRegionDev j
 //   [off_blocks + 24*j ..]               MtBlockDev j (POLY mode)
+//   [off_binlut ..]                      uint16 momentum-bin table (two per word), see MtParams::bin_shift
 struct MtBlobLayout {
-  int32_t off_edges_open, off_steps, off_axes, off_zlo, off_regions, off_blocks, n_words;
+  int32_t off_edges_open, off_steps, off_axes, off_zlo, off_regions, off_blocks, off_binlut, n_words;
 };
 
 // Polyhedra block as staged in shared memory: six float4.  inv_dz = 1 / (z_hi - z_lo), dx_i = xh_i - xl_i and
@@ -45,11 +46,39 @@ struct __align__(32) MtCellPair {
 //                   ends below log2(0.999) with a margin of 2^-9 (the cap on f) and every theta axis below log2(0.78)
 //                   (theta < pi/4: the cap at pi and the quadrant reduction of its sine and cosine); JOINT tables: the
 //                   transverse axis ends at or below 0 (ft <= 1: the new |p| stays in the fast sqrt / rcp range)
+//                   and the momentum-bin table exists (bin_shift != 0): the bin is read from it instead of being seeded
+//                   with a logarithm
 //   MT_LEAN_INSIDE  lean_{x,y,z}_{lo,hi} bound the part of the world box whose every float32 position maps to a cell of
 //                   the voxel grid (the whole box but for a few floats next to a face, which take the general code)
 enum { MT_LEAN_AXES = 1, MT_LEAN_INSIDE = 2, MT_LEAN_ALL = 3 };
 
+// Checked build (-DMT_CHECKED, `python -m paper_2512_10520_b200.build --checked` -> libmuon_transport_checked.so): every
+// index the kernels form into a global array is compared with the array's size first, and a violation is counted in
+// MtParams::check instead of being dereferenced.  compute-sanitizer is not available on the GPU pool this was developed on
+// (profiles/r2_sanitizers.md); this is the bounds check of our own that stands in for memcheck.  In the normal build the
+// macro expands to nothing.
+enum {
+  MT_CHK_INPUT = 1, MT_CHK_PERM = 2, MT_CHK_RECORD = 3, MT_CHK_PARK_SLOT = 4, MT_CHK_SORT_KEY = 5, MT_CHK_TABLE = 6,
+  MT_CHK_GRID = 7, MT_CHK_HASH = 8, MT_CHK_PBIN = 9, MT_CHK_MATERIAL = 10, MT_CHK_PERM_SLOT = 11, MT_CHK_OUTPUT = 12
+};
+#ifdef MT_CHECKED
+#define MT_CHECK(P, cond, code)                                    \
+  do {                                                             \
+    if (!(cond)) { atomicAdd((P).check, 1u); atomicMax((P).check + 1, (unsigned)(code)); } \
+  } while (0)
+#define MT_CHECKED_BUILD 1
+#else
+#define MT_CHECK(P, cond, code) ((void)0)
+#define MT_CHECKED_BUILD 0
+#endif
+
 struct MtParams {
+  // ---- checked build: {violations, highest MT_CHK_* code seen}, and the sizes the indices are held to
+  unsigned* check;
+  uint32_t n_tab_cells;          // cells of the packed alias tables
+  uint64_t n_grid_cells;         // records of the padded field grid
+  uint32_t n_keys;               // WAVEFRONT sort keys
+  uint32_t n_hash_cells, n_hash_list;
   // ---- geometry
   int32_t mode;
   float x_min, x_max, y_min, y_max, z_min, z_exit, p_min;
@@ -68,6 +97,11 @@ struct MtParams {
   // ---- tables
   int32_t n_materials, n_pbins, n_dp, n_th;
   float inv_p_lo, bin_scale;     // bin guess: floor(log2(P * inv_p_lo) * bin_scale), then fixed on the edges
+  // Momentum-bin table (LEAN kernels): key = (bits(P) >> bin_shift) - bin_key_lo, clamped to
+  // [0, bin_key_max], names a run of consecutive floats; binlut[key] is the bin (§3.4) of the run's smallest float and the
+  // host has checked that no run holds more than one edge, so the bin of P is binlut[key] or the next one: ONE comparison
+  // with the float32 edge decides, as §3.4 demands, and no logarithm is taken.  bin_shift = 0: no table (bins too narrow).
+  int32_t bin_shift, bin_key_lo, bin_key_max;
   const uint32_t* tab32;         // pack32: [material block][pbin][n_dp + n_th] = threshold24 << 8 | alias8; the blocks are
   const uint2* tab64;            // ordered most-used material first.  pack64: same shape, {threshold (<= 2^24), alias}
   const float* blob;             // const blob (global copy)
@@ -87,7 +121,8 @@ struct MtParams {
   int32_t hnx, hny, hnz;
   float h_inv_x, h_inv_y, h_inv_z;   // cells per metre along each axis
   // ---- this call
-  uint64_t n, id_base;
+  uint64_t n, id_base;           // this lane's muons: n of them, the first with id id_base (= the call's id_base + idx_base)
+  uint32_t idx_base;             // index of this lane's first muon within the call (exit records carry call indices)
   uint32_t key0, key1;           // Philox key = seed lo, hi
   uint32_t rk[20];               // the ten round keys (key + r * Weyl), precomputed on the host
   const float4* in_pos_q;

@@ -3,7 +3,7 @@ import numpy as np
 
 
 def gpu_transport(mt, wl, sched=0, block=0, placement=0, id_base=0, exit_capacity=0, min_idle=0, slab=0,
-                  sel=None, handle=None):
+                  sel=None, handle=None, lanes=0):
     """Run workload `wl` on cuda:0 through the binding; returns numpy dict (pos, mom, flag, steps, ...)."""
     import torch
     b = mt.binding
@@ -12,6 +12,7 @@ def gpu_transport(mt, wl, sched=0, block=0, placement=0, id_base=0, exit_capacit
     try:
         h.set_option(b.MT_OPT_SCHEDULE, sched).set_option(b.MT_OPT_BLOCK_THREADS, block)
         h.set_option(b.MT_OPT_REFILL_MIN_IDLE, min_idle).set_option(b.MT_OPT_SLAB_CELLS, slab)
+        h.set_option(b.MT_OPT_LANES, lanes)
         pos_q, mom = wl.muons.pos_q, wl.muons.mom
         if sel is not None:
             pos_q, mom = pos_q[sel], mom[sel]
@@ -24,6 +25,9 @@ def gpu_transport(mt, wl, sched=0, block=0, placement=0, id_base=0, exit_capacit
         if exit_capacity:
             res["exit_count"] = int(out["exit_count"].cpu().numpy()[0])
             res["exit_rec"] = out["exit_rec"].cpu().numpy()
+        # checked build (MUON_TRANSPORT_LIB=...libmuon_transport_checked.so): no index left its array
+        errors = b.mt_get_info(h.ctx, b.MT_INFO_CHECK_ERRORS)
+        assert errors in (0, -1), "bounds violations: %d, highest code %d" % (errors & 0xFFFFFFFF, errors >> 32)
         return res
     finally:
         if own:

@@ -1,8 +1,11 @@
-"""Target program for compute-sanitizer (not a pytest file):
+"""Target program for memory checking (not a pytest file):
 
-    compute-sanitizer --tool memcheck  python tests/sanitize_target.py
-    compute-sanitizer --tool racecheck python tests/sanitize_target.py
-    compute-sanitizer --tool initcheck python tests/sanitize_target.py [--quick]
+    MUON_TRANSPORT_LIB=paper_2512_10520_b200/libmuon_transport_checked.so python tests/sanitize_target.py --checked
+    compute-sanitizer --tool memcheck  python tests/sanitize_target.py [--quick]      (where the tool is available)
+    compute-sanitizer --tool racecheck python tests/sanitize_target.py [--quick]
+
+--checked: the library is the bounds-checked build (paper_2512_10520_b200/build.py --checked); every case must finish
+with zero violations, and a self-test that hands the kernels a wrong table size must make the checks fire.
 
 Small transports through every schedule (STATIC, REFILL, WAVEFRONT: park / index-sort path with its per-key atomics,
 single-CTA scan and alternating record buffers), both table placements (L2 gathers and the shared-memory staged copy),
@@ -56,6 +59,18 @@ def main():
     h = b.MuonTransport(0).setup(wl3.hist, wl3.geom)
     out = h.transport_host(wl3.muons.pos_q, wl3.muons.mom, wl3.seed, exit_capacity=64)
     assert compare(unpack(out["pos_flag"], out["mom_steps"]), ref3)["bit_exact"] == 1.0
+    h.set_option(b.MT_OPT_LANES, 3)
+    out = h.transport_host(wl3.muons.pos_q, wl3.muons.mom, wl3.seed, exit_capacity=64)
+    assert compare(unpack(out["pos_flag"], out["mom_steps"]), ref3)["bit_exact"] == 1.0
+    if "--checked" in sys.argv:
+        assert b.mt_get_info(h.ctx, b.MT_INFO_CHECK_ERRORS) == 0, "this is not the checked build, or a check fired"
+        # the checks are alive: with a table size of one cell nearly every alias draw is out of bounds (and is counted,
+        # not dereferenced)
+        h.set_option(b.MT_OPT_CHECK_SELFTEST, 1)
+        h.transport_host(wl3.muons.pos_q, wl3.muons.mom, wl3.seed)
+        errors = b.mt_get_info(h.ctx, b.MT_INFO_CHECK_ERRORS)
+        assert (errors & 0xFFFFFFFF) > 1000 and (errors >> 32) == 6, errors            # MT_CHK_TABLE
+        print("checked build: 0 violations in every case; self-test fired %d times (code %d)" % (errors & 0xFFFFFFFF, errors >> 32))
     h.close()
     torch.cuda.synchronize()
     print("sanitize_target: all cases bit-exact against the oracle")

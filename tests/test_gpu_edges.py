@@ -27,7 +27,9 @@ def test_results_do_not_depend_on_launch_shape(mt, wl1, ref1):
     assert compare(base, ref1)["bit_exact"] == 1.0
     for kw in (dict(sched=1, block=32), dict(sched=2, block=64, min_idle=1), dict(sched=2, block=256, min_idle=16),
                dict(sched=2, block=128, min_idle=32), dict(sched=3, block=96, slab=10), dict(sched=3, slab=1000),
-               dict(sched=2, placement=2), dict(sched=2, placement=1)):
+               dict(sched=2, placement=2), dict(sched=2, placement=1),
+               # concurrent lanes (contiguous id ranges on the library's own streams): ragged last lane, more lanes than fit
+               dict(sched=3, lanes=2), dict(sched=3, lanes=7, slab=30), dict(sched=2, lanes=3), dict(sched=1, lanes=16)):
         assert _same(gpu_transport(mt, wl1, **kw), base), kw
 
 
@@ -114,6 +116,14 @@ def test_exit_records_and_counters(mt, wl1, ref1):
     assert len(np.unique(idx)) == n_exit and np.array_equal(np.sort(idx), np.nonzero(ref1["flag"] == 2)[0])
     assert np.array_equal(rec[:, :3], ref1["pos"][idx]) and np.array_equal(rec[:, 4:7], ref1["mom"][idx])
     assert np.array_equal(rec[:, 7].copy().view(np.int32), ref1["steps"][idx])
+    # lanes: the records carry the index within the CALL, not within the lane
+    for sched in (2, 3):
+        g = gpu_transport(mt, wl1, sched=sched, exit_capacity=n, lanes=5)
+        assert g["exit_count"] == n_exit
+        rec = g["exit_rec"][:n_exit]
+        idx = rec[:, 3].copy().view(np.uint32)
+        assert np.array_equal(np.sort(idx), np.nonzero(ref1["flag"] == 2)[0])
+        assert np.array_equal(rec[:, :3], ref1["pos"][idx]) and np.array_equal(rec[:, 4:7], ref1["mom"][idx])
     # capacity smaller than the number of hits: the count still reports all, only `capacity` records are written
     g = gpu_transport(mt, wl1, sched=3, exit_capacity=100)
     assert g["exit_count"] == n_exit
@@ -158,6 +168,12 @@ def test_host_buffer_call(mt, wl1, ref1):
         g = unpack(out["pos_flag"], out["mom_steps"])
         assert compare(g, ref1)["bit_exact"] == 1.0
         assert out["counters"][0] == ref1["steps"].sum() and out["exit_count"][0] == (ref1["flag"] == 2).sum()
+        # lanes copy their own ranges in and out
+        h.set_option(b.MT_OPT_LANES, 3)
+        out = h.transport_host(wl1.muons.pos_q, wl1.muons.mom, wl1.seed, exit_capacity=64)
+        assert compare(unpack(out["pos_flag"], out["mom_steps"]), ref1)["bit_exact"] == 1.0
+        assert out["counters"][0] == ref1["steps"].sum() and out["exit_count"][0] == (ref1["flag"] == 2).sum()
+        assert b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES) == 3
         # pinned torch tensors work too
         pq = torch.from_numpy(wl1.muons.pos_q).pin_memory()
         mo = torch.from_numpy(wl1.muons.mom).pin_memory()
