@@ -169,8 +169,11 @@ def make_workload(config, n_muons, device, rank, joint=False, field_mode=0, poly
         wl = w.config1(n=8, joint=joint, n_draws=n_draws)
         wl.geom.field_mode = field_mode & 2
         wl.muons = w.spectrum_muons(1, n_muons, "gauss", batch=rank)
+    elif config == 0:
+        # the oracle-sized parity case (4096 identical muons by default): timed only to fill BASELINE.md's table
+        wl = w.config0(n=n_muons, joint=joint, n_draws=n_draws)
     else:
-        raise SystemExit("bench.py times configs 1, 2 and 3 (config 0 is the oracle-sized parity case)")
+        raise SystemExit("bench.py times BASELINE.json configs 0-3; configs[4] is --sweep")
     log("[bench] rank %d: %s, %d muons generated in %.1f s" % (rank, wl.name, n_muons, time.time() - t0))
     return wl
 
@@ -210,7 +213,7 @@ def run_reference(args, rank, world):
     import torch
     dev = "cuda" if torch.cuda.is_available() else "cpu"          # the grid generator may use the GPU; the timed code never does
     wl = make_workload(args.config, args.muons, dev, 0, args.joint, args.field_mode, args.poly, args.draws)
-    cores, desc, runner = oracle_sample(wl, args.muons, 0, args.ref_seconds)
+    cores, desc, runner = oracle_sample(wl, args.muons, 0, args.ref_seconds, threads=args.ref_threads or None)
     for _ in range(args.warmup):
         runner()
     t_tot, s_tot, m_tot = 0.0, 0, 0
@@ -502,18 +505,28 @@ def main():
     ap.add_argument("--lanes", type=int, default=0, help="MT_OPT_LANES: concurrent lanes per call (0 = library default)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-seconds", type=float, default=15.0, help="CPU work per oracle sample")
+    ap.add_argument("--ref-threads", type=int, default=0, help="--impl reference: oracle threads (0 = all host cores)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--joint", action="store_true", help="the paper's joint 2D histograms (DESIGN.md 3.10) instead of two 1D ones")
     ap.add_argument("--field-mode", type=int, default=0, help="MT_FIELD_*: 1 nearest, 2 per-stage, 3 both (DESIGN.md 3.11)")
     ap.add_argument("--no-lean", action="store_true", help="MT_OPT_NO_LEAN: general kernels even where the lean variant applies")
     ap.add_argument("--poly", action="store_true", help="with --config 2: the convex-polyhedra shield (DESIGN.md 3.12)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
+    ap.add_argument("--probes", action="store_true", help="only the in-process peak and field-path probes (one JSON line)")
     ap.add_argument("--draws", type=int, default=1_000_000, help="draws per generated histogram (BASELINE.json: 10^6)")
     ap.add_argument("--sweep-batches", type=int, default=10)
     ap.add_argument("--sweep-draws", type=int, default=1_000_000, help="draws per generated histogram")
     args = ap.parse_args()
     if args.warmup < 1:
         args.warmup = 1
+    if args.probes:
+        from paper_2512_10520_b200 import binding as b, build as lib_build
+        lib_build.build()
+        fp = b.mt_probe_field_paths(0)
+        print(json.dumps({"measured_peaks": b.mt_measure_peaks(0),
+                          "field_paths_TB_per_s": {k[:3]: v * 32 / 1e12 for k, v in fp.items() if k.endswith("_per_s")},
+                          "field_paths_records_per_launch": fp["records_per_launch"]}), flush=True)
+        return
     if args.gpus < 1:
         raise SystemExit("bench.py: --gpus must be at least 1")
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not args.sweep:

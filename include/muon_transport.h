@@ -248,6 +248,17 @@ typedef struct {
 } mt_peaks;
 int mt_measure_peaks(int cuda_device, mt_peaks* out);
 
+/* The three ways of serving the trilinear field corners that north_star subsystem (5) names, timed on one synthetic
+ * access pattern (csrc/mt_probe_field.cu): read-only 256-bit global loads (what the transport kernels use), point-sampled
+ * 3D texture fetches, and a shared-memory window staged by TMA (cp.async.bulk.tensor).  Rates are 32-byte corner records
+ * per second over the whole GPU; tma_records_per_s = 0 if the driver offers no cuTensorMapEncodeTiled.  ~100 MB of
+ * temporary device memory; synchronises.  Not on the transport path. */
+typedef struct {
+  double records_per_launch;
+  double ldg_records_per_s, tex_records_per_s, tma_records_per_s;
+} mt_field_paths;
+int mt_probe_field_paths(int cuda_device, mt_field_paths* out);
+
 /* Test hooks (DEVICE buffers, asynchronous on the stream).
  * mt_debug_sample: cell_out[i] = alias draw from table `which` (0 = Dp/p, 1 = theta) of
  * (material, pbin) with word d_words[i].  JOINT mode (which = 0): d_words holds 2n words, the select word of draw i

@@ -27,7 +27,7 @@ MT_FIELD_TRILINEAR, MT_FIELD_NEAREST, MT_FIELD_PER_STAGE = 0, 1, 2
 # every symbol include/muon_transport.h declares (tests check that the library exports each one)
 SYMBOLS = ["mt_strerror", "mt_last_error", "mt_create", "mt_destroy", "mt_set_option", "mt_load_histograms",
            "mt_build_alias", "mt_get_alias", "mt_set_geometry", "mt_transport", "mt_transport_host",
-           "mt_launch_count", "mt_get_info", "mt_measure_peaks", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
+           "mt_launch_count", "mt_get_info", "mt_measure_peaks", "mt_probe_field_paths", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
 
 
 class mt_hist_desc(C.Structure):
@@ -69,6 +69,11 @@ class mt_peaks(C.Structure):
                 ("gather_64m_bytes_per_s", C.c_double), ("gather_1400m_bytes_per_s", C.c_double)]
 
 
+class mt_field_paths(C.Structure):
+    _fields_ = [("records_per_launch", C.c_double), ("ldg_records_per_s", C.c_double),
+                ("tex_records_per_s", C.c_double), ("tma_records_per_s", C.c_double)]
+
+
 class mt_muons_in(C.Structure):
     _fields_ = [("pos_q", C.c_void_p), ("mom", C.c_void_p)]
 
@@ -107,6 +112,7 @@ def lib():
         L.mt_launch_count.argtypes = [C.c_void_p]
         L.mt_get_info.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]
         L.mt_measure_peaks.argtypes = [C.c_int, C.POINTER(mt_peaks)]
+        L.mt_probe_field_paths.argtypes = [C.c_int, C.POINTER(mt_field_paths)]
         L.mt_debug_sample.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_philox.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -321,6 +327,15 @@ def mt_measure_peaks(device=0):
     if rc != MT_OK:
         raise MtError(rc, "mt_measure_peaks(device=%d)" % device)
     return {name: getattr(p, name) for name, _ in mt_peaks._fields_}
+
+
+def mt_probe_field_paths(device=0):
+    """corner records per second through global loads / texture fetches / a TMA-staged shared-memory window"""
+    p = mt_field_paths()
+    rc = lib().mt_probe_field_paths(int(device), C.byref(p))
+    if rc != MT_OK:
+        raise MtError(rc, "mt_probe_field_paths(device=%d)" % device)
+    return {name: getattr(p, name) for name, _ in mt_field_paths._fields_}
 
 
 def mt_debug_sample(ctx, material, pbin, which, words, stream=None, joint=False):

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmuon_transport.so")
 SOURCES = ["mt_lib.cu", "mt_kernels.cu", "mt_inst_regions.cu", "mt_inst_poly.cu", "mt_inst_voxel_a.cu",
-           "mt_inst_voxel_b.cu", "mt_inst_lean.cu", "mt_probe.cu"]
+           "mt_inst_voxel_b.cu", "mt_inst_lean.cu", "mt_probe.cu", "mt_probe_field.cu"]
 DEPS = SOURCES + ["mt_kernels.cuh", "mt_step.cuh", "mt_params.h", "mt_launch.h"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
