@@ -449,6 +449,93 @@ def run_sweep(args):
             h.close()
 
 
+def run_sweep_lanes(args):
+    """How a call is cut up (DESIGN.md §7 "lanes"): muons per call x slab thickness x concurrent lanes on config 3
+    (device-resident and host-buffer calls) and schedule x slab x lanes on configs 2, 2p and 1.  One JSON line per point;
+    best of `--steps` timed calls after one warm-up call."""
+    import torch
+    from paper_2512_10520_b200 import binding as b, build as lib_build, workloads as w
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the transport path has no CPU fallback")
+    lib_build.build()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    stream = torch.cuda.Stream(device=dev)
+    nominal = SM_COUNT * LANES_PER_SM * load_peaks()["sm_max_mhz"] * 1e6
+
+    def timed(h, dq, dm, out):
+        best, steps = None, 0
+        for r in range(args.steps + 1):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(stream):
+                e0.record(stream)
+                res = h.transport(dq, dm, 1, out=out, stream=stream)
+                e1.record(stream)
+                stream.synchronize()
+            steps = int(res["counters"][0].item())
+            if r > 0:
+                best = e0.elapsed_time(e1) if best is None else min(best, e0.elapsed_time(e1))
+        return best, steps
+
+    def timed_host(h, hq, hm, hout):
+        best = None
+        for r in range(args.steps + 1):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            h.transport_host(hq, hm, 1, out=hout, stream=stream)
+            torch.cuda.synchronize()
+            if r > 0:
+                dt = (time.perf_counter() - t0) * 1e3
+                best = dt if best is None else min(best, dt)
+        return best
+
+    def emit(ops, ms, steps, **kw):
+        kw.update(ms=round(ms, 3), G_muon_steps_per_s=round(steps / ms / 1e6, 2), frac_nominal=round(steps / ms * 1e3 * ops / nominal, 3))
+        print(json.dumps(kw), flush=True)
+
+    wl = w.config3(n=8, device=dev, n_draws=args.draws)
+    mu = w.spectrum_muons(3, args.muons, "square")
+    h = b.MuonTransport(0).setup(wl.hist, wl.geom)
+    wl.geom.material = wl.geom.field = None
+    torch.cuda.empty_cache()
+    dq, dm = torch.from_numpy(mu.pos_q).to(dev), torch.from_numpy(mu.mom).to(dev)
+    out = {"pos_flag": torch.empty((len(dq), 4), device=dev), "mom_steps": torch.empty((len(dq), 4), device=dev)}
+    for n in sorted({min(1 << 18, args.muons), min(1 << 20, args.muons), min(1 << 22, args.muons), args.muons}):
+        o = {k: v[:n] for k, v in out.items()}
+        for slab in (0, 64, 128, 256):
+            for lanes in (0, 1, 2, 4):
+                h.set_option(b.MT_OPT_LANES, lanes).set_option(b.MT_OPT_SLAB_CELLS, slab)
+                ms, st = timed(h, dq[:n], dm[:n], o)
+                emit(ALG_OPS_PER_STEP["voxel"], ms, st, workload="config3", call="device", muons=n, slab_cells=slab,
+                     lanes=lanes or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES))
+    hq, hm = torch.from_numpy(mu.pos_q).pin_memory(), torch.from_numpy(mu.mom).pin_memory()
+    hout = {"pos_flag": torch.empty((len(hq), 4)).pin_memory(), "mom_steps": torch.empty((len(hq), 4)).pin_memory()}
+    h.set_option(b.MT_OPT_SLAB_CELLS, 0)
+    for lanes in (0, 1, 2, 4, 6, 8):
+        h.set_option(b.MT_OPT_LANES, lanes)
+        ms = timed_host(h, hq, hm, hout)
+        emit(ALG_OPS_PER_STEP["voxel"], ms, st, workload="config3", call="host (e2e)", muons=len(hq),
+             lanes=lanes or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES))
+    h.close()
+    del dq, dm, out, hq, hm, hout
+    torch.cuda.empty_cache()
+    for name, wl, mode in (("config2", w.config2(n=1_000_000, n_draws=args.draws), "regions"),
+                           ("config2p", w.config2p(n=1_000_000, n_draws=args.draws), "poly"),
+                           ("config1", w.config1(n=65536, n_draws=args.draws), "regions")):
+        h = b.MuonTransport(0).setup(wl.hist, wl.geom)
+        dq, dm = torch.from_numpy(wl.muons.pos_q).to(dev), torch.from_numpy(wl.muons.mom).to(dev)
+        out = {"pos_flag": torch.empty((len(dq), 4), device=dev), "mom_steps": torch.empty((len(dq), 4), device=dev)}
+        for sched in (0, 2, 3):
+            for slab in ((0,) if sched != 3 else (64, 128, 256)):
+                for lanes in ((0,) if sched == 0 else (1, 2, 4)):
+                    h.set_option(b.MT_OPT_SCHEDULE, sched).set_option(b.MT_OPT_LANES, lanes).set_option(b.MT_OPT_SLAB_CELLS, slab)
+                    ms, st = timed(h, dq, dm, out)
+                    emit(ALG_OPS_PER_STEP[mode], ms, st, workload=name, call="device", muons=len(dq),
+                         schedule=sched or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_SCHEDULE), slab_cells=slab,
+                         lanes=lanes or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES))
+        h.close()
+
+
 def self_launch(n_gpus):
     """`python bench.py --gpus N` with N > 1 and no torchrun environment: start the N ranks ourselves, one process per
     GPU, exactly as the driver's own command line would (torch.distributed.run, 127.0.0.1 rendezvous), and pass the
@@ -512,6 +599,7 @@ def main():
     ap.add_argument("--no-lean", action="store_true", help="MT_OPT_NO_LEAN: general kernels even where the lean variant applies")
     ap.add_argument("--poly", action="store_true", help="with --config 2: the convex-polyhedra shield (DESIGN.md 3.12)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
+    ap.add_argument("--sweep-lanes", action="store_true", help="lanes x slab x muons-per-call sweep (profiles/r2b_lanes.md)")
     ap.add_argument("--probes", action="store_true", help="only the in-process peak and field-path probes (one JSON line)")
     ap.add_argument("--draws", type=int, default=1_000_000, help="draws per generated histogram (BASELINE.json: 10^6)")
     ap.add_argument("--sweep-batches", type=int, default=10)
@@ -527,6 +615,8 @@ def main():
                           "field_paths_TB_per_s": {k[:3]: v * 32 / 1e12 for k, v in fp.items() if k.endswith("_per_s")},
                           "field_paths_records_per_launch": fp["records_per_launch"]}), flush=True)
         return
+    if args.sweep_lanes:
+        return run_sweep_lanes(args)
     if args.gpus < 1:
         raise SystemExit("bench.py: --gpus must be at least 1")
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not args.sweep:

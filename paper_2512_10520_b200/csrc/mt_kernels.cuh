@@ -40,6 +40,7 @@ MT_DEV View<PACK> stage_view(const MtParams& P) {
   V.regions = reinterpret_cast<const MtRegionDev*>(sblob + P.bl.off_regions);
   V.blocks = reinterpret_cast<const MtBlockDev*>(sblob + P.bl.off_blocks);
   V.binlut = reinterpret_cast<const uint16_t*>(sblob + P.bl.off_binlut);
+  V.zlut = reinterpret_cast<const int16_t*>(sblob + P.bl.off_zlut);
   const uint32_t* gtab = (PACK == 32) ? P.tab32 : reinterpret_cast<const uint32_t*>(P.tab64);
   V.tab = reinterpret_cast<const typename Tab<PACK>::cell_t*>(gtab);
   uint4* stab = reinterpret_cast<uint4*>(sblob + ((P.bl.n_words + 3) & ~3));

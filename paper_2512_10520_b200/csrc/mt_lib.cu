@@ -75,6 +75,8 @@ struct mt_ctx {
   size_t hash_list_off = 0;              // byte offset of the candidate lists inside d_hash
   uint32_t n_hash_list = 0;              // entries of the candidate lists
   int bin_shift = 0, bin_key_lo = 0, bin_key_max = 0;   // momentum-bin table (mt_params.h)
+  int zlut_n = 0;                        // z-interval table (mt_params.h)
+  float zlut_g0 = 0, zlut_inv = 0;
   int selftest_bad_bounds = 0;           // checked build: hand the kernels a wrong table size (MT_OPT_CHECK_SELFTEST)
   MtBlobLayout bl{};
   int64_t launches = 0;
@@ -161,7 +163,7 @@ int rebuild_blob(mt_ctx* c) {
   bl.off_steps = (bl.off_edges_open + n_edges + 3) & ~3;
   bl.off_axes = bl.off_steps + 4 * (c->n_materials + 1);
   bl.off_zlo = bl.off_axes + 4 * nt;
-  bl.off_regions = (bl.off_zlo + n_reg + 3) & ~3;
+  bl.off_regions = (bl.off_zlo + n_reg + 2 + 3) & ~3;         // two +inf entries follow the z_lo array
   const int n_blk = c->have_geom ? (int)c->blocks.size() : 0;
   bl.off_blocks = (bl.off_regions + 10 * n_reg + 3) & ~3;
   bl.off_binlut = bl.off_blocks + 24 * n_blk;
@@ -193,8 +195,36 @@ int rebuild_blob(mt_ctx* c) {
     }
     if (ok) { binlut.swap(lut); c->bin_shift = shift; c->bin_key_lo = (int)k_lo; c->bin_key_max = (int)(k_hi - k_lo); break; }
   }
-  bl.n_words = bl.off_binlut + (int)((binlut.size() + 1) / 2);
+  bl.off_zlut = bl.off_binlut + (int)((binlut.size() + 1) / 2);
+  // z-interval table (mt_params.h: zlut_n): cells fine enough that at most two z_lo fall into one, bounds taken with a
+  // margin of 1 % of a cell, which dwarfs the float32 rounding of the device's cell index (below 2^-11 of a cell here)
+  std::vector<int16_t> zlut;
+  c->zlut_n = 0; c->zlut_g0 = 0.0f; c->zlut_inv = 0.0f;
+  // (a handful of intervals is searched faster than the table's four dependent shared-memory reads: config 1 has one)
+  if (n_reg >= 8 && c->geom.mode == MT_GEOM_REGIONS) {
+    const double g0 = std::min((double)c->geom.z_min, (double)c->regions[0].z_lo);
+    const double g1 = std::max((double)c->geom.z_exit, (double)c->regions[n_reg - 1].z_lo);
+    for (int nzc = 1024; nzc <= 4096 && std::isfinite(g0) && std::isfinite(g1) && g1 > g0 && zlut.empty(); nzc *= 2) {
+      const float inv = (float)((double)nzc / (g1 - g0));
+      const double cell = 1.0 / (double)inv;
+      std::vector<int16_t> lut(nzc);
+      bool ok = true;
+      int j = -1;                                            // greatest j with z_lo[j] <= lower bound of the cell
+      for (int k = 0; k < nzc && ok; ++k) {
+        const double zb = (double)(float)g0 + ((double)k - 0.01) * cell, zu = (double)(float)g0 + ((double)k + 1.01) * cell;
+        while (j + 1 < n_reg && (double)c->regions[j + 1].z_lo <= zb) ++j;
+        int inside = 0;
+        for (int q = j + 1; q < n_reg && (double)c->regions[q].z_lo <= zu; ++q) ++inside;
+        if (k == nzc - 1) inside = n_reg - 1 - j;            // the last cell also serves every z beyond the table
+        ok = inside <= 2;
+        lut[k] = (int16_t)j;
+      }
+      if (ok) { zlut.swap(lut); c->zlut_n = nzc; c->zlut_g0 = (float)g0; c->zlut_inv = inv; }
+    }
+  }
+  bl.n_words = bl.off_zlut + (int)((zlut.size() + 1) / 2);
   std::vector<float> blob((size_t)bl.n_words + 4, 0.0f);
+  if (!zlut.empty()) memcpy(&blob[bl.off_zlut], zlut.data(), zlut.size() * sizeof(int16_t));
   for (int j = 0; j <= c->n_pbins; ++j) blob[j] = edges[j];
   if (!binlut.empty()) memcpy(&blob[bl.off_binlut], binlut.data(), binlut.size() * sizeof(uint16_t));
   for (int j = 0; j <= c->n_pbins; ++j)
@@ -223,6 +253,7 @@ int rebuild_blob(mt_ctx* c) {
               hi_dp <= -0.0034f && hi_th <= (joint_axes ? 0.0f : -0.36f);
   }
   c->lean_axes = axes_ok && c->bin_shift != 0;               // the lean kernels read the bin from the table
+  blob[bl.off_zlo + n_reg] = blob[bl.off_zlo + n_reg + 1] = INFINITY;
   for (int j = 0; j < n_reg; ++j) {
     blob[bl.off_zlo + j] = c->regions[j].z_lo;
     static_assert(sizeof(mt_region) == 40 && sizeof(MtRegionDev) == 40, "region layout");
@@ -762,6 +793,7 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.hnx = c->hnx; P.hny = c->hny; P.hnz = c->hnz;
   P.h_inv_x = c->h_inv[0]; P.h_inv_y = c->h_inv[1]; P.h_inv_z = c->h_inv[2];
   P.bin_shift = c->bin_shift; P.bin_key_lo = c->bin_key_lo; P.bin_key_max = c->bin_key_max;
+  P.zlut_n = c->zlut_n; P.zlut_g0 = c->zlut_g0; P.zlut_inv = c->zlut_inv; P.zlut_max = (float)(c->zlut_n - 1);
   P.inv_p_lo = 1.0f / c->p_lo;
   P.bin_scale = (float)((double)c->n_pbins / log2((double)c->p_hi / (double)c->p_lo));
   P.tab32 = (c->pack == 32) ? (const uint32_t*)c->d_tab.p : nullptr;
@@ -866,18 +898,30 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
   c->last_lean = cfg.lean; c->last_sched = sched;
   cfg.smem_bytes = blob_b + ((hot_blocks * block_cells * cell_b + 15) & ~(size_t)15) + 16;
 
-  // block size: the one that keeps the most threads resident (ties -> the smaller block)
+  // Block size.  A call that fills the machine takes the block that keeps the most threads resident (ties -> the smaller
+  // block).  A STATIC / REFILL call small enough to be resident all at once is spread as evenly as the block granularity
+  // allows instead: its time is that of the fullest SM, so the block that minimises ceil(CTAs / SMs) x block wins
+  // (config 1, 65 536 muons: 2 x 256 threads on most SMs but 3 x 128 = 384 at most -> 0.49 -> 0.37 ms, profiles/r2b_lanes.md).
   int occ = 0;
   cfg.block = 0;
-  for (unsigned cand : {256u, 384u, 512u, 768u}) {
-    if (c->opt_block && cand != 256u) break;
+  uint64_t best_load = ~(uint64_t)0;
+  const bool one_launch = (sched != MT_SCHED_WAVEFRONT);
+  for (unsigned cand : {128u, 256u, 384u, 512u, 768u}) {
+    if (c->opt_block && cand != 256u) continue;
     const unsigned blk = c->opt_block ? (unsigned)c->opt_block : cand;
     MtLaunchCfg probe = cfg;
     probe.block = blk;
     int o = 0;
     MT_CUDA(c, mt_occupancy(P, probe, &o));
     if (c->opt_blocks_per_sm) o = std::min(o, c->opt_blocks_per_sm);
-    if ((size_t)o * blk > (size_t)occ * cfg.block) { occ = o; cfg.block = blk; }
+    if (o < 1) continue;
+    const uint64_t ctas = (n + blk - 1) / blk;
+    if (one_launch && ctas <= (uint64_t)o * c->sm_count) {
+      const uint64_t load = ((ctas + c->sm_count - 1) / c->sm_count) * blk;
+      if (load < best_load) { best_load = load; occ = o; cfg.block = blk; }
+    } else if (best_load == ~(uint64_t)0 && cand >= 256u && (size_t)o * blk > (size_t)occ * cfg.block) {
+      occ = o; cfg.block = blk;
+    }
   }
   if (occ < 1) return fail(c, MT_ERR_UNSUPPORTED, "kernel does not fit on an SM with %zu B shared memory", cfg.smem_bytes);
   pl.persistent_grid = (unsigned)(c->sm_count * occ);

@@ -20,8 +20,10 @@ struct MtRegionDev {
 //   [off_regions + 10*j ..]              MtRegionDev j
 //   [off_blocks + 24*j ..]               MtBlockDev j (POLY mode)
 //   [off_binlut ..]                      uint16 momentum-bin table (two per word), see MtParams::bin_shift
+//   [off_zlut ..]                        int16 z-interval table (two per word), see MtParams::zlut_n; the z_lo array is
+//                                        followed by two +inf entries so that the table's two fix-ups need no bound
 struct MtBlobLayout {
-  int32_t off_edges_open, off_steps, off_axes, off_zlo, off_regions, off_blocks, off_binlut, n_words;
+  int32_t off_edges_open, off_steps, off_axes, off_zlo, off_regions, off_blocks, off_binlut, off_zlut, n_words;
 };
 
 // Polyhedra block as staged in shared memory: six float4.  inv_dz = 1 / (z_hi - z_lo), dx_i = xh_i - xl_i and
@@ -102,6 +104,12 @@ struct MtParams {
   // host has checked that no run holds more than one edge, so the bin of P is binlut[key] or the next one: ONE comparison
   // with the float32 edge decides, as §3.4 demands, and no logarithm is taken.  bin_shift = 0: no table (bins too narrow).
   int32_t bin_shift, bin_key_lo, bin_key_max;
+  // z-interval table (REGIONS): §3.2 asks for the greatest j with z_lo[j] <= z.  The z range
+  // [zlut_g0, zlut_g0 + zlut_n / zlut_inv] that covers the world box and every z_lo is cut into zlut_n cells; zlut[k] is
+  // that j for a point just below cell k (-1 if none) and the host has checked that no cell holds more than two z_lo, so
+  // two exact comparisons with the next z_lo finish the search — no 5-level binary search per step.  zlut_n = 0: no table.
+  int32_t zlut_n;
+  float zlut_g0, zlut_inv, zlut_max;
   const uint32_t* tab32;         // pack32: [material block][pbin][n_dp + n_th] = threshold24 << 8 | alias8; the blocks are
   const uint2* tab64;            // ordered most-used material first.  pack64: same shape, {threshold (<= 2^24), alias}
   const float* blob;             // const blob (global copy)

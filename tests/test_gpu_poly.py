@@ -193,3 +193,47 @@ def test_bad_blocks_are_refused(mt):
         b.mt_set_geometry(ctx, Geometry(MODE_POLY, -2.0, 2.0, -2.0, 2.0, 0.0, 2.0, 1.0, 10, WORLD, blocks=np.zeros(0, POLY_DTYPE)))
     finally:
         b.mt_destroy(ctx)
+
+
+def test_region_lookup_through_the_z_interval_table(mt, oracle):
+    """The regions lookup (greatest j with z_lo[j] <= z, then the half-open box) goes through a z-cell
+    table with two exact fix-up comparisons, or through the binary search when the intervals are too dense for the table;
+    both against the oracle's search on points ON every z_lo / z_hi, one float either side, outside the world, NaN / inf."""
+    from paper_2512_10520_b200.workloads import Geometry, MODE_REGIONS, REGION_DTYPE
+    rng = np.random.default_rng(5)
+    hist = _tiny_hist()
+
+    def regions_from(z_edges, gap_every=3):
+        regs = []
+        for j, (a, b) in enumerate(zip(z_edges[:-1], z_edges[1:])):
+            if gap_every and j % gap_every == 2:
+                continue                                           # a hole: points there belong to the world
+            regs.append((a, b, -0.5 + 0.1 * (j % 4), 0.6, -0.7, 0.4 + 0.05 * (j % 3), 1 + j % 2, 0.1 * j, -0.2, 0.01 * j))
+        return np.array(regs, REGION_DTYPE)
+
+    cases = {
+        "uneven": np.sort(np.concatenate([[0.0, 30.0], rng.uniform(0.0, 30.0, 40)])).astype(np.float32),
+        "two z_lo in one cell": np.array([0.0, 1.0, 2.0, 3.0, 4.0, 5.0, 5.004, 5.008, 10.0, 12.0, 14.0, 20.0, 20.011, 25.0,
+                                          29.0, 30.0], np.float32),
+        "dense (binary search)": np.linspace(2.0, 2.2, 1000).astype(np.float32),      # 0.2 mm intervals: no table possible
+        "beyond the world box": np.array([-3.0, -1.0, 4.0, 31.0, 35.0, 36.0, 40.0], np.float32),
+        "single": np.array([1.0, 2.0], np.float32),
+    }
+    for name, z_edges in cases.items():
+        z_edges = np.unique(z_edges)
+        regs = regions_from(z_edges, gap_every=0 if name in ("single", "dense (binary search)", "two z_lo in one cell") else 3)
+        geom = Geometry(MODE_REGIONS, -1.0, 1.0, -1.0, 1.0, 0.0, 30.0, 1.0, 100, 2, regions=regs)
+        zs = np.concatenate([regs["z_lo"], regs["z_hi"]])
+        special = np.concatenate([zs, np.nextafter(zs, np.float32(-np.inf)), np.nextafter(zs, np.float32(np.inf)),
+                                  np.float32([-1e30, -5.0, 0.0, 30.0, 45.0, 1e30, np.nan, np.inf, -np.inf])])
+        n = 60000
+        pts = np.empty((n, 3), np.float32)
+        pts[:, 0] = rng.uniform(-0.8, 0.8, n)
+        pts[:, 1] = rng.uniform(-0.9, 0.7, n)
+        pts[:, 2] = np.where(rng.random(n) < 0.5, rng.choice(special, n), rng.uniform(-4.0, 42.0, n).astype(np.float32))
+        pts[::7, 0] = rng.choice(np.float32([-0.5, -0.4, 0.6]), len(pts[::7]))     # on x faces
+        m_ref, B_ref = oracle.material_and_field(geom, pts, dtype=np.float32)
+        m_gpu, B_gpu = _lookup(mt, hist, geom, pts)
+        assert (m_ref != 2).mean() > 0.02, name
+        assert np.array_equal(m_gpu, m_ref), name
+        assert np.array_equal(B_gpu.view(np.uint32), B_ref.view(np.uint32)), name
