@@ -792,6 +792,7 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.hash_list = (const uint16_t*)((const char*)c->d_hash.p + c->hash_list_off);
   P.hnx = c->hnx; P.hny = c->hny; P.hnz = c->hnz;
   P.h_inv_x = c->h_inv[0]; P.h_inv_y = c->h_inv[1]; P.h_inv_z = c->h_inv[2];
+  P.h_max_x = (float)(c->hnx - 1); P.h_max_y = (float)(c->hny - 1); P.h_max_z = (float)(c->hnz - 1);
   P.bin_shift = c->bin_shift; P.bin_key_lo = c->bin_key_lo; P.bin_key_max = c->bin_key_max;
   P.zlut_n = c->zlut_n; P.zlut_g0 = c->zlut_g0; P.zlut_inv = c->zlut_inv; P.zlut_max = (float)(c->zlut_n - 1);
   P.inv_p_lo = 1.0f / c->p_lo;

@@ -128,6 +128,7 @@ struct MtParams {
   const uint16_t* hash_list;     // block indices
   int32_t hnx, hny, hnz;
   float h_inv_x, h_inv_y, h_inv_z;   // cells per metre along each axis
+  float h_max_x, h_max_y, h_max_z;   // (float)(hnx - 1), ...: the last cell along each axis
   // ---- this call
   uint64_t n, id_base;           // this lane's muons: n of them, the first with id id_base (= the call's id_base + idx_base)
   uint32_t idx_base;             // index of this lane's first muon within the call (exit records carry call indices)
