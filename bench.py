@@ -33,7 +33,7 @@ ALG_GATHER_BYTES_PER_STEP = {"voxel": 168, "regions": 40, "poly": 50}
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ALL launches of the dominant kernel in one 10^7-muon
 # batch of config 3, summed over the batch's z-slab passes from the ncu launch list profiles/r2_dram_launches.csv
 # (profiles/r2_summary.md has the command); None where no capture exists.  bench.py cannot run ncu itself.
-NCU_DRAM_BYTES_PER_BATCH = {"voxel": None, "regions": None, "poly": None}
+NCU_DRAM_BYTES_PER_BATCH = {"voxel": 29.19e9, "regions": None, "poly": None}     # 17.56 GB read + 11.63 GB written, 47 passes
 NCU_DRAM_SOURCE = "profiles/r2_dram_launches.csv"
 SM_COUNT, LANES_PER_SM = 148, 128          # B200: 4 SMSPs x 32 lanes issue one warp instruction per clock
 

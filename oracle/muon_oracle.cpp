@@ -34,7 +34,10 @@
 // exp2/sin/cos polynomials vs libm; two-word alias draw vs the exact pmf of the table; joint-mode kick vs its
 // geometry; nearest field vs the stored cell values; per-stage push vs h^4 convergence in a field gradient;
 // polyhedra containment vs scipy's convex hull of the eight vertices, the prismatoid volume, and the box regions;
-// exit projection vs the exact plane crossing of a straight line and the sagitta bound in a uniform field.  Physics fidelity vs Geant4 (Figs. 5, 7): parity unpinned
+// exit projection vs the exact plane crossing of a straight line and the sagitta bound in a uniform field; the break
+// tests of Algorithm 1 l.2-4 vs hand-worked literals for every bound, NaN and the priority order (test_oracle_breaks.py);
+// the whole loop vs its own libm witness (ELEM_LIBM below) at north_star's tolerance (test_oracle_witness.py).
+// Physics fidelity vs Geant4 (Figs. 5, 7): parity unpinned
 // (needs Geant4 histograms, not available).
 
 #include <cmath>
