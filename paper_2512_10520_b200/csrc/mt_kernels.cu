@@ -81,6 +81,16 @@ __global__ void __launch_bounds__(256) wave_perm_kernel(const __grid_constant__ 
   }
 }
 
+// item-mode passes add their tallies to MT_COUNTER_SLOTS spread copies (mt_kernels.cuh: Tally::flush); this folds them into
+// the caller's counters at the end of a lane's work and clears them for the next call
+__global__ void reduce_counters_kernel(unsigned long long* __restrict__ spread, unsigned long long* __restrict__ counters) {
+  const int c = threadIdx.x;
+  if (c >= 8) return;
+  unsigned long long sum = 0;
+  for (int k = 0; k < MT_COUNTER_SLOTS; ++k) { sum += spread[8 * k + c]; spread[8 * k + c] = 0ull; }
+  if (sum) atomicAdd(counters + c, sum);
+}
+
 // ---- voxel repack: {material u8, field f32x3} -> one 32-byte record {cell x, cell x+1 minus cell x} per cell of a grid with a
 // one-cell border that replicates the faces (so the clamped corner indices of DESIGN.md §3.3 need no clamps in
 // the step loop and an x-pair of corners is one load); also counts the cells of each material
@@ -214,6 +224,11 @@ cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, unsigned grid, cu
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   wave_perm_kernel<<<grid, 256, 0, stream>>>(P);
+  return cudaGetLastError();
+}
+
+cudaError_t mt_launch_reduce_counters(unsigned long long* spread, unsigned long long* counters, cudaStream_t stream) {
+  reduce_counters_kernel<<<1, 32, 0, stream>>>(spread, counters);
   return cudaGetLastError();
 }
 

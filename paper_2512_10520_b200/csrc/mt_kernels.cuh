@@ -29,13 +29,17 @@ extern __shared__ __align__(16) unsigned char mt_smem[];
 template <int PACK, bool TAB_SMEM>
 MT_DEV View<PACK> stage_view(const MtParams& P) {
   // const blob (edges, step lengths, axes, regions) -> shared memory, then the hot prefix of the packed tables
+  // (the per-table axes, by far the largest part, are NOT staged: one 128-bit read-only load per step serves them from
+  // L1, and a CTA then starts after copying ~1.5 KB instead of ~7 KB — what makes small CTAs and item-mode passes cheap)
   float* sblob = reinterpret_cast<float*>(mt_smem);
-  for (int i = threadIdx.x; i < P.bl.n_words; i += blockDim.x) sblob[i] = __ldg(P.blob + i);
+  for (int i = threadIdx.x; i < P.bl.n_words; i += blockDim.x)
+    if (!MT_AXES_GLOBAL || i < P.bl.off_axes || i >= P.bl.off_zlo) sblob[i] = __ldg(P.blob + i);
   View<PACK> V;
   V.edges = sblob;
   V.edges_open = sblob + P.bl.off_edges_open;
   V.steps = sblob + P.bl.off_steps;
-  V.axes = reinterpret_cast<const float4*>(sblob + P.bl.off_axes);
+  V.axes = MT_AXES_GLOBAL ? reinterpret_cast<const float4*>(P.blob + P.bl.off_axes)
+                          : reinterpret_cast<const float4*>(sblob + P.bl.off_axes);
   V.zlo = sblob + P.bl.off_zlo;
   V.regions = reinterpret_cast<const MtRegionDev*>(sblob + P.bl.off_regions);
   V.blocks = reinterpret_cast<const MtBlockDev*>(sblob + P.bl.off_blocks);
@@ -59,8 +63,11 @@ struct Tally {
   unsigned long long steps = 0;
   unsigned f1 = 0, f2 = 0, f3 = 0, f4 = 0;
   MT_DEV void count(int flag) { f1 += (flag == 1); f2 += (flag == 2); f3 += (flag == 3); f4 += (flag == 4); }
-  MT_DEV void flush(unsigned long long* counters, unsigned lane) {
+  // `spread`: slot of 8 counters to add to (item-mode kernels flush once per warp-item, hundreds of thousands of times
+  // per pass: the adds are spread over MT_COUNTER_SLOTS copies and summed by reduce_counters_kernel at the end of the call)
+  MT_DEV void flush(unsigned long long* counters, unsigned lane, unsigned spread = 0) {
     if (!counters) return;
+    counters += 8 * spread;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) steps += __shfl_xor_sync(kFull, steps, o);
     f1 = __reduce_add_sync(kFull, f1); f2 = __reduce_add_sync(kFull, f2);
@@ -201,17 +208,29 @@ MT_DEV uint32_t sort_key(const MtParams& P, float x, float y, float px, float py
 template <int GEOM, int PACK, bool TAB_SMEM, bool JOINT, int FIELD, bool LEAN = false>
 __global__ void __launch_bounds__(MT_MAX_THREADS, MT_MIN_BLOCKS)
 wave_transport_kernel(const __grid_constant__ MtParams P) {
+  const uint32_t n_items = *P.live_in_count;
+  // item mode (P.persistent == 0): warp w of CTA b owns the 32 muons from (b * warps + w) * 32 and the CTA exits when its
+  // warps are done, so that the CTAs of another lane's pass (or of this lane's sort) take the freed slots at once; the
+  // grid covers the lane's muon count, CTAs beyond the live count leave before staging anything
+  const unsigned warps_per_cta = blockDim.x >> 5;
+  if (!P.persistent && (uint64_t)blockIdx.x * warps_per_cta * 32u >= n_items) return;
   const View<PACK> V = stage_view<PACK, TAB_SMEM>(P);
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt_mask = (1u << lane) - 1u;
-  const uint32_t n_items = *P.live_in_count;
   Tally tally;
+  bool first = true;
 
   for (;;) {
     // ---- the warp takes the next 32 muons of the sorted list
     unsigned long long base = 0;
-    if (lane == 0) base = atomicAdd(P.work_counter, 32ull);
-    base = __shfl_sync(kFull, base, 0);
+    if (P.persistent) {
+      if (lane == 0) base = atomicAdd(P.work_counter, 32ull);
+      base = __shfl_sync(kFull, base, 0);
+    } else {
+      if (!first) break;
+      first = false;
+      base = ((unsigned long long)blockIdx.x * warps_per_cta + (threadIdx.x >> 5)) * 32ull;
+    }
     if (base >= n_items) break;
     const uint32_t item = (uint32_t)base + lane;
     Muon m;
@@ -278,7 +297,7 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
       }
     }
   }
-  tally.flush(P.counters, lane);
+  tally.flush(P.persistent ? P.counters : P.counters_spread, lane, P.persistent ? 0u : (blockIdx.x & (MT_COUNTER_SLOTS - 1)));
 }
 
 // Instantiated combinations: geometry x table kind {pack32, pack32 + shared prefix, pack64, pack64 + shared prefix,

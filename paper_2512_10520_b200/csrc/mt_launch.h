@@ -40,6 +40,8 @@ cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_
 // puts the parked records (P.sort_key) in sorted order (P.perm)
 cudaError_t mt_launch_wave_bin(const MtParams& P, unsigned grid, cudaStream_t stream);
 cudaError_t mt_launch_wave_sort(const MtParams& P, int n_keys, unsigned grid, cudaStream_t stream);
+// item-mode passes: spread tallies [MT_COUNTER_SLOTS][8] -> the caller's counters [8] (and cleared)
+cudaError_t mt_launch_reduce_counters(unsigned long long* spread, unsigned long long* counters, cudaStream_t stream);
 // d_material_cells: [256] counters (zeroed by the caller) of grid cells per material id
 cudaError_t mt_launch_repack(const uint8_t* mat, const float* fld, MtCellPair* out, int nx, int ny, int nz,
                              unsigned long long* d_material_cells, cudaStream_t stream);

@@ -33,7 +33,8 @@ struct DevBuf {
 
 // a lane of concurrent transport work inside one call (run_transport): own stream, own scratch
 struct Lane {
-  cudaStream_t stream = nullptr;
+  cudaStream_t stream = nullptr;                 // priority descending with the lane index
+  cudaStream_t stream_eq = nullptr;              // default priority: lanes that should advance side by side
   cudaEvent_t done = nullptr, ready = nullptr;   // its kernels (and copies out) are done / its inputs have landed
   DevBuf scratch, wave;
   size_t zero_bytes = 0;
@@ -81,7 +82,7 @@ struct mt_ctx {
   MtBlobLayout bl{};
   int64_t launches = 0;
   int last_lean = 0, last_sched = 0, last_lanes = 0;
-  int opt_lanes = 0;
+  int opt_lanes = 0, opt_pass_mode = 0, opt_lane_prio = 0;
   std::vector<Lane> lanes;
   cudaEvent_t ev_fork = nullptr;
   cudaStream_t copy_in = nullptr;
@@ -486,6 +487,7 @@ int mt_destroy(mt_ctx* c) {
   for (DevBuf* b : bufs) b->release();
   for (Lane& L : c->lanes) {
     if (L.stream) { cudaStreamSynchronize(L.stream); cudaStreamDestroy(L.stream); }
+    if (L.stream_eq) { cudaStreamSynchronize(L.stream_eq); cudaStreamDestroy(L.stream_eq); }
     if (L.done) cudaEventDestroy(L.done);
     if (L.ready) cudaEventDestroy(L.ready);
     L.scratch.release(); L.wave.release();
@@ -523,6 +525,12 @@ int mt_set_option(mt_ctx* c, int option, int64_t value) {
     case MT_OPT_CHECK_SELFTEST:
       if (!MT_CHECKED_BUILD) return fail(c, MT_ERR_UNSUPPORTED, "not a checked build");
       c->selftest_bad_bounds = value != 0; return MT_OK;
+    case MT_OPT_PASS_MODE:
+      if (value < 0 || value > 2) return fail(c, MT_ERR_INVALID_ARG, "bad pass mode");
+      c->opt_pass_mode = (int)value; return MT_OK;
+    case MT_OPT_LANE_PRIORITY:
+      if (value < 0 || value > 2) return fail(c, MT_ERR_INVALID_ARG, "bad lane priority mode");
+      c->opt_lane_prio = (int)value; return MT_OK;
     case MT_OPT_LANES:
       if (value < 0 || value > 16) return fail(c, MT_ERR_INVALID_ARG, "bad lane count");
       c->opt_lanes = (int)value; return MT_OK;
@@ -835,6 +843,7 @@ int ensure_lanes(mt_ctx* c, int K) {
     Lane L;
     const int prio = std::min(least, greatest + (int)c->lanes.size());
     MT_CUDA(c, cudaStreamCreateWithPriority(&L.stream, cudaStreamNonBlocking, prio));
+    MT_CUDA(c, cudaStreamCreateWithPriority(&L.stream_eq, cudaStreamNonBlocking, least));
     MT_CUDA(c, cudaEventCreateWithFlags(&L.done, cudaEventDisableTiming));
     MT_CUDA(c, cudaEventCreateWithFlags(&L.ready, cudaEventDisableTiming));
     c->lanes.push_back(L);
@@ -969,7 +978,7 @@ int choose_lanes(const mt_ctx* c, uint64_t n, int sched, bool host_call) {
   // Measured on config 3 and config 2 (profiles/r2b_lanes.md).  Host-buffer calls: four lanes on streams of descending
   // priority leave only the first lane's copy in and the last lane's copy out exposed (164.4 -> 159.7 ms per 10^7
   // muons); each further lane costs ~1.2 ms of pass start-up and tails.  Device calls: two lanes let one lane's
-  // passes fill the tails of the other's between 2^17 and 2^22 muons (+3 to +8 %); above that a single lane's passes
+  // passes fill the tails of the other's between 2^17 and 2^22 muons (+5 to +9 % with item-mode passes); above that a single lane's passes
   // are long enough that their tails do not matter (one lane is 1 % faster), below it there is nothing to overlap.
   // REFILL and STATIC kernels run a muon's whole history in one launch: lanes only serialise them.
   if (host_call && n >= ((uint64_t)1 << 21)) return 4;
@@ -993,6 +1002,19 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   rc = ensure_lanes(c, K);
   if (rc != MT_OK) return rc;
   c->last_lanes = K;
+  // WAVEFRONT pass mode (profiles/r2b_lanes.md).  Persistent CTAs pulling 32-muon items from a counter are the fastest way
+  // through one lane's pass (10^7 muons: 148.2 against 149.0 ms).  With two lanes of a device call, one item per warp and
+  // CTAs that exit with their items let the hardware interleave the lanes' CTAs, so each lane's tail and sort are filled
+  // by the other's pass: 2^18 muons 6.89 -> 6.31 ms, 2^20 muons 18.74 -> 17.84 ms; those lanes run on equal-priority
+  // streams (they should advance side by side).  Host-buffer calls keep persistent passes on streams of descending
+  // priority: there the point of the lanes is that they finish one after the other, each copying out under the next.
+  // 256-thread CTAs in both modes: smaller ones lose more to CTA start-up than they gain in granularity (64 threads: -6 %).
+  const bool item_mode = pl.sched == MT_SCHED_WAVEFRONT &&
+                         (c->opt_pass_mode == 2 || (c->opt_pass_mode == 0 && K > 1 && host == nullptr));
+  const bool equal_prio = c->opt_lane_prio == 2 || (c->opt_lane_prio == 0 && item_mode);
+  const unsigned item_block = c->opt_block ? (unsigned)c->opt_block : 256u;
+  if (item_mode) pl.cfg.block = item_block;
+  auto lane_stream = [&](int k) { return equal_prio ? c->lanes[k].stream_eq : c->lanes[k].stream; };
   const uint64_t chunk = (((n + K - 1) / K) + 31) & ~(uint64_t)31;
 
   // ---- per-lane parameters and scratch
@@ -1010,6 +1032,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
     P.out_pos_flag = (float4*)out->pos_flag + w.off; P.out_mom_steps = (float4*)out->mom_steps + w.off;
     if (w.n == 0) continue;
     w.grid = (unsigned)std::min<uint64_t>(pl.persistent_grid, (w.n + pl.cfg.block - 1) / pl.cfg.block);
+    if (item_mode) w.grid = (unsigned)((w.n + pl.cfg.block - 1) / pl.cfg.block);      // one muon per thread, 32 per warp-item
     if (pl.sched == MT_SCHED_STATIC) {
       w.grid = (unsigned)((w.n + pl.cfg.block - 1) / pl.cfg.block);
     } else if (pl.sched == MT_SCHED_REFILL) {
@@ -1017,10 +1040,14 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
       P.work_counter = (unsigned long long*)L.scratch.p;
     } else {
       // scratch: [n_pass + 1] work counters (u64), [n_pass + 1] live counts (u32), histogram and offsets [n_keys] (u32)
-      const size_t off_counts = (size_t)(n_pass + 1) * 8, off_hist = (off_counts + (size_t)(n_pass + 1) * 4 + 255) & ~(size_t)255;
+      // (item mode: MT_COUNTER_SLOTS x 8 spread tallies in front)
+      const size_t off_work = (size_t)MT_COUNTER_SLOTS * 64;
+      const size_t off_counts = off_work + (size_t)(n_pass + 1) * 8, off_hist = (off_counts + (size_t)(n_pass + 1) * 4 + 255) & ~(size_t)255;
       const size_t zero_b = off_hist + (size_t)n_keys * 4, scratch_b = zero_b + (size_t)n_keys * 4;
       MT_CUDA(c, L.scratch.reserve(std::max<size_t>(scratch_b, 4096)));
-      w.work = (unsigned long long*)L.scratch.p;
+      P.counters_spread = P.counters ? (unsigned long long*)L.scratch.p : nullptr;
+      P.persistent = item_mode ? 0 : 1;
+      w.work = (unsigned long long*)((char*)L.scratch.p + off_work);
       w.counts = (uint32_t*)((char*)L.scratch.p + off_counts);
       P.hist = (uint32_t*)((char*)L.scratch.p + off_hist);
       P.key_offset = P.hist + n_keys;
@@ -1044,14 +1071,15 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   for (int k = 0; k < K; ++k) {
     if (W[k].n == 0) continue;
     Lane& L = c->lanes[k];
-    MT_CUDA(c, cudaStreamWaitEvent(L.stream, c->ev_fork, 0));
+    cudaStream_t LS = lane_stream(k);
+    MT_CUDA(c, cudaStreamWaitEvent(LS, c->ev_fork, 0));
     if (host) {
       // inputs arrive lane by lane on ONE stream (in order, each at full link bandwidth); a lane starts when its own have landed
       const size_t b = (size_t)W[k].n * 16, o = (size_t)W[k].off * 4;
       MT_CUDA(c, cudaMemcpyAsync((float*)in->pos_q + o, host->pos_q + o, b, cudaMemcpyHostToDevice, c->copy_in));
       MT_CUDA(c, cudaMemcpyAsync((float*)in->mom + o, host->mom + o, b, cudaMemcpyHostToDevice, c->copy_in));
       MT_CUDA(c, cudaEventRecord(L.ready, c->copy_in));
-      MT_CUDA(c, cudaStreamWaitEvent(L.stream, L.ready, 0));
+      MT_CUDA(c, cudaStreamWaitEvent(LS, L.ready, 0));
     }
   }
 
@@ -1060,20 +1088,21 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
     LaneWork& w = W[k];
     if (w.n == 0) continue;
     Lane& L = c->lanes[k];
+    cudaStream_t LS = lane_stream(k);
     MtLaunchCfg cfg = pl.cfg;
     cfg.grid = w.grid;
     if (pl.sched == MT_SCHED_STATIC) {
-      MT_CUDA(c, mt_launch_transport(w.P, cfg, L.stream));
+      MT_CUDA(c, mt_launch_transport(w.P, cfg, LS));
       c->launches += 1;
     } else if (pl.sched == MT_SCHED_REFILL) {
-      MT_CUDA(c, cudaMemsetAsync(L.scratch.p, 0, 8, L.stream));
-      MT_CUDA(c, mt_launch_transport(w.P, cfg, L.stream));
+      MT_CUDA(c, cudaMemsetAsync(L.scratch.p, 0, 8, LS));
+      MT_CUDA(c, mt_launch_transport(w.P, cfg, LS));
       c->launches += 1;
     } else {
-      MT_CUDA(c, cudaMemsetAsync(L.scratch.p, 0, L.zero_bytes, L.stream));
+      MT_CUDA(c, cudaMemsetAsync(L.scratch.p, 0, L.zero_bytes, LS));
       w.P.live_out_count = w.counts;                             // counts[s] = muons entering pass s
-      MT_CUDA(c, mt_launch_wave_bin(w.P, w.aux_grid, L.stream));
-      MT_CUDA(c, mt_launch_wave_sort(w.P, n_keys, w.aux_grid, L.stream));
+      MT_CUDA(c, mt_launch_wave_bin(w.P, w.aux_grid, LS));
+      MT_CUDA(c, mt_launch_wave_sort(w.P, n_keys, w.aux_grid, LS));
       c->launches += 3;
     }
   }
@@ -1082,7 +1111,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
       for (int k = 0; k < K; ++k) {
         LaneWork& w = W[k];
         if (w.n == 0) continue;
-        Lane& L = c->lanes[k];
+        cudaStream_t LS = lane_stream(k);
         MtLaunchCfg cfg = pl.cfg;
         cfg.grid = w.grid;
         MtParams& P = w.P;
@@ -1094,11 +1123,14 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
         P.rec_out = w.rec[s & 1];
         P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * pl.slab);
         P.lean_z_hi = std::min(c->lean_box[5], P.slab_z_end);
-        MT_CUDA(c, mt_launch_transport(P, cfg, L.stream));
+        MT_CUDA(c, mt_launch_transport(P, cfg, LS));
         c->launches += 1;
         if (s < n_pass - 1) {
-          MT_CUDA(c, mt_launch_wave_sort(P, n_keys, w.aux_grid, L.stream));
+          MT_CUDA(c, mt_launch_wave_sort(P, n_keys, w.aux_grid, LS));
           c->launches += 2;
+        } else if (item_mode && P.counters) {
+          MT_CUDA(c, mt_launch_reduce_counters(P.counters_spread, P.counters, LS));
+          c->launches += 1;
         }
       }
     }
@@ -1108,12 +1140,13 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   for (int k = 0; k < K; ++k) {
     if (W[k].n == 0) continue;
     Lane& L = c->lanes[k];
+    cudaStream_t LS = lane_stream(k);
     if (host) {
       const size_t b = (size_t)W[k].n * 16, o = (size_t)W[k].off * 4;
-      MT_CUDA(c, cudaMemcpyAsync(host->pos_flag + o, out->pos_flag + o, b, cudaMemcpyDeviceToHost, L.stream));
-      MT_CUDA(c, cudaMemcpyAsync(host->mom_steps + o, out->mom_steps + o, b, cudaMemcpyDeviceToHost, L.stream));
+      MT_CUDA(c, cudaMemcpyAsync(host->pos_flag + o, out->pos_flag + o, b, cudaMemcpyDeviceToHost, LS));
+      MT_CUDA(c, cudaMemcpyAsync(host->mom_steps + o, out->mom_steps + o, b, cudaMemcpyDeviceToHost, LS));
     }
-    MT_CUDA(c, cudaEventRecord(L.done, L.stream));
+    MT_CUDA(c, cudaEventRecord(L.done, LS));
     MT_CUDA(c, cudaStreamWaitEvent(stream, L.done, 0));
   }
   return MT_OK;

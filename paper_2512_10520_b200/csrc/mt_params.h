@@ -74,6 +74,8 @@ enum {
 #define MT_CHECKED_BUILD 0
 #endif
 
+#define MT_COUNTER_SLOTS 64
+
 struct MtParams {
   // ---- checked build: {violations, highest MT_CHK_* code seen}, and the sizes the indices are held to
   unsigned* check;
@@ -142,6 +144,9 @@ struct MtParams {
   uint32_t* exit_count;
   uint32_t exit_capacity;
   unsigned long long* counters;  // optional [8]
+  unsigned long long* counters_spread;  // item-mode kernels: [MT_COUNTER_SLOTS][8] library scratch summed into `counters`
+  int32_t persistent;            // WAVEFRONT passes: 1 = persistent CTAs that pull 32-muon items from work_counter; 0 = one
+                                 // item per warp, the CTA exits with its items (lanes interleave at CTA granularity)
   unsigned long long* work_counter;   // refill scheduler
   int32_t refill_min_idle;
   // ---- wavefront scheduler (mt_kernels.cu): one pass per z-slab.  In-flight muons live in library
