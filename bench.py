@@ -263,7 +263,7 @@ def run_ours(args, rank, world, local_rank):
     h.set_option(b.MT_OPT_SCHEDULE, args.sched).set_option(b.MT_OPT_BLOCK_THREADS, args.block)
     h.set_option(b.MT_OPT_SLAB_CELLS, args.slab).set_option(b.MT_OPT_REFILL_MIN_IDLE, args.min_idle)
     h.set_option(b.MT_OPT_BLOCKS_PER_SM, args.blocks_per_sm).set_option(b.MT_OPT_NO_LEAN, int(args.no_lean))
-    h.set_option(b.MT_OPT_LANES, args.lanes)
+    h.set_option(b.MT_OPT_LANES, args.lanes).set_option(b.MT_OPT_PASS_MODE, args.pass_mode)
     host_geom = None
     if rank == 0 and not args.no_cpu_baseline:
         import copy
@@ -503,11 +503,13 @@ def run_sweep_lanes(args):
     for n in sorted({min(1 << 18, args.muons), min(1 << 20, args.muons), min(1 << 22, args.muons), args.muons}):
         o = {k: v[:n] for k, v in out.items()}
         for slab in (0, 64, 128, 256):
-            for lanes in (0, 1, 2, 4):
-                h.set_option(b.MT_OPT_LANES, lanes).set_option(b.MT_OPT_SLAB_CELLS, slab)
+            for lanes, mode in ((0, 0), (1, 1), (1, 2), (2, 1), (2, 2), (4, 1), (4, 2)):
+                h.set_option(b.MT_OPT_LANES, lanes).set_option(b.MT_OPT_SLAB_CELLS, slab).set_option(b.MT_OPT_PASS_MODE, mode)
                 ms, st = timed(h, dq[:n], dm[:n], o)
                 emit(ALG_OPS_PER_STEP["voxel"], ms, st, workload="config3", call="device", muons=n, slab_cells=slab,
-                     lanes=lanes or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES))
+                     lanes=lanes or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES),
+                     passes={0: "auto", 1: "persistent", 2: "item"}[mode])
+        h.set_option(b.MT_OPT_PASS_MODE, 0)
     hq, hm = torch.from_numpy(mu.pos_q).pin_memory(), torch.from_numpy(mu.mom).pin_memory()
     hout = {"pos_flag": torch.empty((len(hq), 4)).pin_memory(), "mom_steps": torch.empty((len(hq), 4)).pin_memory()}
     h.set_option(b.MT_OPT_SLAB_CELLS, 0)
@@ -590,6 +592,7 @@ def main():
     ap.add_argument("--slab", type=int, default=0)
     ap.add_argument("--min-idle", type=int, default=0)
     ap.add_argument("--lanes", type=int, default=0, help="MT_OPT_LANES: concurrent lanes per call (0 = library default)")
+    ap.add_argument("--pass-mode", type=int, default=0, help="MT_OPT_PASS_MODE: 1 persistent CTAs, 2 one item per warp (0 = default)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-seconds", type=float, default=15.0, help="CPU work per oracle sample")
     ap.add_argument("--ref-threads", type=int, default=0, help="--impl reference: oracle threads (0 = all host cores)")

@@ -98,6 +98,7 @@ enum {
   MT_OPT_PASS_MODE = 12,     /* WAVEFRONT passes: 1 = persistent CTAs pulling 32-muon items from a counter; 2 = one  */
                              /* item per warp, CTAs exit with their items (lanes interleave); 0 = default          */
   MT_OPT_LANE_PRIORITY = 13, /* lane streams: 1 = priorities descending with the lane index; 2 = equal; 0 = default  */
+  MT_OPT_SORT_EVERY = 14,    /* WAVEFRONT: the live list is re-sorted by xy cell after every k-th pass; 0 = default (1) */
   MT_OPT_CHECK_SELFTEST = 11 /* checked build only (MT_INFO_CHECK_ERRORS): 1 hands the kernels a wrong table size */
                              /* so that the bounds checks must fire; MT_ERR_UNSUPPORTED in the normal build     */
 };

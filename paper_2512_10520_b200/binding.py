@@ -19,7 +19,7 @@ MT_PLACE_AUTO, MT_PLACE_SMEM, MT_PLACE_L2 = 0, 1, 2
 MT_SCHED_AUTO, MT_SCHED_STATIC, MT_SCHED_REFILL, MT_SCHED_WAVEFRONT = 0, 1, 2, 3
 MT_OPT_SCHEDULE, MT_OPT_BLOCK_THREADS, MT_OPT_BLOCKS_PER_SM, MT_OPT_SLAB_CELLS, MT_OPT_REFILL_MIN_IDLE = 1, 2, 3, 4, 5
 MT_OPT_KEY_LOOKAHEAD, MT_OPT_HASH_NXY, MT_OPT_HASH_NZ, MT_OPT_NO_LEAN, MT_OPT_LANES, MT_OPT_CHECK_SELFTEST = 6, 7, 8, 9, 10, 11
-MT_OPT_PASS_MODE, MT_OPT_LANE_PRIORITY = 12, 13
+MT_OPT_PASS_MODE, MT_OPT_LANE_PRIORITY, MT_OPT_SORT_EVERY = 12, 13, 14
 MT_HIST_MARGINAL, MT_HIST_JOINT = 0, 1
 MT_EXIT_AT_BREAK, MT_EXIT_PROJECT = 0, 1
 MT_INFO_LEAN_FACTS, MT_INFO_LAST_LEAN, MT_INFO_LAST_SCHEDULE, MT_INFO_LAST_LANES, MT_INFO_CHECK_ERRORS = 1, 2, 3, 4, 5

@@ -240,7 +240,7 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
     m.step = 0;
     if (item < n_items) {
       MT_CHECK(P, item < P.n, MT_CHK_PERM);
-      const uint32_t rec = P.perm[item];
+      const uint32_t rec = P.sorted_in ? P.perm[item] : item;      // unsorted pass: the records in the order they were parked
       MT_CHECK(P, rec < (P.first_pass ? P.n : (uint64_t)n_items), MT_CHK_RECORD);
       float4 a, b;
       if (P.first_pass) {
@@ -280,20 +280,22 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
       if ((int)lane == leader) slot0 = atomicAdd(P.live_out_count, (unsigned)__popc(pm));
       slot0 = __shfl_sync(kFull, slot0, leader);
       if (parked) {
-        const uint32_t key = sort_key(P, m.x, m.y, m.px, m.py, m.pz);
-        const unsigned peers = __match_any_sync(pm, key);
-        const int pl = __ffs(peers) - 1;
-        unsigned r0 = 0;
-        if ((int)lane == pl) r0 = atomicAdd(P.hist + key, (unsigned)__popc(peers));
-        r0 = __shfl_sync(peers, r0, pl);
         const unsigned slot = slot0 + (unsigned)__popc(pm & lt_mask);
         MT_CHECK(P, slot < P.n, MT_CHK_PARK_SLOT);
-        MT_CHECK(P, key < P.n_keys, MT_CHK_SORT_KEY);
         float4* r = P.rec_out + 3 * (size_t)slot;                       // a warp's records are contiguous: full sectors
         r[0] = make_float4(m.x, m.y, m.z, m.q);
         r[1] = make_float4(m.px, m.py, m.pz, __int_as_float(m.step));
         r[2] = make_float4(__uint_as_float(idx), 0.0f, 0.0f, 0.0f);
-        P.sort_key[slot] = make_uint2(key, r0 + (unsigned)__popc(peers & lt_mask));
+        if (P.sort_out) {                                               // the next pass reads them sorted: key and rank
+          const uint32_t key = sort_key(P, m.x, m.y, m.px, m.py, m.pz);
+          MT_CHECK(P, key < P.n_keys, MT_CHK_SORT_KEY);
+          const unsigned peers = __match_any_sync(pm, key);
+          const int pl = __ffs(peers) - 1;
+          unsigned r0 = 0;
+          if ((int)lane == pl) r0 = atomicAdd(P.hist + key, (unsigned)__popc(peers));
+          r0 = __shfl_sync(peers, r0, pl);
+          P.sort_key[slot] = make_uint2(key, r0 + (unsigned)__popc(peers & lt_mask));
+        }
       }
     }
   }

@@ -82,7 +82,7 @@ struct mt_ctx {
   MtBlobLayout bl{};
   int64_t launches = 0;
   int last_lean = 0, last_sched = 0, last_lanes = 0;
-  int opt_lanes = 0, opt_pass_mode = 0, opt_lane_prio = 0;
+  int opt_lanes = 0, opt_pass_mode = 0, opt_lane_prio = 0, opt_sort_every = 0;
   std::vector<Lane> lanes;
   cudaEvent_t ev_fork = nullptr;
   cudaStream_t copy_in = nullptr;
@@ -531,6 +531,9 @@ int mt_set_option(mt_ctx* c, int option, int64_t value) {
     case MT_OPT_LANE_PRIORITY:
       if (value < 0 || value > 2) return fail(c, MT_ERR_INVALID_ARG, "bad lane priority mode");
       c->opt_lane_prio = (int)value; return MT_OK;
+    case MT_OPT_SORT_EVERY:
+      if (value < 0 || value > 64) return fail(c, MT_ERR_INVALID_ARG, "bad sort interval");
+      c->opt_sort_every = (int)value; return MT_OK;
     case MT_OPT_LANES:
       if (value < 0 || value > 16) return fail(c, MT_ERR_INVALID_ARG, "bad lane count");
       c->opt_lanes = (int)value; return MT_OK;
@@ -1119,13 +1122,17 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
         P.live_out_count = w.counts + s + 1;
         P.work_counter = w.work + s;
         P.first_pass = (s == 0);
+        // the live list is sorted before pass 0 and after every sort_every-th pass
+        const int sort_every = c->opt_sort_every > 0 ? c->opt_sort_every : 1;
+        P.sorted_in = (s % sort_every) == 0;
+        P.sort_out = (s < n_pass - 1) && ((s + 1) % sort_every) == 0;
         P.rec_in = w.rec[(s + 1) & 1];
         P.rec_out = w.rec[s & 1];
         P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * pl.slab);
         P.lean_z_hi = std::min(c->lean_box[5], P.slab_z_end);
         MT_CUDA(c, mt_launch_transport(P, cfg, LS));
         c->launches += 1;
-        if (s < n_pass - 1) {
+        if (P.sort_out) {
           MT_CUDA(c, mt_launch_wave_sort(P, n_keys, w.aux_grid, LS));
           c->launches += 2;
         } else if (item_mode && P.counters) {

@@ -157,6 +157,9 @@ struct MtParams {
   uint32_t* live_out_count;      // device count of the records it parks (zero on entry)
   float slab_z_end;              // a pass advances each muon until z >= slab_z_end (or it terminates)
   int32_t first_pass;            // 1: the records are the caller's input arrays (step 0, index = position)
+  int32_t sorted_in, sort_out;   // this pass reads its records through `perm` / parks them with sort keys for the next sort
+                                 // (the live list is re-sorted every MT_OPT_SORT_EVERY-th pass; in between, a pass reads
+                                 // the records in the order in which the previous one parked them)
   const float4* rec_in;          // [live][3]
   float4* rec_out;               // [parked][3]
   uint2* sort_key;               // [parked] {sort key, rank within key} of the records just parked / of the inputs

@@ -3,7 +3,7 @@ import numpy as np
 
 
 def gpu_transport(mt, wl, sched=0, block=0, placement=0, id_base=0, exit_capacity=0, min_idle=0, slab=0,
-                  sel=None, handle=None, lanes=0, pass_mode=0, lane_prio=0):
+                  sel=None, handle=None, lanes=0, pass_mode=0, lane_prio=0, sort_every=0):
     """Run workload `wl` on cuda:0 through the binding; returns numpy dict (pos, mom, flag, steps, ...)."""
     import torch
     b = mt.binding
@@ -13,6 +13,7 @@ def gpu_transport(mt, wl, sched=0, block=0, placement=0, id_base=0, exit_capacit
         h.set_option(b.MT_OPT_SCHEDULE, sched).set_option(b.MT_OPT_BLOCK_THREADS, block)
         h.set_option(b.MT_OPT_REFILL_MIN_IDLE, min_idle).set_option(b.MT_OPT_SLAB_CELLS, slab)
         h.set_option(b.MT_OPT_LANES, lanes).set_option(b.MT_OPT_PASS_MODE, pass_mode).set_option(b.MT_OPT_LANE_PRIORITY, lane_prio)
+        h.set_option(b.MT_OPT_SORT_EVERY, sort_every)
         pos_q, mom = wl.muons.pos_q, wl.muons.mom
         if sel is not None:
             pos_q, mom = pos_q[sel], mom[sel]

@@ -32,7 +32,9 @@ def test_results_do_not_depend_on_launch_shape(mt, wl1, ref1):
                dict(sched=3, lanes=2), dict(sched=3, lanes=7, slab=30), dict(sched=2, lanes=3), dict(sched=1, lanes=16),
                # WAVEFRONT pass modes: persistent CTAs / one item per warp, with either lane-priority scheme and odd blocks
                dict(sched=3, lanes=1, pass_mode=2), dict(sched=3, lanes=3, pass_mode=2, block=96, lane_prio=1),
-               dict(sched=3, lanes=4, pass_mode=1, lane_prio=2), dict(sched=3, lanes=5, pass_mode=2, block=32, slab=17)):
+               dict(sched=3, lanes=4, pass_mode=1, lane_prio=2), dict(sched=3, lanes=5, pass_mode=2, block=32, slab=17),
+               # the live list re-sorted only after every k-th pass
+               dict(sched=3, slab=20, sort_every=2), dict(sched=3, slab=7, sort_every=5, lanes=2), dict(sched=3, slab=20, sort_every=64)):
         assert _same(gpu_transport(mt, wl1, **kw), base), kw
 
 
