@@ -102,7 +102,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ roofline
-def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_muons, peaks, mp):
+def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_muons, grid_bytes, peaks, mp):
     """north_star's roofline for one step of this rank: "the larger of FP32-issue time ... at peak and gather bytes at
     L2/HBM bandwidth", with both terms, against peaks MEASURED in this process (mt_measure_peaks: csrc/mt_probe.cu) and
     the nominal issue peak beside them.  DESIGN.md §7 derives the per-muon-step figures."""
@@ -115,7 +115,8 @@ def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_m
     t_issue, t_issue_nominal = ops / measured, ops / nominal
     t_gather = {"l1_resident_64k": gbytes / mp["gather_l1_bytes_per_s"], "l2_resident_64m": gbytes / mp["gather_64m_bytes_per_s"],
                 "hbm_1400m": gbytes / mp["gather_1400m_bytes_per_s"]}
-    state_bytes = 64 * n_muons                                             # 32 B in + 32 B out per muon: the only compulsory HBM traffic
+    # compulsory HBM traffic: 32 B in + 32 B out per muon, and the part of the field grid the batch touches, once
+    state_bytes = 64 * n_muons + grid_bytes
     dram = NCU_DRAM_BYTES_PER_BATCH[mode]
     return {
         "bound": "alu", "unit": "T thread-ops/s",
@@ -148,6 +149,7 @@ def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_m
         "traffic_unit": "DRAM bytes per launch of the kernel = per-batch total / passes (ncu, %s)" % NCU_DRAM_SOURCE,
         "traffic_per_batch": dram,
         "algorithmic_hbm_bytes_per_batch": state_bytes,
+        "algorithmic_hbm_bytes_note": "64 B of state per muon + the library's 32-byte-per-cell field grid read once",
         "traffic_over_algorithmic": (dram / state_bytes) if dram else None,
     }
 
@@ -259,11 +261,13 @@ def run_ours(args, rank, world, local_rank):
     n, id_base = shard.n, shard.id_base
     wl = make_workload(args.config, n, dev, rank, args.joint, args.field_mode, args.poly, args.draws)
     mode = {0: "regions", 1: "voxel", 2: "poly"}[wl.geom.mode]
+    grid_bytes = 32 * (wl.geom.nx + 2) * (wl.geom.ny + 2) * (wl.geom.nz + 2) if mode == "voxel" else 0
     h = b.MuonTransport(local_rank).setup(wl.hist, wl.geom, args.placement)
     h.set_option(b.MT_OPT_SCHEDULE, args.sched).set_option(b.MT_OPT_BLOCK_THREADS, args.block)
     h.set_option(b.MT_OPT_SLAB_CELLS, args.slab).set_option(b.MT_OPT_REFILL_MIN_IDLE, args.min_idle)
     h.set_option(b.MT_OPT_BLOCKS_PER_SM, args.blocks_per_sm).set_option(b.MT_OPT_NO_LEAN, int(args.no_lean))
     h.set_option(b.MT_OPT_LANES, args.lanes).set_option(b.MT_OPT_PASS_MODE, args.pass_mode)
+    h.set_option(b.MT_OPT_SORT_EVERY, args.sort_every)
     host_geom = None
     if rank == 0 and not args.no_cpu_baseline:
         import copy
@@ -342,7 +346,7 @@ def run_ours(args, rank, world, local_rank):
     value = steps_all * args.steps / t_dev_max
     e2e_value = steps_all * e2e_steps / t_e2e_max
     roofline = roofline_block(mode, steps_per_call, t_dev / args.steps, max(1, launches // args.steps), lanes_used, n,
-                              peaks, b.mt_measure_peaks(local_rank))
+                              grid_bytes, peaks, b.mt_measure_peaks(local_rank))
     line = {
         "metric": "muon_steps_per_s", "value": value, "unit": "muon-steps/s",
         "muons_per_s": muons_all * args.steps / t_dev_max,
@@ -592,6 +596,7 @@ def main():
     ap.add_argument("--slab", type=int, default=0)
     ap.add_argument("--min-idle", type=int, default=0)
     ap.add_argument("--lanes", type=int, default=0, help="MT_OPT_LANES: concurrent lanes per call (0 = library default)")
+    ap.add_argument("--sort-every", type=int, default=0, help="MT_OPT_SORT_EVERY: re-sort the live list after every k-th pass")
     ap.add_argument("--pass-mode", type=int, default=0, help="MT_OPT_PASS_MODE: 1 persistent CTAs, 2 one item per warp (0 = default)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-seconds", type=float, default=15.0, help="CPU work per oracle sample")

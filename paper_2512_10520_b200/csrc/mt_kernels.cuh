@@ -169,7 +169,8 @@ transport_kernel(const __grid_constant__ MtParams P) {
       continue;
     }
 
-    // ---- a few steps for every active lane; the loop itself stays warp-uniform
+    // ---- a few steps for every active lane; the loop itself stays warp-uniform.  Nothing but the step happens on a step
+    // in which no lane of the warp terminates (one vote tells).
 #pragma unroll 1
     for (int k = 0; k < kInnerSteps; ++k) {
       int flag = 0;
@@ -178,12 +179,14 @@ transport_kernel(const __grid_constant__ MtParams P) {
         flag = step_once<GEOM, PACK, TAB_SMEM, false, JOINT, FIELD, true, LEAN>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
         if (flag == 0) tally.steps += 1;
       }
-      write_final(P, m, idx, flag, lane);
-      if (flag) {
-        tally.count(flag);
-        active = false;
+      if (__any_sync(kFull, flag != 0)) {
+        write_final(P, m, idx, flag, lane);
+        if (flag) {
+          tally.count(flag);
+          active = false;
+        }
+        if (!__any_sync(kFull, active)) break;
       }
-      if (!__any_sync(kFull, active)) break;
     }
     if (SCHED == SCHED_STATIC && !__any_sync(kFull, active)) break;
   }

@@ -878,10 +878,8 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
   P.refill_min_idle = c->opt_min_idle ? c->opt_min_idle : 1;
 
   // Table placement (north_star subsystem 1).  The packed tables start with the most-used material; shared
-  // memory takes the longest prefix of whole material blocks that fits.  AUTO stages everything when that still
-  // leaves room for two CTAs per SM and otherwise nothing: on config 3 a shared-memory copy of the iron tables
-  // (154 KB, one 768-thread CTA per SM) measured 2 % slower than L1/L2 gathers (profiles/r1c_summary.md).
-  // MT_PLACE_SMEM stages as many materials as fit.
+  // memory takes the longest prefix of whole material blocks that fits.  MT_PLACE_SMEM stages as many materials as fit;
+  // AUTO: see below.
   MtLaunchCfg& cfg = pl.cfg;
   cfg.pack = c->pack;
   cfg.sched = sched;
@@ -901,7 +899,15 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
     if (fit_blocks == 0) return fail(c, MT_ERR_UNSUPPORTED, "no material's tables (%zu B) fit in shared memory", block_cells * cell_b);
     hot_blocks = fit_blocks;
   } else if (c->placement == MT_PLACE_AUTO) {
-    if ((blob_b + c->table_bytes + 16) * 2 <= smem_budget) hot_blocks = c->n_materials;
+    // Stage when EVERY material's tables fit in one CTA's shared memory and the call is large enough to amortise the copy
+    // each CTA makes: config 4's 50x128x64 shape (115 KB, one 768-thread CTA per SM) 0.769 staged against 0.735 from L2;
+    // a partial prefix loses (100x256x128, iron only: 0.688 against 0.730), and so does staging for a small call
+    // (config 1, 65 536 muons, 38 KB per CTA: 0.397 against 0.382 ms from L2) — profiles/r2_config4_sweep.md
+    if (blob_b + c->table_bytes + 16 <= smem_budget && n >= ((uint64_t)1 << 20)) hot_blocks = c->n_materials;
+    // ... unless staging would cost the lean kernel variant (they exist for fewer staged combinations, mt_has_lean)
+    MtLaunchCfg staged = cfg, gathered = cfg;
+    staged.tab_smem = true; gathered.tab_smem = false;
+    if (hot_blocks && !mt_has_lean(c->geom.mode, staged) && mt_has_lean(c->geom.mode, gathered)) hot_blocks = 0;
   }
   P.hot_cells = (uint32_t)(hot_blocks * block_cells);
   cfg.tab_smem = hot_blocks > 0;

@@ -36,7 +36,7 @@ def _worker(rank, world, port, out_dir):
     import torch.distributed as dist
     import oracle
     from paper_2512_10520_b200 import workloads as w
-    from paper_2512_10520_b200.sharding import reduce_job, strong_shard
+    from paper_2512_10520_b200.sharding import gather_ranges, reduce_job, strong_shard
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
@@ -47,7 +47,7 @@ def _worker(rank, world, port, out_dir):
                              wl.muons.mom[sel], wl.seed, id_base=sh.id_base, threads=1)
         times, totals = reduce_job([0.5 + rank, 2.0 - rank], [int(r["steps"].sum()), sh.n], dist)
         np.savez(os.path.join(out_dir, "rank%d.npz" % rank), pos=r["pos"], mom=r["mom"], flag=r["flag"],
-                 steps=r["steps"], id_base=sh.id_base, times=times, totals=totals)
+                 steps=r["steps"], id_base=sh.id_base, times=times, totals=totals, ranges=gather_ranges(sh, dist))
     finally:
         dist.destroy_process_group()
 
@@ -62,6 +62,8 @@ def test_two_rank_gloo_job_equals_the_unsharded_one(tmp_path, oracle, workloads)
     assert [int(p["id_base"]) for p in parts] == [0, 1001]
     for k in ("pos", "mom", "flag", "steps"):
         assert np.array_equal(np.concatenate([p[k] for p in parts]), ref[k])
+    for p in parts:                                   # every rank sees the id ranges all ranks report: disjoint, covering
+        assert p["ranges"].tolist() == [[0, 1001], [1001, 2001]]
     for p in parts:                                   # every rank holds the same whole-job figures
         assert list(p["times"]) == [1.5, 2.0]        # max over ranks
         assert list(p["totals"]) == [float(ref["steps"].sum()), 2001.0]
