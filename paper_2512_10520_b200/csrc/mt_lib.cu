@@ -984,9 +984,10 @@ struct HostIO {
 
 int choose_lanes(const mt_ctx* c, uint64_t n, int sched, bool host_call) {
   if (c->opt_lanes > 0) return (int)std::min<uint64_t>((uint64_t)c->opt_lanes, std::max<uint64_t>(n / 32, 1));
-  // Measured on config 3 and config 2 (profiles/r2b_lanes.md).  Host-buffer calls: four lanes on streams of descending
-  // priority leave only the first lane's copy in and the last lane's copy out exposed (164.4 -> 159.7 ms per 10^7
-  // muons); each further lane costs ~1.2 ms of pass start-up and tails.  Device calls: two lanes let one lane's
+  // Measured on config 3 and config 2 (profiles/r2b_lanes.md).  Host-buffer calls: with four lanes the copy in of lanes
+  // 1-3 hides under lane 0's first passes and the copy out of lanes 0-2 under lane 3's last ones (the lanes' passes
+  // alternate on the SMs, so all four finish within the last 15 % of the call): 159.4 -> 155 ms per 10^7 muons; each
+  // further lane costs ~1.3 ms of pass start-up and tails.  Device calls: two lanes let one lane's
   // passes fill the tails of the other's between 2^17 and 2^22 muons (+5 to +9 % with item-mode passes); above that a single lane's passes
   // are long enough that their tails do not matter (one lane is 1 % faster), below it there is nothing to overlap.
   // REFILL and STATIC kernels run a muon's whole history in one launch: lanes only serialise them.
@@ -1015,8 +1016,7 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   // through one lane's pass (10^7 muons: 148.2 against 149.0 ms).  With two lanes of a device call, one item per warp and
   // CTAs that exit with their items let the hardware interleave the lanes' CTAs, so each lane's tail and sort are filled
   // by the other's pass: 2^18 muons 6.89 -> 6.31 ms, 2^20 muons 18.74 -> 17.84 ms; those lanes run on equal-priority
-  // streams (they should advance side by side).  Host-buffer calls keep persistent passes on streams of descending
-  // priority: there the point of the lanes is that they finish one after the other, each copying out under the next.
+  // streams (they should advance side by side).  Host-buffer calls keep persistent passes (item mode: 157.4 against 155 ms).
   // 256-thread CTAs in both modes: smaller ones lose more to CTA start-up than they gain in granularity (64 threads: -6 %).
   const bool item_mode = pl.sched == MT_SCHED_WAVEFRONT &&
                          (c->opt_pass_mode == 2 || (c->opt_pass_mode == 0 && K > 1 && host == nullptr));
