@@ -73,7 +73,7 @@ def build(force: bool = False, verbose: bool = False, defines=(), checked: bool 
             raise RuntimeError("nvcc failed linking libmuon_transport.so")
         os.replace(tmp, LIB)
     finally:
-        for obj in objs:
+        for obj, _, _ in done:                    # every object this build wrote, also after a failed compile
             if os.path.exists(obj):
                 os.remove(obj)
         with open(os.path.join(bdir, "ptxas_checked.log" if checked else "ptxas.log"), "w") as f:
