@@ -30,6 +30,25 @@ if ROOT not in sys.path:
 # DESIGN.md §3 counted one each; loads not counted as operations)
 ALG_OPS_PER_STEP = {"voxel": 383, "regions": 308, "poly": 349}
 ALG_GATHER_BYTES_PER_STEP = {"voxel": 168, "regions": 40, "poly": 50}
+
+
+def variant_work(mode, field_mode=0, joint=False):
+    """(ops, gathered bytes) per muon-step of a SURVEY.md §8(f) variant, by the counting rules of DESIGN.md §7:
+    nearest-neighbour field = no trilinear (78 ops, 128 B) but one 16-byte cell record; field at every RK4 stage = three
+    more stage positions (3 fma), lookups (voxel: 12 for the cell and the inside test + the interpolation; regions: 20;
+    polyhedra: 61) and c1 * B products (3); joint tables = one draw instead of two, an integer cell split, no polar
+    sine / cosine, one more square root."""
+    ops, gb = ALG_OPS_PER_STEP[mode], ALG_GATHER_BYTES_PER_STEP[mode]
+    interp_ops, interp_b = (78, 128) if mode == "voxel" else (0, 0)
+    if mode == "voxel" and (field_mode & 1):
+        ops, gb = ops - 78 + 1, gb - 128 + 16
+        interp_ops, interp_b = 6, 16
+    if field_mode & 2:
+        lookup = {"voxel": 12 + interp_ops, "regions": 20, "poly": 61}[mode]
+        ops, gb = ops + 2 + 3 * (3 + lookup + 3), gb + 3 * (interp_b if mode == "voxel" else 0)
+    if joint:
+        ops += -6 + 3 - 23 + 8
+    return ops, gb
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ALL launches of the dominant kernel in one 10^7-muon
 # batch of config 3, summed over the batch's z-slab passes from the ncu launch list profiles/r2_dram_launches.csv
 # (profiles/r2_summary.md has the command); None where no capture exists.  bench.py cannot run ncu itself.
@@ -102,12 +121,14 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ roofline
-def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_muons, grid_bytes, peaks, mp):
+def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_muons, grid_bytes, peaks, mp, field_mode=0,
+                   joint=False):
     """north_star's roofline for one step of this rank: "the larger of FP32-issue time ... at peak and gather bytes at
     L2/HBM bandwidth", with both terms, against peaks MEASURED in this process (mt_measure_peaks: csrc/mt_probe.cu) and
     the nominal issue peak beside them.  DESIGN.md §7 derives the per-muon-step figures."""
-    ops = steps_per_call * ALG_OPS_PER_STEP[mode]                          # thread-operations per step
-    gbytes = steps_per_call * ALG_GATHER_BYTES_PER_STEP[mode]              # gathered bytes per step
+    ops_step, gb_step = variant_work(mode, field_mode, joint)
+    ops = steps_per_call * ops_step                                        # thread-operations per step
+    gbytes = steps_per_call * gb_step                                      # gathered bytes per step
     nominal = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6           # thread-ops/s: one per lane per clock
     measured = mp["ffma_thread_ops_per_s"]                                 # a pure FFMA stream on this device, now
     per_lane = launches_per_step // max(lanes, 1)
@@ -127,7 +148,7 @@ def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_m
         "kernel": ("wave_transport_kernel: %d z-slab passes (%d lane(s)) among the %d launches of a step (the rest sort "
                    "the live list)" % (passes, lanes, launches_per_step)) if per_lane > 1 else
                   "transport_kernel (%d launch(es) per step)" % launches_per_step,
-        "ops_per_muon_step": ALG_OPS_PER_STEP[mode], "gather_bytes_per_muon_step": ALG_GATHER_BYTES_PER_STEP[mode],
+        "ops_per_muon_step": ops_step, "gather_bytes_per_muon_step": gb_step,
         "terms_ms": {
             "measured": 1e3 * t_call_s,
             "t_issue_at_measured_ffma_peak": 1e3 * t_issue, "t_issue_at_nominal_peak": 1e3 * t_issue_nominal,
@@ -346,7 +367,7 @@ def run_ours(args, rank, world, local_rank):
     value = steps_all * args.steps / t_dev_max
     e2e_value = steps_all * e2e_steps / t_e2e_max
     roofline = roofline_block(mode, steps_per_call, t_dev / args.steps, max(1, launches // args.steps), lanes_used, n,
-                              grid_bytes, peaks, b.mt_measure_peaks(local_rank))
+                              grid_bytes, peaks, b.mt_measure_peaks(local_rank), args.field_mode, args.joint)
     line = {
         "metric": "muon_steps_per_s", "value": value, "unit": "muon-steps/s",
         "muons_per_s": muons_all * args.steps / t_dev_max,
