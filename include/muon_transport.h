@@ -214,7 +214,9 @@ typedef struct {
 int mt_transport(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
                  const mt_muons_out* out, void* cuda_stream);
 
-/* Same with HOST buffers: copies in, transports, copies out on `cuda_stream`, then synchronises it.
+/* Same with HOST buffers: copies in, transports, copies out, then synchronises `cuda_stream`; returns when the outputs
+ * are in host memory.  Large calls are cut into lanes (MT_OPT_LANES) so that one lane computes while others copy; pinned
+ * (page-locked) buffers are what makes those copies asynchronous — pageable buffers work, serially.
  * exit_rec / exit_count / counters (if non-NULL) are HOST too; exit_count and counters are overwritten. */
 int mt_transport_host(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
                       const mt_muons_out* out, void* cuda_stream);
