@@ -49,3 +49,17 @@ def test_mismatched_world_size_is_refused():
                        env=_env(WORLD_SIZE="1", RANK="0", LOCAL_RANK="0"), capture_output=True, text=True, timeout=600)
     assert r.returncode != 0 and not _json_lines(r.stdout)
     assert "--gpus 4 but WORLD_SIZE=1" in r.stderr
+
+
+def test_gpu_arm_without_a_gpu_fails_loudly():
+    """no CPU fallback: on a box without CUDA the product arm refuses to run (and prints no line), also when it starts
+    its own ranks"""
+    import torch
+    if torch.cuda.is_available():
+        import pytest
+        pytest.skip("this check is for the CPU box")
+    for gpus in ("1", "2"):
+        r = subprocess.run([sys.executable, BENCH, "--gpus", gpus, "--config", "1", "--muons", "1000", "--draws", "20000"],
+                           env=_env(), capture_output=True, text=True, timeout=600)
+        assert r.returncode != 0 and not _json_lines(r.stdout)
+        assert "no CPU fallback" in r.stderr
