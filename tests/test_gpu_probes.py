@@ -1,0 +1,32 @@
+"""-m gpu: the in-process probes behind bench.py's roofline.measured_peaks (csrc/mt_probe.cu, mt_probe_field.cu) return
+numbers that are physically ordered and inside the hardware's envelope — a probe whose loop the compiler deleted, or one
+that timed an empty launch, shows up here as a rate above what 148 SMs can issue."""
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def test_measured_peaks_are_ordered_and_bounded(mt):
+    b = mt.binding
+    p = b.mt_measure_peaks(0)
+    nominal = p["sm_count"] * 128 * p["sm_clock_mhz_nominal"] * 1e6           # one thread-op per lane per clock
+    assert 0.80 * nominal < p["ffma_thread_ops_per_s"] <= 1.001 * nominal
+    # the 16-lane pipes run at half the FP32 rate, the wide multiply and the special-function unit below that
+    assert 0.40 * nominal < p["lop3_thread_ops_per_s"] < 0.60 * nominal
+    assert 0.40 * nominal < p["imad_thread_ops_per_s"] < 0.60 * nominal
+    assert 0.10 * nominal < p["mulhi_thread_ops_per_s"] < 0.40 * nominal
+    assert 0.05 * nominal < p["mufu_thread_ops_per_s"] < 0.30 * nominal
+    # gathers: L1-resident > L2-resident > HBM, the last below the pool's measured copy bandwidth
+    assert p["gather_l1_bytes_per_s"] > p["gather_64m_bytes_per_s"] > p["gather_1400m_bytes_per_s"] > 2e11
+    assert abs(p["gather_675k_bytes_per_s"] / p["gather_64m_bytes_per_s"] - 1.0) < 0.25     # both L2-resident
+    assert p["gather_1400m_bytes_per_s"] < 8e12 and p["gather_l1_bytes_per_s"] < 148 * 128 * 2.1e9
+
+
+def test_field_path_probe(mt):
+    b = mt.binding
+    f = b.mt_probe_field_paths(0)
+    assert f["records_per_launch"] == 148 * 3 * 16 * 256 * 64 * 4 or f["records_per_launch"] > 1e8
+    assert f["ldg_records_per_s"] > 0 and f["tex_records_per_s"] > 0 and f["tma_records_per_s"] > 0
+    # what DESIGN.md §7 concludes from it: plain read-only loads are the fastest of the three on the step loop's pattern
+    assert f["ldg_records_per_s"] > f["tma_records_per_s"] > 0.5 * f["tex_records_per_s"]
+    assert f["ldg_records_per_s"] * 32 < 148 * 128 * 2.1e9 * 2                    # below the L1 data path's envelope
