@@ -900,10 +900,10 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
     hot_blocks = fit_blocks;
   } else if (c->placement == MT_PLACE_AUTO) {
     // Stage when EVERY material's tables fit in one CTA's shared memory and the call is large enough to amortise the copy
-    // each CTA makes: config 4's 50x128x64 shape (115 KB, one 768-thread CTA per SM) 0.769 staged against 0.735 from L2;
+    // each CTA makes (and to run as one lane of persistent 768-thread CTAs: from 2^22 muons): config 4's 50x128x64 shape (115 KB, one 768-thread CTA per SM) 0.769 staged against 0.735 from L2;
     // a partial prefix loses (100x256x128, iron only: 0.688 against 0.730), and so does staging for a small call
     // (config 1, 65 536 muons, 38 KB per CTA: 0.397 against 0.382 ms from L2) — profiles/r2_config4_sweep.md
-    if (blob_b + c->table_bytes + 16 <= smem_budget && n >= ((uint64_t)1 << 20)) hot_blocks = c->n_materials;
+    if (blob_b + c->table_bytes + 16 <= smem_budget && n >= ((uint64_t)1 << 22)) hot_blocks = c->n_materials;
     // ... unless staging would cost the lean kernel variant (they exist for fewer staged combinations, mt_has_lean)
     MtLaunchCfg staged = cfg, gathered = cfg;
     staged.tab_smem = true; gathered.tab_smem = false;
@@ -1021,7 +1021,8 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
   const bool item_mode = pl.sched == MT_SCHED_WAVEFRONT &&
                          (c->opt_pass_mode == 2 || (c->opt_pass_mode == 0 && K > 1 && host == nullptr));
   const bool equal_prio = c->opt_lane_prio == 2 || (c->opt_lane_prio == 0 && item_mode);
-  const unsigned item_block = c->opt_block ? (unsigned)c->opt_block : 256u;
+  // (staged tables: the block the occupancy search chose — one big CTA per SM holds the copy)
+  const unsigned item_block = c->opt_block ? (unsigned)c->opt_block : (pl.cfg.tab_smem ? pl.cfg.block : 256u);
   if (item_mode) pl.cfg.block = item_block;
   auto lane_stream = [&](int k) { return equal_prio ? c->lanes[k].stream_eq : c->lanes[k].stream; };
   // Lane boundaries (multiples of 32 muons).  Device calls: equal shares.  Host-buffer calls: the first and the last lane
