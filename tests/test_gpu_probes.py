@@ -10,12 +10,14 @@ def test_measured_peaks_are_ordered_and_bounded(mt):
     b = mt.binding
     p = b.mt_measure_peaks(0)
     nominal = p["sm_count"] * 128 * p["sm_clock_mhz_nominal"] * 1e6           # one thread-op per lane per clock
-    assert 0.80 * nominal < p["ffma_thread_ops_per_s"] <= 1.001 * nominal
-    # the 16-lane pipes run at half the FP32 rate, the wide multiply and the special-function unit below that
-    assert 0.40 * nominal < p["lop3_thread_ops_per_s"] < 0.60 * nominal
-    assert 0.40 * nominal < p["imad_thread_ops_per_s"] < 0.60 * nominal
-    assert 0.10 * nominal < p["mulhi_thread_ops_per_s"] < 0.40 * nominal
-    assert 0.05 * nominal < p["mufu_thread_ops_per_s"] < 0.30 * nominal
+    ffma = p["ffma_thread_ops_per_s"]
+    assert 0.40 * nominal < ffma <= 1.001 * nominal                          # (a power-capped box clocks lower, never higher)
+    # relative to the FP32 stream of the same moment: the 16-lane pipes run at half its rate, the wide multiply and the
+    # special-function unit below that
+    assert 0.40 < p["lop3_thread_ops_per_s"] / ffma < 0.65
+    assert 0.40 < p["imad_thread_ops_per_s"] / ffma < 0.65
+    assert 0.10 < p["mulhi_thread_ops_per_s"] / ffma < 0.45
+    assert 0.05 < p["mufu_thread_ops_per_s"] / ffma < 0.35
     # gathers: L1-resident > L2-resident > HBM, the last below the pool's measured copy bandwidth
     assert p["gather_l1_bytes_per_s"] > p["gather_64m_bytes_per_s"] > p["gather_1400m_bytes_per_s"] > 2e11
     assert abs(p["gather_675k_bytes_per_s"] / p["gather_64m_bytes_per_s"] - 1.0) < 0.25     # both L2-resident
