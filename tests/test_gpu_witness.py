@@ -28,8 +28,11 @@ def test_config1_full_against_libm_witness(mt, oracle, workloads):
 
 
 def test_config2_against_libm_witness(mt, oracle, workloads):
-    wl = workloads.config2(n=100_000, n_draws=100_000)           # 30 m, ~720 steps per muon
-    check_against_witness(gpu_transport(mt, wl), _witness(oracle, wl), "GPU config2 (100k muons)")
+    # 30 m, ~720 steps per muon; 250k muons leave more than 100 residual muons, so the KS test on the residual subset
+    # alone (north_star's rule for them) is exercised as well
+    wl = workloads.config2(n=250_000, n_draws=100_000)
+    c = check_against_witness(gpu_transport(mt, wl), _witness(oracle, wl), "GPU config2 (250k muons)")
+    assert (~c["mask"]).sum() >= 100
 
 
 def test_config3_small_against_libm_witness(mt, oracle, workloads):

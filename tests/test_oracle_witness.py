@@ -34,6 +34,7 @@ def check_against_witness(got, witness, label):
     if residual.sum() >= 100:            # the residual subset on its own when it is large enough
         sub = lambda d: {k: d[k][residual] for k in ("pos", "mom")}
         ks_res = ks_populations(sub(got), sub(witness))
+        print("[witness] %s: KS on the %d residual muons alone %s" % (label, residual.sum(), {k: round(float(v), 3) for k, v in ks_res.items()}))
         assert min(ks_res.values()) > 0.01, (label, ks_res)
     # the witness is NOT the contract: if every muon were bit-identical the two modes would be the same code
     assert c["bit_exact"] < 1.0
