@@ -269,7 +269,9 @@ int mt_probe_field_paths(int cuda_device, mt_field_paths* out);
  * mt_debug_sample: cell_out[i] = alias draw from table `which` (0 = Dp/p, 1 = theta) of
  * (material, pbin) with word d_words[i].  JOINT mode (which = 0): d_words holds 2n words, the select word of draw i
  * at [i] and its accept word at [n + i]; cell_out[i] is the flat cell index.
- * mt_debug_philox: out[i][0..3] = Philox4x32-10 block for (seed, id_base + i, step). */
+ * mt_debug_philox: out[i][0..3] = Philox4x32-10 block for (seed, id_base + i, step), computed by the
+ * step loop's own routine (host-made round keys) and cross-checked on the device against the form with the key
+ * schedule inline. */
 int mt_debug_sample(mt_ctx* ctx, int material, int pbin, int which, const uint32_t* d_words, uint64_t n,
                     uint32_t* d_cell_out, void* cuda_stream);
 int mt_debug_philox(mt_ctx* ctx, uint64_t seed, uint64_t id_base, uint32_t step, uint64_t n,

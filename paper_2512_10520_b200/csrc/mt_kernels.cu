@@ -135,14 +135,20 @@ __global__ void debug_sample_kernel(const typename Tab<PACK>::cell_t* tab, uint3
   out[i] = draw<PACK, false>(P, V, 0u, N, words[i]);
 }
 
-__global__ void debug_philox_kernel(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,
-                                    uint32_t* out) {
+// Both forms of the block: the textbook one with the key schedule inline, and the hot path's own (philox4x32_10_rk, round
+// keys from the host exactly as run_transport fills them).  The hook returns the hot path's words; if the two ever
+// differed it would return the textbook words XOR 0xFFFFFFFF, which no oracle comparison survives.
+struct MtRoundKeys { uint32_t rk[20]; };
+__global__ void debug_philox_kernel(uint32_t k0, uint32_t k1, const __grid_constant__ MtRoundKeys keys, uint64_t id_base,
+                                    uint32_t step, uint64_t n, uint32_t* out) {
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const uint64_t id = id_base + i;
-  uint32_t w[4];
+  uint32_t w[4], v[4];
   philox4x32_10((uint32_t)id, (uint32_t)(id >> 32), step, 0u, k0, k1, w);
-  reinterpret_cast<uint4*>(out)[i] = make_uint4(w[0], w[1], w[2], w[3]);
+  philox4x32_10_rk((uint32_t)id, (uint32_t)(id >> 32), step, 0u, keys.rk, v);
+  const bool same = (w[0] == v[0]) & (w[1] == v[1]) & (w[2] == v[2]) & (w[3] == v[3]);
+  reinterpret_cast<uint4*>(out)[i] = same ? make_uint4(v[0], v[1], v[2], v[3]) : make_uint4(~w[0], ~w[1], ~w[2], ~w[3]);
 }
 
 // two-word draw of the joint tables: words[i] selects, words[n + i] accepts
@@ -265,6 +271,11 @@ cudaError_t mt_launch_debug_lookup(const MtParams& P, size_t smem_bytes, const f
 cudaError_t mt_launch_debug_philox(uint32_t k0, uint32_t k1, uint64_t id_base, uint32_t step, uint64_t n,
                                    uint32_t* out, cudaStream_t stream) {
   if (n == 0) return cudaSuccess;
-  debug_philox_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(k0, k1, id_base, step, n, out);
+  MtRoundKeys keys;
+  for (uint32_t r = 0; r < 10; ++r) {                       // as run_transport fills MtParams::rk
+    keys.rk[2 * r] = k0 + r * 0x9E3779B9u;
+    keys.rk[2 * r + 1] = k1 + r * 0xBB67AE85u;
+  }
+  debug_philox_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(k0, k1, keys, id_base, step, n, out);
   return cudaGetLastError();
 }
