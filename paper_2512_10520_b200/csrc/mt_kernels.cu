@@ -201,6 +201,10 @@ cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaS
   mt_kernel_fn fn = pick_kernel(P.mode, cfg);
   cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
   if (e != cudaSuccess) return e;
+  // as much L1 as the staged data leaves: the alias tables live there (mt_step.cuh: MT_GRID_HINT)
+  e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout,
+                           cfg.tab_smem ? (int)cudaSharedmemCarveoutMaxShared : (int)cudaSharedmemCarveoutMaxL1);
+  if (e != cudaSuccess) return e;
   void* args[] = {(void*)&P};
   return cudaLaunchKernel((const void*)fn, dim3(cfg.grid), dim3(cfg.block), args, cfg.smem_bytes, stream);
 }

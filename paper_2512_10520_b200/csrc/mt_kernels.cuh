@@ -32,22 +32,26 @@ MT_DEV View<PACK> stage_view(const MtParams& P) {
   // (the per-table axes, by far the largest part, are NOT staged: one 128-bit read-only load per step serves them from
   // L1, and a CTA then starts after copying ~1.5 KB instead of ~7 KB — what makes small CTAs and item-mode passes cheap)
   float* sblob = reinterpret_cast<float*>(mt_smem);
-  for (int i = threadIdx.x; i < P.bl.n_words; i += blockDim.x)
-    if (!MT_AXES_GLOBAL || i < P.bl.off_axes || i >= P.bl.off_zlo) sblob[i] = __ldg(P.blob + i);
+  const int cut = MT_AXES_GLOBAL ? P.bl.off_zlo - P.bl.off_axes : 0;      // words of the blob that are not staged (a multiple of 4)
+  for (int i = threadIdx.x; i < P.bl.n_words; i += blockDim.x) {
+    if (i < P.bl.off_axes) sblob[i] = __ldg(P.blob + i);
+    else if (i >= P.bl.off_zlo) sblob[i - cut] = __ldg(P.blob + i);
+    else if (!MT_AXES_GLOBAL) sblob[i] = __ldg(P.blob + i);
+  }
   View<PACK> V;
   V.edges = sblob;
   V.edges_open = sblob + P.bl.off_edges_open;
   V.steps = sblob + P.bl.off_steps;
   V.axes = MT_AXES_GLOBAL ? reinterpret_cast<const float4*>(P.blob + P.bl.off_axes)
                           : reinterpret_cast<const float4*>(sblob + P.bl.off_axes);
-  V.zlo = sblob + P.bl.off_zlo;
-  V.regions = reinterpret_cast<const MtRegionDev*>(sblob + P.bl.off_regions);
-  V.blocks = reinterpret_cast<const MtBlockDev*>(sblob + P.bl.off_blocks);
-  V.binlut = reinterpret_cast<const uint16_t*>(sblob + P.bl.off_binlut);
-  V.zlut = reinterpret_cast<const int16_t*>(sblob + P.bl.off_zlut);
+  V.zlo = sblob + (P.bl.off_zlo - cut);
+  V.regions = reinterpret_cast<const MtRegionDev*>(sblob + (P.bl.off_regions - cut));
+  V.blocks = reinterpret_cast<const MtBlockDev*>(sblob + (P.bl.off_blocks - cut));
+  V.binlut = reinterpret_cast<const uint16_t*>(sblob + (P.bl.off_binlut - cut));
+  V.zlut = reinterpret_cast<const int16_t*>(sblob + (P.bl.off_zlut - cut));
   const uint32_t* gtab = (PACK == 32) ? P.tab32 : reinterpret_cast<const uint32_t*>(P.tab64);
   V.tab = reinterpret_cast<const typename Tab<PACK>::cell_t*>(gtab);
-  uint4* stab = reinterpret_cast<uint4*>(sblob + ((P.bl.n_words + 3) & ~3));
+  uint4* stab = reinterpret_cast<uint4*>(sblob + ((MT_STAGED_WORDS(P.bl) + 3) & ~3));
   V.hot = reinterpret_cast<const typename Tab<PACK>::cell_t*>(stab);
   if (TAB_SMEM) {
     const uint32_t n16 = (P.hot_cells * (PACK / 8) + 15u) / 16u;          // the device array is padded to 16 bytes

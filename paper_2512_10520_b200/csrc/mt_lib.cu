@@ -152,7 +152,7 @@ uint32_t threshold24(float prob) {
   return t <= 0.0 ? 0u : (t >= 16777216.0 ? 16777216u : (uint32_t)t);
 }
 
-size_t blob_bytes(const mt_ctx* c) { return (size_t)c->bl.n_words * sizeof(float); }
+size_t blob_bytes(const mt_ctx* c) { return (size_t)MT_STAGED_WORDS(c->bl) * sizeof(float); }   // shared memory a CTA stages
 
 int rebuild_blob(mt_ctx* c) {
   // [edges][steps x4][axes x4][z_lo][regions]; see mt_params.h

@@ -22,6 +22,12 @@ struct MtRegionDev {
 //   [off_binlut ..]                      uint16 momentum-bin table (two per word), see MtParams::bin_shift
 //   [off_zlut ..]                        int16 z-interval table (two per word), see MtParams::zlut_n; the z_lo array is
 //                                        followed by two +inf entries so that the table's two fix-ups need no bound
+#ifndef MT_AXES_GLOBAL
+#define MT_AXES_GLOBAL 1     // per-table axes read from global memory (L1) instead of a shared-memory copy
+#endif
+// Words of the blob a CTA stages: everything, or everything but the axes (which then take no shared memory either: the
+// arrays behind them move down by the axes' length)
+#define MT_STAGED_WORDS(bl) (MT_AXES_GLOBAL ? (bl).n_words - ((bl).off_zlo - (bl).off_axes) : (bl).n_words)
 struct MtBlobLayout {
   int32_t off_edges_open, off_steps, off_axes, off_zlo, off_regions, off_blocks, off_binlut, off_zlut, n_words;
 };
