@@ -949,12 +949,19 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
     // one pass per z-slab; between passes the live muons are counting-sorted by xy cell
     const bool voxel = (c->geom.mode == MT_GEOM_VOXEL);
     const double unit = voxel ? (double)c->geom.cell : 0.01;
-    // default slab (units of 1 cm): voxel grids 64 cells — the slab's field layers stay L2-resident — and 128 for small
-    // batches, which are bound by the latency of one muon's ~3000 dependent steps and want fewer passes; region and
-    // polyhedra geometries have no field working set to bound: 256 (profiles/r2b_lanes.md)
-    const double auto_slab = voxel ? (n < ((uint64_t)1 << 19) ? 128.0 : 64.0) : 256.0;
-    pl.slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : auto_slab) * unit;
+    // default slab (units of 1 cm).  Voxel grids: 96 cells for a full batch (the slab's field layers stay L2-resident;
+    // 64 ... 128 cells are within 0.4 % of each other at 10^7 muons); smaller calls are bound more and more by the latency
+    // of one muon's ~2600 dependent steps and by the tails of their passes, and want fewer, thicker ones: 128 cells below
+    // 2^22 muons, 512 below 2^18, and a single pass over the whole path below 2^15 (2^14 muons: 4.15 -> 3.13 ms, 2^16:
+    // 4.20 -> 3.67, 2^19: 10.2 -> 9.8, 2^21: 33.3 -> 32.5; profiles/r2c_summary.md).  Region and polyhedra geometries
+    // have no field working set to bound: 256 (profiles/r2b_lanes.md)
+    const double auto_slab = !voxel ? 256.0
+                             : n < ((uint64_t)1 << 15) ? 1e9
+                             : n < ((uint64_t)1 << 18) ? 512.0
+                             : n < ((uint64_t)1 << 22) ? 128.0 : 96.0;
     const double span = (double)c->geom.z_exit - (double)c->geom.z_min;
+    pl.slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : auto_slab) * unit;
+    if (span > 0.0 && std::isfinite(span)) pl.slab = std::min(pl.slab, span);      // (one pass: the slab is the whole path)
     pl.n_pass = (int)std::max(1.0, std::min(ceil(span / pl.slab), 4096.0));
     // sort key: the voxel column (coarsened until there are at most 2^18 keys), or a 128 x 128 grid over the world box
     int key_nx, key_ny;
