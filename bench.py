@@ -161,6 +161,11 @@ def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_m
         "measured_peaks": {"ffma_T_thread_ops_per_s": measured / 1e12, "lop3_T": mp["lop3_thread_ops_per_s"] / 1e12,
                            "imad_T": mp["imad_thread_ops_per_s"] / 1e12, "mulhi_T": mp["mulhi_thread_ops_per_s"] / 1e12,
                            "mufu_T": mp["mufu_thread_ops_per_s"] / 1e12,
+                           # mixed streams as a fraction of the fma rate: near 1 = that pipe runs beside the FP32 stream,
+                           # 0.75 / 0.625 = its instructions take 2 / 4 FP32 issue cycles each
+                           "mix_over_ffma": {"8_fma_4_lop3": mp["mix_ffma8_lop3_4_thread_ops_per_s"] / measured,
+                                             "8_fma_4_imad": mp["mix_ffma8_imad4_thread_ops_per_s"] / measured,
+                                             "8_fma_2_mulwide": mp["mix_ffma8_mulwide2_thread_ops_per_s"] / measured},
                            "gather_TB_per_s": {"l1_resident_64k": mp["gather_l1_bytes_per_s"] / 1e12,
                                                "l2_resident_675k": mp["gather_675k_bytes_per_s"] / 1e12,
                                                "l2_resident_64m": mp["gather_64m_bytes_per_s"] / 1e12,

@@ -244,13 +244,17 @@ int mt_get_info(const mt_ctx* ctx, int what, int64_t* value);
  *                        kind with no dependency stalls (8 warps per scheduler, 8 independent chains per thread):
  *                        fma.rn.f32 / lop3.b32 / mad.lo.u32 / mul.hi.u32 / rsqrt.approx.f32 (the conversion unit)
  *   gather_*_bytes_per_s 32-byte sectors per second x 32 for one random sector per lane out of a working set of
- *                        64 KB (L1-resident), 675 KB and 64 MB (L2-resident), 1400 MB (HBM)                              */
+ *                        64 KB (L1-resident), 675 KB and 64 MB (L2-resident), 1400 MB (HBM)
+ *   mix_*                the same count for mixed streams, 8 fma.rn.f32 to 4 lop3.b32 / 4 mad.lo.u32 / 2 mul.wide.u32 per
+ *                        group: a pipe that runs beside the FP32 stream leaves the total near the fma rate, one that takes
+ *                        its place pulls it down by its own cycles                                                      */
 typedef struct {
   int32_t sm_count;
   double sm_clock_mhz_nominal;
   double ffma_thread_ops_per_s, ffma_warp_instr_per_s_per_smsp;
   double lop3_thread_ops_per_s, imad_thread_ops_per_s, mulhi_thread_ops_per_s, mufu_thread_ops_per_s;
   double gather_l1_bytes_per_s, gather_675k_bytes_per_s, gather_64m_bytes_per_s, gather_1400m_bytes_per_s;
+  double mix_ffma8_lop3_4_thread_ops_per_s, mix_ffma8_imad4_thread_ops_per_s, mix_ffma8_mulwide2_thread_ops_per_s;
 } mt_peaks;
 int mt_measure_peaks(int cuda_device, mt_peaks* out);
 

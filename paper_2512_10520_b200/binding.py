@@ -67,7 +67,9 @@ class mt_peaks(C.Structure):
                 ("lop3_thread_ops_per_s", C.c_double), ("imad_thread_ops_per_s", C.c_double),
                 ("mulhi_thread_ops_per_s", C.c_double), ("mufu_thread_ops_per_s", C.c_double),
                 ("gather_l1_bytes_per_s", C.c_double), ("gather_675k_bytes_per_s", C.c_double),
-                ("gather_64m_bytes_per_s", C.c_double), ("gather_1400m_bytes_per_s", C.c_double)]
+                ("gather_64m_bytes_per_s", C.c_double), ("gather_1400m_bytes_per_s", C.c_double),
+                ("mix_ffma8_lop3_4_thread_ops_per_s", C.c_double), ("mix_ffma8_imad4_thread_ops_per_s", C.c_double),
+                ("mix_ffma8_mulwide2_thread_ops_per_s", C.c_double)]
 
 
 class mt_field_paths(C.Structure):

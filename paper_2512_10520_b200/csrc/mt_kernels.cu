@@ -201,10 +201,24 @@ cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaS
   mt_kernel_fn fn = pick_kernel(P.mode, cfg);
   cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
   if (e != cudaSuccess) return e;
-  // as much L1 as the staged data leaves: the alias tables live there (mt_step.cuh: MT_GRID_HINT)
-  e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout,
-                           cfg.tab_smem ? (int)cudaSharedmemCarveoutMaxShared : (int)cudaSharedmemCarveoutMaxL1);
-  if (e != cudaSuccess) return e;
+  // As much L1 as the resident CTAs' shared memory leaves: the alias tables live there (mt_step.cuh: MT_GRID_HINT).  The
+  // carveout is a preference the driver may honour at the cost of occupancy, so it is sized for the number of CTAs that fit
+  // an SM when shared memory is not restricted (1 KB per CTA is the system's own), never below that.
+  {
+    struct Key { const void* fn; unsigned block; size_t smem; int carve; };
+    static thread_local Key last = {nullptr, 0u, 0, 0};
+    if (last.fn != (const void*)fn || last.block != cfg.block || last.smem != cfg.smem_bytes) {
+      e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutDefault);
+      if (e != cudaSuccess) return e;
+      int occ = 0;
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)fn, (int)cfg.block, cfg.smem_bytes);
+      if (e != cudaSuccess) return e;
+      const size_t need = (size_t)std::max(occ, 1) * (cfg.smem_bytes + 1024);
+      last = {(const void*)fn, cfg.block, cfg.smem_bytes, (int)std::min<size_t>(100, need * 100 / (228 * 1024) + 1)};
+    }
+    e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout, last.carve);
+    if (e != cudaSuccess) return e;
+  }
   void* args[] = {(void*)&P};
   return cudaLaunchKernel((const void*)fn, dim3(cfg.grid), dim3(cfg.block), args, cfg.smem_bytes, stream);
 }
@@ -212,6 +226,9 @@ cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaS
 cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm) {
   mt_kernel_fn fn = pick_kernel(P.mode, cfg);
   cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
+  if (e != cudaSuccess) return e;
+  // (the answer wanted is the one with shared memory unrestricted: mt_launch_transport sizes the carveout from it)
+  e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutDefault);
   if (e != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, (const void*)fn, cfg.block, cfg.smem_bytes);
 }

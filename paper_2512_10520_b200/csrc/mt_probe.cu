@@ -43,6 +43,39 @@ __global__ void __launch_bounds__(256) probe_issue_kernel(int iters, uint32_t se
   if (acc == 0x12345678u) sink[0] = acc;          // never true in practice: keeps the chains alive
 }
 
+// ---- mixed streams: per group 8 fma.rn.f32 and NI instructions of another kind, all on independent chains.  They tell
+// which pipes run beside the FP32 stream and which take its place: lop3 (ALU pipe) overlaps it, mad.lo and
+// mul.wide (the FMA pipe's integer half) add their own 2 and 4 cycles per warp instruction.
+enum { MIX_LOP3 = 0, MIX_IMAD = 1, MIX_MULWIDE = 2 };
+template <int NI, int KIND>
+__global__ void __launch_bounds__(256) probe_mix_kernel(int iters, uint32_t seed, uint32_t* sink) {
+  float f[kChains];
+  uint32_t u[kChains];
+  uint64_t w[kChains];
+  const float a = 1.0f + 1e-7f * (float)(seed & 7u), b = 1e-9f * (float)(threadIdx.x & 3);
+  const uint32_t m = 0x9E3779B9u ^ seed, k = threadIdx.x | 1u;
+#pragma unroll
+  for (int c = 0; c < kChains; ++c) { f[c] = 1.0f + 0.001f * (float)(c + (threadIdx.x & 1)); u[c] = seed + 77u * c + threadIdx.x; w[c] = u[c]; }
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+#pragma unroll
+      for (int c = 0; c < kChains; ++c) {
+        asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[c]) : "f"(a), "f"(b));
+        if (c < NI) {
+          if (KIND == MIX_LOP3) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[c]) : "r"(m), "r"(k));
+          else if (KIND == MIX_IMAD) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(u[c]) : "r"(m), "r"(k));
+          else asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(w[c]) : "r"((uint32_t)(w[c] >> 32)), "r"(m));
+        }
+      }
+    }
+  }
+  uint32_t acc = 0;
+#pragma unroll
+  for (int c = 0; c < kChains; ++c) acc ^= u[c] ^ __float_as_uint(f[c]) ^ (uint32_t)w[c] ^ (uint32_t)(w[c] >> 32);
+  if (acc == 0x12345678u) sink[0] = acc;
+}
+
 // ---- gather probe: every lane reads one 32-byte sector (the size of a field-grid record) at a
 // pseudo-random position of a buffer of `n_sectors` sectors; four loads in flight per thread.  Positions come from a
 // multiplicative hash of (thread, trip), so a warp's 32 sectors are unrelated: the worst case the step loop can meet.
@@ -100,6 +133,15 @@ template <int OP> cudaError_t issue_rate(int sm_count, uint32_t* sink, double* w
   return cudaSuccess;
 }
 
+template <int NI, int KIND> cudaError_t mix_rate(int sm_count, uint32_t* sink, double* thread_ops_per_s) {
+  const int grid = sm_count * 8, block = 256, iters = 1000;
+  float ms = 0.0f;
+  cudaError_t e = time_best([&] { probe_mix_kernel<NI, KIND><<<grid, block>>>(iters, 12345u, sink); }, 3, &ms);
+  if (e != cudaSuccess) return e;
+  *thread_ops_per_s = (double)iters * 8 * (kChains + NI) * grid * block / (ms * 1e-3);
+  return cudaSuccess;
+}
+
 }  // namespace
 
 extern "C" int mt_measure_peaks(int cuda_device, mt_peaks* out) {
@@ -128,6 +170,9 @@ extern "C" int mt_measure_peaks(int cuda_device, mt_peaks* out) {
     if (issue_rate<OP_IMAD>(sms, sink, &per_smsp, &out->imad_thread_ops_per_s) != cudaSuccess) { rc = MT_ERR_CUDA; break; }
     if (issue_rate<OP_IMAD_WIDE>(sms, sink, &per_smsp, &out->mulhi_thread_ops_per_s) != cudaSuccess) { rc = MT_ERR_CUDA; break; }
     if (issue_rate<OP_MUFU>(sms, sink, &per_smsp, &out->mufu_thread_ops_per_s) != cudaSuccess) { rc = MT_ERR_CUDA; break; }
+    if (mix_rate<4, MIX_LOP3>(sms, sink, &out->mix_ffma8_lop3_4_thread_ops_per_s) != cudaSuccess) { rc = MT_ERR_CUDA; break; }
+    if (mix_rate<4, MIX_IMAD>(sms, sink, &out->mix_ffma8_imad4_thread_ops_per_s) != cudaSuccess) { rc = MT_ERR_CUDA; break; }
+    if (mix_rate<2, MIX_MULWIDE>(sms, sink, &out->mix_ffma8_mulwide2_thread_ops_per_s) != cudaSuccess) { rc = MT_ERR_CUDA; break; }
     // gathers: one buffer of the largest size, the smaller working sets are prefixes of it
     const size_t sizes[4] = {(size_t)64 << 10, (size_t)675 << 10, (size_t)64 << 20, (size_t)1400 << 20};
     if (cudaMalloc(&buf, sizes[3]) != cudaSuccess) { cudaGetLastError(); rc = MT_ERR_NOMEM; break; }

@@ -18,6 +18,12 @@ def test_measured_peaks_are_ordered_and_bounded(mt):
     assert 0.40 < p["imad_thread_ops_per_s"] / ffma < 0.65
     assert 0.10 < p["mulhi_thread_ops_per_s"] / ffma < 0.45
     assert 0.05 < p["mufu_thread_ops_per_s"] / ffma < 0.35
+    # mixed streams: the ALU pipe runs beside the FP32 stream (12 instructions in about the time of the 8
+    # fma alone would be 1.5x; anything above 0.85 of the fma rate shows the overlap), the FMA pipe's integer half does not:
+    # 8 fma + 4 mad.lo cost 8 + 4 x 2 cycles (0.75), 8 fma + 2 mul.wide 8 + 2 x 4 (0.625)
+    assert 0.85 < p["mix_ffma8_lop3_4_thread_ops_per_s"] / ffma < 1.05
+    assert 0.60 < p["mix_ffma8_imad4_thread_ops_per_s"] / ffma < 0.85
+    assert 0.45 < p["mix_ffma8_mulwide2_thread_ops_per_s"] / ffma < 0.75
     # gathers: L1-resident > L2-resident > HBM, the last below the pool's measured copy bandwidth
     assert p["gather_l1_bytes_per_s"] > p["gather_64m_bytes_per_s"] > p["gather_1400m_bytes_per_s"] > 2e11
     assert abs(p["gather_675k_bytes_per_s"] / p["gather_64m_bytes_per_s"] - 1.0) < 0.25     # both L2-resident
