@@ -214,7 +214,12 @@ cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaS
       e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)fn, (int)cfg.block, cfg.smem_bytes);
       if (e != cudaSuccess) return e;
       const size_t need = (size_t)std::max(occ, 1) * (cfg.smem_bytes + 1024);
-      last = {(const void*)fn, cfg.block, cfg.smem_bytes, (int)std::min<size_t>(100, need * 100 / (228 * 1024) + 1)};
+      // the SM's shared-memory configurations (KB); the preference is a percentage of 228 KB that the driver rounds UP to
+      // one of them, so the smallest configuration that holds `need` is asked for by its own size rounded DOWN to a percent
+      static const int kb[] = {8, 16, 32, 64, 100, 132, 164, 196, 228};
+      int pick = 228;
+      for (int c : kb) if ((size_t)c * 1024 >= need) { pick = c; break; }
+      last = {(const void*)fn, cfg.block, cfg.smem_bytes, std::max(1, pick * 100 / 228)};
     }
     e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout, last.carve);
     if (e != cudaSuccess) return e;

@@ -917,8 +917,9 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
   c->last_lean = cfg.lean; c->last_sched = sched;
   cfg.smem_bytes = blob_b + ((hot_blocks * block_cells * cell_b + 15) & ~(size_t)15) + 16;
 
-  // Block size.  A call that fills the machine takes the block that keeps the most threads resident (ties -> the smaller
-  // block).  A STATIC / REFILL call small enough to be resident all at once is spread as evenly as the block granularity
+  // Block size.  A call that fills the machine takes the block that keeps the most threads resident; ties go to the smaller
+  // block, except for the persistent CTAs of a z-slab pass, where fewer and larger CTAs are faster for the same 24 resident
+  // warps (10^7 muons: 6 x 128 threads 143.6 ms, 3 x 256 142.4, 2 x 384 141.5, 1 x 768 139.2; profiles/r2c_summary.md).  A STATIC / REFILL call small enough to be resident all at once is spread as evenly as the block granularity
   // allows instead: its time is that of the fullest SM, so the block that minimises ceil(CTAs / SMs) x block wins
   // (config 1, 65 536 muons: 2 x 256 threads on most SMs but 3 x 128 = 384 at most -> 0.49 -> 0.37 ms, profiles/r2b_lanes.md).
   int occ = 0;
@@ -938,8 +939,9 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
     if (one_launch && ctas <= (uint64_t)o * c->sm_count) {
       const uint64_t load = ((ctas + c->sm_count - 1) / c->sm_count) * blk;
       if (load < best_load) { best_load = load; occ = o; cfg.block = blk; }
-    } else if (best_load == ~(uint64_t)0 && cand >= 256u && (size_t)o * blk > (size_t)occ * cfg.block) {
-      occ = o; cfg.block = blk;
+    } else if (best_load == ~(uint64_t)0 && cand >= 256u &&
+               ((size_t)o * blk > (size_t)occ * cfg.block || (!one_launch && (size_t)o * blk == (size_t)occ * cfg.block))) {
+      occ = o; cfg.block = blk;                     // (WAVEFRONT: ties -> the LARGER block, see above)
     }
   }
   if (occ < 1) return fail(c, MT_ERR_UNSUPPORTED, "kernel does not fit on an SM with %zu B shared memory", cfg.smem_bytes);
