@@ -919,7 +919,8 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
 
   // Block size.  A call that fills the machine takes the block that keeps the most threads resident; ties go to the smaller
   // block, except for the persistent CTAs of a z-slab pass, where fewer and larger CTAs are faster for the same 24 resident
-  // warps (10^7 muons: 6 x 128 threads 143.6 ms, 3 x 256 142.4, 2 x 384 141.5, 1 x 768 139.2; profiles/r2c_summary.md).  A STATIC / REFILL call small enough to be resident all at once is spread as evenly as the block granularity
+  // warps (10^7 muons: 6 x 128 threads 143.6 ms, 3 x 256 142.4, 2 x 384 141.5, 1 x 768 139.2; from 2^21 muons on — a 2^17-muon
+  // call is faster with 256-thread CTAs, 4.80 against 5.28 ms; profiles/r2c_summary.md).  A STATIC / REFILL call small enough to be resident all at once is spread as evenly as the block granularity
   // allows instead: its time is that of the fullest SM, so the block that minimises ceil(CTAs / SMs) x block wins
   // (config 1, 65 536 muons: 2 x 256 threads on most SMs but 3 x 128 = 384 at most -> 0.49 -> 0.37 ms, profiles/r2b_lanes.md).
   int occ = 0;
@@ -940,7 +941,8 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
       const uint64_t load = ((ctas + c->sm_count - 1) / c->sm_count) * blk;
       if (load < best_load) { best_load = load; occ = o; cfg.block = blk; }
     } else if (best_load == ~(uint64_t)0 && cand >= 256u &&
-               ((size_t)o * blk > (size_t)occ * cfg.block || (!one_launch && (size_t)o * blk == (size_t)occ * cfg.block))) {
+               ((size_t)o * blk > (size_t)occ * cfg.block ||
+                (!one_launch && n >= ((uint64_t)1 << 21) && (size_t)o * blk == (size_t)occ * cfg.block))) {
       occ = o; cfg.block = blk;                     // (WAVEFRONT: ties -> the LARGER block, see above)
     }
   }
@@ -997,11 +999,11 @@ int choose_lanes(const mt_ctx* c, uint64_t n, int sched, bool host_call) {
   // 1-3 hides under lane 0's first passes and the copy out of lanes 0-2 under lane 3's last ones (the lanes' passes
   // alternate on the SMs, so all four finish within the last 15 % of the call): 159.4 -> 155 ms per 10^7 muons; each
   // further lane costs ~1.3 ms of pass start-up and tails.  Device calls: two lanes let one lane's
-  // passes fill the tails of the other's between 2^17 and 2^22 muons (+5 to +9 % with item-mode passes); above that a single lane's passes
+  // passes fill the tails of the other's between 2^18 and 2^21 muons (+1 to +6 % with item-mode passes); above that a single lane's passes
   // are long enough that their tails do not matter (one lane is 1 % faster), below it there is nothing to overlap.
   // REFILL and STATIC kernels run a muon's whole history in one launch: lanes only serialise them.
   if (host_call && n >= ((uint64_t)1 << 21)) return 4;
-  if (sched == MT_SCHED_WAVEFRONT && n >= ((uint64_t)1 << 17) && n < ((uint64_t)1 << 22)) return 2;
+  if (sched == MT_SCHED_WAVEFRONT && n >= ((uint64_t)1 << 18) && n < ((uint64_t)1 << 21)) return 2;
   return 1;
 }
 
