@@ -50,10 +50,10 @@ def variant_work(mode, field_mode=0, joint=False):
         ops += -6 + 3 - 23 + 8
     return ops, gb
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ALL launches of the dominant kernel in one 10^7-muon
-# batch of config 3, summed over the batch's z-slab passes from the ncu launch list profiles/r2_dram_launches.csv
-# (profiles/r2_summary.md has the command); None where no capture exists.  bench.py cannot run ncu itself.
-NCU_DRAM_BYTES_PER_BATCH = {"voxel": 29.19e9, "regions": None, "poly": None}     # 17.56 GB read + 11.63 GB written, 47 passes
-NCU_DRAM_SOURCE = "profiles/r2_dram_launches.csv"
+# batch of config 3, summed over the batch's z-slab passes from the ncu launch list profiles/r2c_dram_launches.csv
+# (profiles/r2c_summary.md has the command); None where no capture exists.  bench.py cannot run ncu itself.
+NCU_DRAM_BYTES_PER_BATCH = {"voxel": 27.71e9, "regions": None, "poly": None}     # 20.14 GB read + 7.57 GB written, 32 passes
+NCU_DRAM_SOURCE = "profiles/r2c_dram_launches.csv"
 SM_COUNT, LANES_PER_SM = 148, 128          # B200: 4 SMSPs x 32 lanes issue one warp instruction per clock
 
 
@@ -155,8 +155,9 @@ def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_m
             "t_gather_if_every_record_came_from": {k: 1e3 * v for k, v in t_gather.items()},
             "reading": "the issue term binds.  The gather terms price every lane's record as a separate 32-byte sector "
                        "at the random-sector rate of that level; a term above the measured time means the schedule does "
-                       "not pay it: the sorted wavefront makes a warp's lanes share sectors in L1 (ncu: L1 hit 57-77 %, "
-                       "L2 hit 88-91 %, DRAM 2-3 % busy)"},
+                       "not pay it: the sorted wavefront makes a warp's lanes share sectors, the alias tables are served "
+                       "from L1 and the field grid (which does not allocate in L1) from the L2-resident z-slab (ncu: L2 hit "
+                       "93-95 %, 778 GB of L2 traffic per batch = 5.6 TB/s, DRAM 3 % busy)"},
         "gather_tb_per_s": gbytes / t_call_s / 1e12,
         "measured_peaks": {"ffma_T_thread_ops_per_s": measured / 1e12, "lop3_T": mp["lop3_thread_ops_per_s"] / 1e12,
                            "imad_T": mp["imad_thread_ops_per_s"] / 1e12, "mulhi_T": mp["mulhi_thread_ops_per_s"] / 1e12,

@@ -76,6 +76,16 @@ MT_DEV View<PACK> stage_view(const MtParams& P) {
 struct Tally {
   unsigned long long steps = 0;
   unsigned f1 = 0, f2 = 0, f3 = 0, f4 = 0;
+#ifdef MT_SLOT_STATS
+  // diagnostic build (-DMT_SLOT_STATS; profiles/r2c_summary.md): lane-steps a WAVEFRONT pass had room for, and where the
+  // unused ones went.  counters[5] += 32 x (steps of the item's slowest lane), [6] += steps that lanes whose muon
+  // terminated in the item sat out, [7] += steps that parked lanes waited for the slowest one
+  unsigned slots = 0, idle_fin = 0, idle_park = 0;
+  MT_DEV void slot_stats(unsigned own, bool fin, bool parked) {
+    const unsigned mx = __reduce_max_sync(kFull, own);
+    slots += mx; idle_fin += fin ? mx - own : 0u; idle_park += parked ? mx - own : 0u;
+  }
+#endif
   MT_DEV void count(int flag) { f1 += (flag == 1); f2 += (flag == 2); f3 += (flag == 3); f4 += (flag == 4); }
   // `spread`: slot of 8 counters to add to (item-mode kernels flush once per warp-item, hundreds of thousands of times
   // per pass: the adds are spread over MT_COUNTER_SLOTS copies and summed by reduce_counters_kernel at the end of the call)
@@ -93,6 +103,13 @@ struct Tally {
       if (f3) atomicAdd(counters + 3, (unsigned long long)f3);
       if (f4) atomicAdd(counters + 4, (unsigned long long)f4);
     }
+#ifdef MT_SLOT_STATS
+    slots = __reduce_add_sync(kFull, slots); idle_fin = __reduce_add_sync(kFull, idle_fin); idle_park = __reduce_add_sync(kFull, idle_park);
+    if (lane == 0) {
+      atomicAdd(counters + 5, (unsigned long long)slots); atomicAdd(counters + 6, (unsigned long long)idle_fin);
+      atomicAdd(counters + 7, (unsigned long long)idle_park);
+    }
+#endif
   }
 };
 
@@ -290,6 +307,9 @@ wave_transport_kernel(const __grid_constant__ MtParams P) {
     write_final(P, m, idx, fin, lane);
     tally.count(fin);
     const bool parked = (flag == MT_PARK);
+#ifdef MT_SLOT_STATS
+    tally.slot_stats((unsigned)(m.step - step_in), fin != 0, parked);
+#endif
     const unsigned pm = __ballot_sync(kFull, parked);
     if (pm) {
       const int leader = __ffs(pm) - 1;

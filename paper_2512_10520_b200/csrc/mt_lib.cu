@@ -899,15 +899,11 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
     if (fit_blocks == 0) return fail(c, MT_ERR_UNSUPPORTED, "no material's tables (%zu B) fit in shared memory", block_cells * cell_b);
     hot_blocks = fit_blocks;
   } else if (c->placement == MT_PLACE_AUTO) {
-    // Stage when EVERY material's tables fit in one CTA's shared memory and the call is large enough to amortise the copy
-    // each CTA makes (and to run as one lane of persistent 768-thread CTAs: from 2^22 muons): config 4's 50x128x64 shape (115 KB, one 768-thread CTA per SM) 0.769 staged against 0.735 from L2;
-    // a partial prefix loses (100x256x128, iron only: 0.688 against 0.730), and so does staging for a small call
-    // (config 1, 65 536 muons, 38 KB per CTA: 0.397 against 0.382 ms from L2) — profiles/r2_config4_sweep.md
-    if (blob_b + c->table_bytes + 16 <= smem_budget && n >= ((uint64_t)1 << 22)) hot_blocks = c->n_materials;
-    // ... unless staging would cost the lean kernel variant (they exist for fewer staged combinations, mt_has_lean)
-    MtLaunchCfg staged = cfg, gathered = cfg;
-    staged.tab_smem = true; gathered.tab_smem = false;
-    if (hot_blocks && !mt_has_lean(c->geom.mode, staged) && mt_has_lean(c->geom.mode, gathered)) hot_blocks = 0;
+    // AUTO gathers from L1 / L2.  Since the field-grid loads stopped allocating in L1 (mt_step.cuh: MT_GRID_HINT) the tables
+    // have it to themselves and staging loses for every shape: config 4's 50x128x64 (115 KB, all three materials in one
+    // 768-thread CTA) 0.773 staged against 0.789 from L1 / L2, 100x256x128 (iron only) 0.711 against 0.775
+    // (profiles/r2c_summary.md; in round 2, with the grid allocating, the smallest shape still gained 2 % from staging).
+    hot_blocks = 0;
   }
   P.hot_cells = (uint32_t)(hot_blocks * block_cells);
   cfg.tab_smem = hot_blocks > 0;
@@ -959,10 +955,14 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
     // 2^22 muons, 512 below 2^18, and a single pass over the whole path below 2^15 (2^14 muons: 4.15 -> 3.13 ms, 2^16:
     // 4.20 -> 3.67, 2^19: 10.2 -> 9.8, 2^21: 33.3 -> 32.5; profiles/r2c_summary.md).  Region and polyhedra geometries
     // have no field working set to bound: 256 (profiles/r2b_lanes.md)
+    // A trilinear field evaluated at every Runge-Kutta stage reads four times the grid records per step: its full
+    // batches want the slab well inside L2 (32 cells 296 ms, 64 cells 309, 96 cells 328 per 10^7 muons).
+    const bool stage_trilinear = voxel && (c->geom.field_mode & 3) == MT_FIELD_PER_STAGE;
     const double auto_slab = !voxel ? 256.0
                              : n < ((uint64_t)1 << 15) ? 1e9
                              : n < ((uint64_t)1 << 18) ? 512.0
-                             : n < ((uint64_t)1 << 22) ? 128.0 : 96.0;
+                             : n < ((uint64_t)1 << 22) ? 128.0
+                             : stage_trilinear ? 32.0 : 96.0;
     const double span = (double)c->geom.z_exit - (double)c->geom.z_min;
     pl.slab = (c->opt_slab_cells ? (double)c->opt_slab_cells : auto_slab) * unit;
     if (span > 0.0 && std::isfinite(span)) pl.slab = std::min(pl.slab, span);      // (one pass: the slab is the whole path)
