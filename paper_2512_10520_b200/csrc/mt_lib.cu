@@ -166,7 +166,7 @@ int rebuild_blob(mt_ctx* c) {
   bl.off_zlo = bl.off_axes + 4 * nt;
   bl.off_regions = (bl.off_zlo + n_reg + 2 + 3) & ~3;         // two +inf entries follow the z_lo array
   const int n_blk = c->have_geom ? (int)c->blocks.size() : 0;
-  bl.off_blocks = (bl.off_regions + 10 * n_reg + 3) & ~3;
+  bl.off_blocks = (bl.off_regions + 12 * n_reg + 3) & ~3;
   bl.off_binlut = bl.off_blocks + 24 * n_blk;
   const double lo = (double)c->p_lo, hi = (double)c->p_hi;
   std::vector<float> edges(n_edges);
@@ -201,8 +201,8 @@ int rebuild_blob(mt_ctx* c) {
   // margin of 1 % of a cell, which dwarfs the float32 rounding of the device's cell index (below 2^-11 of a cell here)
   std::vector<int16_t> zlut;
   c->zlut_n = 0; c->zlut_g0 = 0.0f; c->zlut_inv = 0.0f;
-  // (a handful of intervals is searched faster than the table's four dependent shared-memory reads: config 1 has one)
-  if (n_reg >= 8 && c->geom.mode == MT_GEOM_REGIONS) {
+  // (one region needs neither: a single comparison; the lean kernels take no geometry that would need the search)
+  if (n_reg >= 2 && c->geom.mode == MT_GEOM_REGIONS) {
     const double g0 = std::min((double)c->geom.z_min, (double)c->regions[0].z_lo);
     const double g1 = std::max((double)c->geom.z_exit, (double)c->regions[n_reg - 1].z_lo);
     for (int nzc = 1024; nzc <= 4096 && std::isfinite(g0) && std::isfinite(g1) && g1 > g0 && zlut.empty(); nzc *= 2) {
@@ -257,8 +257,8 @@ int rebuild_blob(mt_ctx* c) {
   blob[bl.off_zlo + n_reg] = blob[bl.off_zlo + n_reg + 1] = INFINITY;
   for (int j = 0; j < n_reg; ++j) {
     blob[bl.off_zlo + j] = c->regions[j].z_lo;
-    static_assert(sizeof(mt_region) == 40 && sizeof(MtRegionDev) == 40, "region layout");
-    memcpy(&blob[bl.off_regions + 10 * j], &c->regions[j], sizeof(mt_region));
+    static_assert(sizeof(mt_region) == 40 && sizeof(MtRegionDev) == 48, "region layout");
+    memcpy(&blob[bl.off_regions + 12 * j], &c->regions[j], sizeof(mt_region));      // same field order; two pad words follow
   }
   for (int j = 0; j < n_blk; ++j) {
     // §3.12: the per-block constants of the slice interpolation, each ONE float32 operation
@@ -788,7 +788,8 @@ void fill_params(const mt_ctx* c, MtParams& P) {
   P.grid_k = (0x4B400000u - 1u) * (uint32_t)(P.gsz + P.gsy + 1);
   P.gsy_bytes = (uint64_t)P.gsy * sizeof(MtCellPair); P.gsz_bytes = (uint64_t)P.gsz * sizeof(MtCellPair);
   P.gsyz_bytes = P.gsy_bytes + P.gsz_bytes;
-  P.lean = (c->lean_axes ? MT_LEAN_AXES : 0) | (c->lean_inside ? MT_LEAN_INSIDE : 0);
+  P.lean = (c->lean_axes ? MT_LEAN_AXES : 0) | (c->lean_inside ? MT_LEAN_INSIDE : 0) |
+           ((c->zlut_n != 0 || g.n_regions <= 1) ? MT_LEAN_ZTABLE : 0);
   P.lean_x_lo = c->lean_box[0]; P.lean_x_hi = c->lean_box[1]; P.lean_y_lo = c->lean_box[2]; P.lean_y_hi = c->lean_box[3];
   P.lean_z_lo = c->lean_box[4]; P.lean_z_hi = c->lean_box[5];
   P.n_materials = c->n_materials; P.n_pbins = c->n_pbins; P.n_dp = c->n_dp; P.n_th = c->n_th;
@@ -908,7 +909,9 @@ int make_plan(mt_ctx* c, uint64_t n, uint64_t seed, const mt_muons_out* out, Pla
   P.hot_cells = (uint32_t)(hot_blocks * block_cells);
   cfg.tab_smem = hot_blocks > 0;
   // voxel grids need both facts (the lean kernel has no inside-grid test), regions and polyhedra the axes fact only
-  const bool facts = (c->geom.mode == MT_GEOM_VOXEL) ? (P.lean == MT_LEAN_ALL) : ((P.lean & MT_LEAN_AXES) != 0);
+  const bool facts = (c->geom.mode == MT_GEOM_VOXEL) ? ((P.lean & MT_LEAN_ALL) == MT_LEAN_ALL)
+                     : (c->geom.mode == MT_GEOM_REGIONS) ? ((P.lean & (MT_LEAN_AXES | MT_LEAN_ZTABLE)) == (MT_LEAN_AXES | MT_LEAN_ZTABLE))
+                     : ((P.lean & MT_LEAN_AXES) != 0);
   cfg.lean = !c->opt_no_lean && facts && mt_has_lean(c->geom.mode, cfg);
   c->last_lean = cfg.lean; c->last_sched = sched;
   cfg.smem_bytes = blob_b + ((hot_blocks * block_cells * cell_b + 15) & ~(size_t)15) + 16;

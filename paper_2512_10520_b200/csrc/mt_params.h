@@ -3,11 +3,14 @@
 #pragma once
 #include <stdint.h>
 
-// Region record as staged in shared memory.  Same field order as mt_region.
-struct MtRegionDev {
-  float z_lo, z_hi, x_lo, x_hi, y_lo, y_hi;
+// Region record as staged in shared memory: mt_region's ten words in three 16-byte groups, so that a
+// lookup is three 128-bit shared-memory loads instead of ten scalar ones.
+struct __align__(16) MtRegionDev {
+  float z_lo, z_hi, x_lo, x_hi;
+  float y_lo, y_hi;
   int32_t material;
-  float bx, by, bz;
+  float bx;
+  float by, bz, pad0, pad1;
 };
 
 // The "const blob": small read-only arrays every CTA stages into shared memory at start.
@@ -17,7 +20,7 @@ struct MtRegionDev {
 //                                        first cell of the material's tables in the packed array (int bits)
 //   [off_axes + 4*t .. +3]               lo_dp, d_dp * 2^-16, lo_th, d_th * 2^-16 (log2) of table t = (m-1)*n_pbins + i
 //   [off_zlo  + j]                       z_lo of region j (search array)
-//   [off_regions + 10*j ..]              MtRegionDev j
+//   [off_regions + 12*j ..]              MtRegionDev j
 //   [off_blocks + 24*j ..]               MtBlockDev j (POLY mode)
 //   [off_binlut ..]                      uint16 momentum-bin table (two per word), see MtParams::bin_shift
 //   [off_zlut ..]                        int16 z-interval table (two per word), see MtParams::zlut_n; the z_lo array is
@@ -58,7 +61,9 @@ struct __align__(32) MtCellPair {
 //                   with a logarithm
 //   MT_LEAN_INSIDE  lean_{x,y,z}_{lo,hi} bound the part of the world box whose every float32 position maps to a cell of
 //                   the voxel grid (the whole box but for a few floats next to a face, which take the general code)
-enum { MT_LEAN_AXES = 1, MT_LEAN_INSIDE = 2, MT_LEAN_ALL = 3 };
+//   MT_LEAN_ZTABLE  (regions) the z-interval table exists (zlut_n != 0) or there is at most one region: the region lookup
+//                   needs no binary search
+enum { MT_LEAN_AXES = 1, MT_LEAN_INSIDE = 2, MT_LEAN_ALL = 3, MT_LEAN_ZTABLE = 4 };
 
 // Checked build (-DMT_CHECKED, `python -m paper_2512_10520_b200.build --checked` -> libmuon_transport_checked.so): every
 // index the kernels form into a global array is compared with the array's size first, and a violation is counted in
