@@ -120,7 +120,8 @@ def test_lean_variants_of_the_other_voxel_modes(mt, oracle, joint, field_mode):
 
 
 @pytest.mark.parametrize("which,sched", [("config1", 0), ("config2", 0), ("config2", 3), ("config2p", 0), ("config2p", 2),
-                                         ("config2_joint", 0), ("config2p_per_stage", 0)])
+                                         ("config2_joint", 0), ("config2p_per_stage", 0), ("config2_few_regions", 2),
+                                         ("config2_few_regions", 3)])
 def test_lean_variants_of_regions_and_polyhedra(mt, oracle, which, sched):
     # regions and polyhedra take the lean kernels on the table facts alone (clamps, caps, theta < pi/4): REFILL and
     # WAVEFRONT, tables from L2 or (config 1: 38 KB) staged in shared memory
@@ -129,6 +130,9 @@ def test_lean_variants_of_regions_and_polyhedra(mt, oracle, which, sched):
     b = mt.binding
     wl = {"config1": lambda: w.config1(n=20_000, n_draws=100_000),
           "config2": lambda: w.config2(n=40_000, n_draws=100_000, n_cells=4),
+          # one cell of the shield: a handful of regions, for which the z-interval table is built too (the LEAN region
+          # kernels contain no binary search: MT_LEAN_ZTABLE)
+          "config2_few_regions": lambda: w.config2(n=20_000, n_draws=100_000, n_cells=1),
           "config2p": lambda: w.config2p(n=40_000, n_draws=100_000, n_cells=4),
           "config2_joint": lambda: w.config2(n=20_000, n_draws=100_000, n_cells=2, joint=True, table_shape=(20, 32, 16)),
           "config2p_per_stage": lambda: w.config2p(n=20_000, n_draws=100_000, n_cells=2, field_mode=w.FIELD_PER_STAGE)}[which]()
@@ -141,6 +145,37 @@ def test_lean_variants_of_regions_and_polyhedra(mt, oracle, which, sched):
             torch.cuda.synchronize()
             assert b.mt_get_info(h.ctx, b.MT_INFO_LEAN_FACTS) & 1
             assert b.mt_get_info(h.ctx, b.MT_INFO_LAST_LEAN) == 1 - no_lean
+            got = unpack(out["pos_flag"].cpu().numpy(), out["mom_steps"].cpu().numpy())
+        finally:
+            h.close()
+        c = compare(got, ref)
+        assert c["bit_exact"] == 1.0 and c["matched"] >= 0.999
+
+
+def test_lean_region_kernels_are_refused_when_no_z_interval_table_exists(mt, oracle):
+    # 1000 slabs of 0.2 mm: more than two z_lo per table cell at any table size, so the lookup has to search — which only the
+    # general kernels contain (MT_LEAN_ZTABLE is part of the facts a LEAN region kernel needs)
+    import copy
+    import torch
+    from paper_2512_10520_b200 import workloads as w
+    b = mt.binding
+    wl = w.config1(n=8192, n_draws=100_000)
+    edges = np.linspace(2.0, 2.2, 1001).astype(np.float32)
+    regs = np.array([(a, c, -1.0, 1.0, -1.0, 1.0, 1, 0.0, 1.7 * (1 - 2 * (j & 1)), 0.0)
+                     for j, (a, c) in enumerate(zip(edges[:-1], edges[1:])) if c > a], w.REGION_DTYPE)
+    geom = copy.copy(wl.geom)
+    geom.regions = regs
+    wl = copy.copy(wl)
+    wl.geom = geom
+    ref = oracle_transport(oracle, wl)
+    for sched in (2, 3):
+        h = b.MuonTransport(0).setup(wl.hist, wl.geom)
+        try:
+            h.set_option(b.MT_OPT_SCHEDULE, sched)
+            out = h.transport(torch.from_numpy(wl.muons.pos_q).cuda(), torch.from_numpy(wl.muons.mom).cuda(), wl.seed)
+            torch.cuda.synchronize()
+            assert b.mt_get_info(h.ctx, b.MT_INFO_LEAN_FACTS) & 1            # the table axes would allow it
+            assert b.mt_get_info(h.ctx, b.MT_INFO_LAST_LEAN) == 0
             got = unpack(out["pos_flag"].cpu().numpy(), out["mom_steps"].cpu().numpy())
         finally:
             h.close()

@@ -218,10 +218,13 @@ def test_region_lookup_through_the_z_interval_table(mt, oracle):
         "dense (binary search)": np.linspace(2.0, 2.2, 1000).astype(np.float32),      # 0.2 mm intervals: no table possible
         "beyond the world box": np.array([-3.0, -1.0, 4.0, 31.0, 35.0, 36.0, 40.0], np.float32),
         "single": np.array([1.0, 2.0], np.float32),
+        # the table is built from two regions on (the LEAN region kernels contain no search: MT_LEAN_ZTABLE)
+        "two regions": np.array([1.0, 2.0, 7.5], np.float32),
+        "three regions": np.array([0.0, 0.25, 29.0, 30.0], np.float32),
     }
     for name, z_edges in cases.items():
         z_edges = np.unique(z_edges)
-        regs = regions_from(z_edges, gap_every=0 if name in ("single", "dense (binary search)", "two z_lo in one cell") else 3)
+        regs = regions_from(z_edges, gap_every=0 if name in ("single", "dense (binary search)", "two z_lo in one cell", "two regions", "three regions") else 3)
         geom = Geometry(MODE_REGIONS, -1.0, 1.0, -1.0, 1.0, 0.0, 30.0, 1.0, 100, 2, regions=regs)
         zs = np.concatenate([regs["z_lo"], regs["z_hi"]])
         special = np.concatenate([zs, np.nextafter(zs, np.float32(-np.inf)), np.nextafter(zs, np.float32(np.inf)),
