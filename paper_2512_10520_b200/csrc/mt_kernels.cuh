@@ -209,9 +209,14 @@ transport_kernel(const __grid_constant__ MtParams P) {
     for (int k = 0; k < kInnerSteps; ++k) {
       int flag = 0;
       if (active) {
+        // two steps per warp vote, as in the z-slab passes
         const uint64_t id = P.id_base + idx;
         flag = step_once<GEOM, PACK, TAB_SMEM, false, JOINT, FIELD, true, LEAN>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
-        if (flag == 0) tally.steps += 1;
+        if (flag == 0) {
+          tally.steps += 1;
+          flag = step_once<GEOM, PACK, TAB_SMEM, false, JOINT, FIELD, true, LEAN>(P, V, m, (uint32_t)id, (uint32_t)(id >> 32));
+          if (flag == 0) tally.steps += 1;
+        }
       }
       if (__any_sync(kFull, flag != 0)) {
         write_final(P, m, idx, flag, lane);
