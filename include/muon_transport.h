@@ -67,7 +67,9 @@ enum {
   MT_EXIT_PROJECT = 1      /* moved back onto the plane z = z_exit along its final direction; momentum unchanged.  The  */
 };                         /* dense outputs pos_flag / mom_steps are never changed by this                              */
 
-/* alias-table placement (north_star subsystem 1) */
+/* alias-table placement (north_star subsystem 1): gathered through L1 / L2, which is what AUTO picks (the field grid does
+ * not allocate in L1, so the tables have it to themselves), or the longest prefix of whole materials that fits
+ * staged in shared memory by every CTA */
 enum { MT_PLACE_AUTO = 0, MT_PLACE_SMEM = 1, MT_PLACE_L2 = 2 };
 
 /* scheduling of muons onto lanes (north_star subsystem 4); results never depend on it */
@@ -84,7 +86,8 @@ enum {
   MT_OPT_BLOCK_THREADS = 2,  /* 0 = library default; else a multiple of 32 in [32, 768] (the largest block  */
                              /* the transport kernels are compiled for)                                    */
   MT_OPT_BLOCKS_PER_SM = 3,  /* 0 = library default (persistent kernels)                                   */
-  MT_OPT_SLAB_CELLS = 4,     /* wavefront: slab thickness along z, in units of 1 cm; 0 = default           */
+  MT_OPT_SLAB_CELLS = 4,     /* wavefront: slab thickness along z, in units of 1 cm; 0 = default (by geometry */
+                             /* and call size: voxel grids 96 for a full batch, thicker for small calls)      */
   MT_OPT_REFILL_MIN_IDLE = 5,/* refill: lanes of a warp that must be idle before it refills; 0 = default   */
   MT_OPT_KEY_LOOKAHEAD = 6,  /* wavefront: the sort key is the xy cell a muon reaches after this many percent */
                              /* of a slab on a straight line; -1 = default (50), 0 = its current cell         */
