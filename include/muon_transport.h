@@ -204,7 +204,8 @@ typedef struct {
   uint32_t* exit_count;    /* optional, one counter; ADDED to (caller zeroes it): one per EXITED muon, so it */
                            /* may exceed the capacity; may be given WITHOUT exit_rec to count hits only     */
   uint32_t exit_capacity;
-  uint64_t* counters;      /* optional [8], ADDED to: [0] total steps, [1..4] muons per flag               */
+  uint64_t* counters;      /* optional [8], ADDED to: [0] total steps, [1..4] muons per flag; [5..7] stay  */
+                           /* untouched (a -DMT_SLOT_STATS diagnostic build counts lane-slots there)       */
 } mt_muons_out;
 
 /* Transport n muons (ids id_base .. id_base+n-1) until each meets a break condition.  All buffers DEVICE.
