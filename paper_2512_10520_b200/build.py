@@ -34,7 +34,7 @@ CHECKED_LIB = os.path.join(HERE, "libmuon_transport_checked.so")
 
 def build(force: bool = False, verbose: bool = False, defines=(), checked: bool = False) -> str:
     """Compile the translation units in parallel (the kernel instantiations are split over several so that this takes
-    well under a minute), then link.  `defines`: extra -D macros (e.g. MT_MAX_THREADS=1024) for tuning experiments.
+    about a minute on 8 cores), then link.  `defines`: extra -D macros (e.g. MT_MAX_THREADS=1024) for tuning experiments.
     checked=True builds libmuon_transport_checked.so with -DMT_CHECKED: the same kernels with every global-array index
     bounds-checked (csrc/mt_params.h: MT_CHECK); load it through MUON_TRANSPORT_LIB (tests/test_gpu_checked.py)."""
     LIB = CHECKED_LIB if checked else globals()["LIB"]
