@@ -225,6 +225,41 @@ int mt_transport(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t id_bas
 int mt_transport_host(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
                       const mt_muons_out* out, void* cuda_stream);
 
+/* mt_transport for callers that must not allocate device memory while they transport.
+ *
+ * Who that is: code that runs after another component has claimed the device's memory for itself (a framework's caching
+ * pool, a memory budget fixed at start-up, a partition with a hard cap), where a cudaMalloc may fail at any moment; and
+ * code inside a latency-bound loop (a trigger-level or online simulation step, a service answering requests), where
+ * cudaMalloc / cudaFree stall every stream of the device while they run.  mt_transport cannot serve them: its z-slab
+ * passes park the muons still in flight, their sort keys and the pass counters in library scratch that it cudaMallocs
+ * whenever a call is larger than any before it, and it creates streams and events for its lanes.
+ *
+ * This call computes exactly what mt_transport computes (same arguments, all buffers DEVICE and the caller's; same
+ * outputs bit for bit; same schedule: MT_OPT_SCHEDULE, or the library's choice by geometry and n) but keeps all of that
+ * scratch in ONE array that is part of the library's image: MT_STATIC_SCRATCH_BYTES (9 MiB) of device memory that every
+ * GPU holds from the moment it loads the library until the process exits, whether this call is ever used or not.  It
+ * runs as a single lane on `cuda_stream` itself, and it never calls cudaMalloc, cudaFree, a stream / event constructor
+ * or any other routine that allocates.  The price is the size limit: n <= MT_STATIC_SCRATCH_MAX_MUONS (65 536; the
+ * array is sized so that every geometry and option setting fits at that n).  A larger n returns MT_ERR_UNSUPPORTED
+ * with the limit in mt_last_error() and enqueues nothing; cut the batch into calls of at most that size with their own
+ * id_base — results do not depend on the split.
+ *
+ * First call on a device: the library asks the runtime where that device's copy of the array lives (once per device and
+ * process, remembered), and CUDA loads the kernels the call launches.  Make one call — any n >= 1 — during your own
+ * set-up, before the phase that must not allocate and before you begin capturing a stream.  The tables and the geometry
+ * of the context are device memory too: mt_build_alias / mt_set_geometry allocate them and belong in that set-up as well.
+ *
+ * The array is shared by every call of this entry point on the device, from every context and thread, and nothing
+ * remembers who used it last: each call clears the counters it needs on `cuda_stream` before its kernels, so the
+ * previous call's leftovers are harmless, but two calls whose work overlaps on the GPU (different streams without an
+ * event between them, two host threads) overwrite each other's in-flight muons.  Order them on one stream, or make the
+ * second stream wait for the first.  Calls of mt_transport itself use other memory and may overlap with this one.
+ * Errors otherwise as mt_transport: MT_ERR_STATE / MT_ERR_INVALID_ARG before anything is enqueued, MT_ERR_CUDA with the
+ * runtime's message. */
+enum { MT_STATIC_SCRATCH_MAX_MUONS = 65536, MT_STATIC_SCRATCH_BYTES = 9 * 1024 * 1024 };
+int mt_transport_static_scratch(mt_ctx* ctx, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                                const mt_muons_out* out, void* cuda_stream);
+
 /* Number of kernel launches made by this context so far (bench.py's gpu_launches). */
 int64_t mt_launch_count(const mt_ctx* ctx);
 

@@ -24,11 +24,12 @@ MT_HIST_MARGINAL, MT_HIST_JOINT = 0, 1
 MT_EXIT_AT_BREAK, MT_EXIT_PROJECT = 0, 1
 MT_INFO_LEAN_FACTS, MT_INFO_LAST_LEAN, MT_INFO_LAST_SCHEDULE, MT_INFO_LAST_LANES, MT_INFO_CHECK_ERRORS = 1, 2, 3, 4, 5
 MT_FIELD_TRILINEAR, MT_FIELD_NEAREST, MT_FIELD_PER_STAGE = 0, 1, 2
+MT_STATIC_SCRATCH_MAX_MUONS, MT_STATIC_SCRATCH_BYTES = 65536, 9 * 1024 * 1024
 
 # every symbol include/muon_transport.h declares (tests check that the library exports each one)
 SYMBOLS = ["mt_strerror", "mt_last_error", "mt_create", "mt_destroy", "mt_set_option", "mt_load_histograms",
            "mt_build_alias", "mt_get_alias", "mt_set_geometry", "mt_transport", "mt_transport_host",
-           "mt_launch_count", "mt_get_info", "mt_measure_peaks", "mt_probe_field_paths", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
+           "mt_transport_static_scratch", "mt_launch_count", "mt_get_info", "mt_measure_peaks", "mt_probe_field_paths", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
 
 
 class mt_hist_desc(C.Structure):
@@ -108,7 +109,7 @@ def lib():
         L.mt_build_alias.argtypes = [C.c_void_p, C.c_int]
         L.mt_get_alias.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.mt_set_geometry.argtypes = [C.c_void_p, C.POINTER(mt_geometry)]
-        for name in ("mt_transport", "mt_transport_host"):
+        for name in ("mt_transport", "mt_transport_host", "mt_transport_static_scratch"):
             getattr(L, name).argtypes = [C.c_void_p, C.POINTER(mt_muons_in), C.c_uint64, C.c_uint64, C.c_uint64,
                                          C.POINTER(mt_muons_out), C.c_void_p]
         L.mt_launch_count.restype = C.c_int64
@@ -280,6 +281,31 @@ def mt_transport(ctx, pos_q, mom, seed, id_base=0, out=None, exit_capacity=0, co
     return out
 
 
+def mt_transport_static_scratch(ctx, pos_q, mom, seed, out, id_base=0, stream=None):
+    """mt_transport for a caller that must not allocate device memory (include/muon_transport.h has the full story):
+    the library keeps the scratch of this call in a fixed array inside its own image, so at most
+    MT_STATIC_SCRATCH_MAX_MUONS muons per call, and calls must not overlap on the GPU.  For the same reason nothing is
+    allocated HERE either: `out` must already hold the caller's CUDA tensors "pos_flag" and "mom_steps" [n,4] float32 and
+    may hold "exit_rec" [cap,8] float32 with "exit_count" [1] int32, "exit_count" alone, and "counters" [8] int64; the
+    caller zeroes exit_count and counters (they are added to).  pos_q / mom must be contiguous.  Returns `out`."""
+    import torch
+    n = pos_q.shape[0]
+    for t, shape in ((pos_q, (n, 4)), (mom, (n, 4)), (out["pos_flag"], (n, 4)), (out["mom_steps"], (n, 4))):
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == shape
+    o = mt_muons_out()
+    o.pos_flag, o.mom_steps = out["pos_flag"].data_ptr(), out["mom_steps"].data_ptr()
+    if "exit_count" in out:
+        o.exit_count = out["exit_count"].data_ptr()
+    if "exit_rec" in out:
+        o.exit_rec, o.exit_capacity = out["exit_rec"].data_ptr(), out["exit_rec"].shape[0]
+    if "counters" in out:
+        o.counters = out["counters"].data_ptr()
+    i = mt_muons_in(pos_q.data_ptr(), mom.data_ptr())
+    _check(ctx, lib().mt_transport_static_scratch(ctx, C.byref(i), n, int(id_base), int(seed), C.byref(o),
+                                                  _stream_ptr(stream)))
+    return out
+
+
 def mt_transport_host(ctx, pos_q, mom, seed, id_base=0, out=None, exit_capacity=0, counters=True, stream=None):
     """Same call with HOST buffers (numpy arrays or pinned CPU torch tensors); returns numpy arrays."""
     pos_q, mom = _as_host(pos_q), _as_host(mom)
@@ -397,6 +423,9 @@ class MuonTransport:
 
     def transport_host(self, pos_q, mom, seed, **kw):
         return mt_transport_host(self.ctx, pos_q, mom, seed, **kw)
+
+    def transport_static_scratch(self, pos_q, mom, seed, out, **kw):
+        return mt_transport_static_scratch(self.ctx, pos_q, mom, seed, out, **kw)
 
     def close(self):
         if self.ctx is not None:

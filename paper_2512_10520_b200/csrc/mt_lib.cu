@@ -1293,3 +1293,146 @@ int mt_debug_philox(mt_ctx* c, uint64_t seed, uint64_t id_base, uint32_t step, u
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// mt_transport_static_scratch: the transport call for callers that may not allocate (include/muon_transport.h)
+// ------------------------------------------------------------------------------------------------
+// All the scratch of one single-lane call, as a file-scope device array: part of the library's image, so each GPU that
+// loads the library sets these 9 MiB aside until the process ends and no call ever has to ask the allocator for them.
+// Sized for MT_STATIC_SCRATCH_MAX_MUONS muons under the largest bookkeeping a plan can ask for (4096 passes, 2^18 sort
+// keys): 2.05 MiB of counters, histogram and offsets + 108 B per muon in flight = 8.80 MiB.
+static __device__ __align__(256) unsigned char mt_static_scratch[MT_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+// In host code the name `mt_static_scratch` is only a handle that the runtime can look the array up by; it is not where
+// the array lives on the GPU, and a kernel handed `mt_static_scratch` itself from the host would read and write through a
+// host address.  The device address comes from cudaGetSymbolAddress, asked once per device with that device current (each
+// GPU has its own copy of the array) and kept for the rest of the process.
+int static_scratch_base(mt_ctx* c, unsigned char** base) {
+  enum { kMaxDevices = 64 };
+  static unsigned char* known[kMaxDevices];      // zero-initialised; written once per device
+  if (c->device < 0 || c->device >= kMaxDevices)
+    return fail(c, MT_ERR_UNSUPPORTED, "mt_transport_static_scratch serves CUDA devices 0..%d", kMaxDevices - 1);
+  unsigned char* p = __atomic_load_n(&known[c->device], __ATOMIC_ACQUIRE);
+  if (!p) {
+    void* sym = nullptr;
+    MT_CUDA(c, cudaGetSymbolAddress(&sym, mt_static_scratch));      // (the caller's DeviceGuard made c->device current)
+    if (!sym) return fail(c, MT_ERR_CUDA, "cudaGetSymbolAddress returned no address for the static scratch");
+    p = (unsigned char*)sym;
+    __atomic_store_n(&known[c->device], p, __ATOMIC_RELEASE);       // (two threads racing here store the same value)
+  }
+  *base = p;
+  return MT_OK;
+}
+
+// One lane of run_transport on the caller's own stream, with the lane's two scratch buffers carved out of the static
+// array instead of reserved from the allocator.  Nothing here may allocate: no DevBuf::reserve, no ensure_lanes (streams
+// and events), no std::vector.
+int run_transport_static_scratch(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                                 const mt_muons_out* out, cudaStream_t stream) {
+  if (!c->have_tables || !c->have_geom)
+    return fail(c, MT_ERR_STATE, "mt_transport_static_scratch needs mt_build_alias and mt_set_geometry after the last mt_load_histograms");
+  if (n == 0) return MT_OK;
+  if (!in->pos_q || !in->mom || !out->pos_flag || !out->mom_steps) return fail(c, MT_ERR_INVALID_ARG, "null muon buffer");
+  if (out->exit_rec && !out->exit_count) return fail(c, MT_ERR_INVALID_ARG, "exit_rec without exit_count");
+  if (n > (uint64_t)MT_STATIC_SCRATCH_MAX_MUONS)
+    return fail(c, MT_ERR_UNSUPPORTED,
+                "mt_transport_static_scratch takes at most %d muons per call (%llu given): its scratch is a fixed %d-byte "
+                "array; split the batch, or use mt_transport", (int)MT_STATIC_SCRATCH_MAX_MUONS, (unsigned long long)n,
+                (int)MT_STATIC_SCRATCH_BYTES);
+  unsigned char* base = nullptr;
+  int rc = static_scratch_base(c, &base);
+  if (rc != MT_OK) return rc;
+
+  Plan pl;
+  rc = make_plan(c, n, seed, out, pl);
+  if (rc != MT_OK) return rc;
+  c->last_lanes = 1;
+  MtParams P = pl.P;
+  P.n = n; P.id_base = id_base; P.idx_base = 0u;
+  P.in_pos_q = (const float4*)in->pos_q; P.in_mom = (const float4*)in->mom;
+  P.out_pos_flag = (float4*)out->pos_flag; P.out_mom_steps = (float4*)out->mom_steps;
+  MtLaunchCfg cfg = pl.cfg;
+  const uint64_t ctas = (n + cfg.block - 1) / cfg.block;
+
+  if (pl.sched == MT_SCHED_STATIC) {                       // one lane per muon: no scratch at all
+    cfg.grid = (unsigned)ctas;
+    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
+    c->launches += 1;
+    return MT_OK;
+  }
+  if (pl.sched == MT_SCHED_REFILL) {                       // the work counter idle lanes refill from
+    cfg.grid = (unsigned)std::min<uint64_t>(pl.persistent_grid, ctas);
+    P.work_counter = (unsigned long long*)base;
+    MT_CUDA(c, cudaMemsetAsync(base, 0, 8, stream));       // (it still holds the last call's final value)
+    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
+    c->launches += 1;
+    return MT_OK;
+  }
+
+  // WAVEFRONT.  Bookkeeping first, as in run_transport: [MT_COUNTER_SLOTS x 8] spread tallies (unused here: persistent
+  // passes add to the caller's counters directly), [n_pass + 1] work counters (u64), [n_pass + 1] live counts (u32), then
+  // the key histogram and its scan [n_keys] (u32) each; then the state in flight: two buffers of 48-byte records, {key,
+  // rank} 8 B and the permutation 4 B per muon.
+  const int n_pass = pl.n_pass, n_keys = pl.n_keys;
+  const size_t off_work = (size_t)MT_COUNTER_SLOTS * 64;
+  const size_t off_counts = off_work + (size_t)(n_pass + 1) * 8;
+  const size_t off_hist = (off_counts + (size_t)(n_pass + 1) * 4 + 255) & ~(size_t)255;
+  const size_t zero_b = off_hist + (size_t)n_keys * 4;     // everything up to and including the histogram starts at zero
+  const size_t off_wave = (zero_b + (size_t)n_keys * 4 + 255) & ~(size_t)255;
+  const size_t n48 = ((size_t)n * 48 + 255) & ~(size_t)255, n8 = ((size_t)n * 8 + 255) & ~(size_t)255,
+               n4 = ((size_t)n * 4 + 255) & ~(size_t)255;
+  const size_t need = off_wave + 2 * n48 + n8 + n4;
+  if (need > (size_t)MT_STATIC_SCRATCH_BYTES)              // (cannot happen for n <= the maximum; kept as the last line of defence)
+    return fail(c, MT_ERR_UNSUPPORTED, "mt_transport_static_scratch: this call needs %zu bytes of scratch, the static array holds %d",
+                need, (int)MT_STATIC_SCRATCH_BYTES);
+  unsigned long long* work = (unsigned long long*)(base + off_work);
+  uint32_t* counts = (uint32_t*)(base + off_counts);
+  P.counters_spread = nullptr;
+  P.persistent = 1;
+  P.hist = (uint32_t*)(base + off_hist);
+  P.key_offset = P.hist + n_keys;
+  float4* rec[2] = {(float4*)(base + off_wave), (float4*)(base + off_wave + n48)};
+  P.sort_key = (uint2*)(base + off_wave + 2 * n48);
+  P.perm = (uint32_t*)(base + off_wave + 2 * n48 + n8);
+  cfg.grid = (unsigned)std::min<uint64_t>(pl.persistent_grid, ctas);
+  const unsigned aux_grid = (unsigned)std::min<uint64_t>((uint64_t)c->sm_count * 8, (n + 255) / 256);
+
+  // The array keeps whatever the last call (of any context) left in it.  Counters and histogram must start at zero; the
+  // records, keys and permutation are written before they are read.
+  MT_CUDA(c, cudaMemsetAsync(base, 0, zero_b, stream));
+  P.live_out_count = counts;                               // counts[s] = muons entering pass s
+  MT_CUDA(c, mt_launch_wave_bin(P, aux_grid, stream));
+  MT_CUDA(c, mt_launch_wave_sort(P, n_keys, aux_grid, stream));
+  c->launches += 3;
+  const int sort_every = c->opt_sort_every > 0 ? c->opt_sort_every : 1;
+  for (int s = 0; s < n_pass; ++s) {
+    P.live_in_count = counts + s;
+    P.live_out_count = counts + s + 1;
+    P.work_counter = work + s;
+    P.first_pass = (s == 0);
+    P.sorted_in = (s % sort_every) == 0;
+    P.sort_out = (s < n_pass - 1) && ((s + 1) % sort_every) == 0;
+    P.rec_in = rec[(s + 1) & 1];
+    P.rec_out = rec[s & 1];
+    P.slab_z_end = (s == n_pass - 1) ? INFINITY : (float)((double)c->geom.z_min + (double)(s + 1) * pl.slab);
+    P.lean_z_hi = std::min(c->lean_box[5], P.slab_z_end);
+    MT_CUDA(c, mt_launch_transport(P, cfg, stream));
+    c->launches += 1;
+    if (P.sort_out) {
+      MT_CUDA(c, mt_launch_wave_sort(P, n_keys, aux_grid, stream));
+      c->launches += 2;
+    }
+  }
+  return MT_OK;
+}
+
+}  // namespace
+
+extern "C" int mt_transport_static_scratch(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base, uint64_t seed,
+                                           const mt_muons_out* out, void* cuda_stream) {
+  if (!c || !in || !out) return MT_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  return guarded(c, [&] { return run_transport_static_scratch(c, in, n, id_base, seed, out, (cudaStream_t)cuda_stream); });
+}
