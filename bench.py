@@ -49,11 +49,42 @@ def variant_work(mode, field_mode=0, joint=False):
     if joint:
         ops += -6 + 3 - 23 + 8
     return ops, gb
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ALL launches of the dominant kernel in one 10^7-muon
-# batch of config 3, summed over the batch's z-slab passes from the ncu launch list profiles/r2c_dram_launches.csv
-# (profiles/r2c_summary.md has the command); None where no capture exists.  bench.py cannot run ncu itself.
-NCU_DRAM_BYTES_PER_BATCH = {"voxel": 27.71e9, "regions": None, "poly": None}     # 20.14 GB read + 7.57 GB written, 32 passes
-NCU_DRAM_SOURCE = "profiles/r2c_dram_launches.csv"
+# Work the host and the grid repack do once, which the counting rules above still charge to every step: the 18 Philox
+# round-key increments (host-made, every mode) and the 12 x-differences of the trilinear corners (stored in the repacked
+# grid).  `frac` is quoted on the full algorithmic count; `frac_without_precomputed` on the count minus these.
+PRECOMPUTED_OPS = {"philox_round_keys": 18, "trilinear_x_differences": 12}
+
+# The ncu launch list of one timed step (per-launch time, DRAM bytes, L2 bytes, L1 sectors, L1 data-stage wavefronts,
+# warp instructions), committed as text; profiles/r3_launches.md names the command.  bench.py cannot run ncu itself: it
+# READS this file, and uses it only for a run of the very configuration it was captured on — anything else gets null.
+NCU_LAUNCH_LIST = "profiles/r3_launches.csv"
+NCU_CAPTURE_CONFIG = dict(config=3, muons=10_000_000, field_mode=0, joint=False, poly=False, sched=0, placement=0, block=0,
+                          slab=0, lanes=0, sort_every=0, pass_mode=0, no_lean=False, blocks_per_sm=0, min_idle=0,
+                          draws=1_000_000)
+
+
+def ncu_capture(args):
+    """Sums over the launches of each kernel in NCU_LAUNCH_LIST, or None if this run is not the captured configuration
+    (or the file is missing / unreadable)."""
+    if any(getattr(args, k) != v for k, v in NCU_CAPTURE_CONFIG.items()):
+        return None
+    import csv
+    try:
+        with open(os.path.join(ROOT, NCU_LAUNCH_LIST), newline="") as f:
+            rows = list(csv.DictReader(f))
+    except OSError:
+        return None
+    agg = {}
+    for r in rows:
+        name = r["kernel"].replace("void ", "").split("<")[0].split("(")[0]
+        a = agg.setdefault(name, {"launches": 0})
+        a["launches"] += 1
+        for k, v in r.items():
+            if k.endswith(".sum") and v != "":
+                a[k] = a.get(k, 0.0) + float(v)
+    return agg or None
+
+
 SM_COUNT, LANES_PER_SM = 148, 128          # B200: 4 SMSPs x 32 lanes issue one warp instruction per clock
 
 
@@ -122,63 +153,131 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------------------------ roofline
 def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_muons, grid_bytes, peaks, mp, field_mode=0,
-                   joint=False):
+                   joint=False, capture=None, probe_clocks=None):
     """north_star's roofline for one step of this rank: "the larger of FP32-issue time ... at peak and gather bytes at
-    L2/HBM bandwidth", with both terms, against peaks MEASURED in this process (mt_measure_peaks: csrc/mt_probe.cu) and
-    the nominal issue peak beside them.  DESIGN.md §7 derives the per-muon-step figures."""
+    L2/HBM bandwidth".  Every term that can be evaluated for this run is evaluated, `bound` is the LARGEST of them, and
+    `achieved` / `peak` / `frac` are that term's.  Terms:
+      alu            algorithmic thread-operations at the nominal issue peak, one per lane per clock — the
+                     peak DESIGN.md derives from unit counts and the measured sm_max_mhz; `frac_nominal` is this term's
+                     fraction whatever binds (the figure comparable across rounds)
+      hbm            compulsory HBM bytes (muon state in and out + the field grid once) at the measured copy bandwidth
+      l1 / l2 / dram L1 data-stage wavefronts at one per SM per clock, L2 bytes at the L2 random-sector rate measured in
+                     this process, DRAM bytes at the measured copy bandwidth — MEASURED traffic of the dominant kernel from
+                     the committed ncu launch list, only when this run is the configuration that list was captured on
+    mp: mt_measure_peaks of this process, or None if the probe failed (then only nominal / driver-measured peaks are used).
+    The per-lane gather estimate (every lane's record a sector of its own) is printed as an upper estimate and takes no
+    part in `bound`: lanes of a sorted warp share sectors."""
     ops_step, gb_step = variant_work(mode, field_mode, joint)
+    pre = PRECOMPUTED_OPS["philox_round_keys"] + (PRECOMPUTED_OPS["trilinear_x_differences"]
+                                                  if mode == "voxel" and not (field_mode & 1) else 0)
     ops = steps_per_call * ops_step                                        # thread-operations per step
-    gbytes = steps_per_call * gb_step                                      # gathered bytes per step
-    nominal = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6           # thread-ops/s: one per lane per clock
-    measured = mp["ffma_thread_ops_per_s"]                                 # a pure FFMA stream on this device, now
+    gbytes = steps_per_call * gb_step                                      # gathered bytes per step, one sector per lane
+    clock_hz = peaks["sm_max_mhz"] * 1e6
+    nominal = SM_COUNT * LANES_PER_SM * clock_hz                           # thread-ops/s: one per lane per clock
+    hbm_bps = peaks["hbm_gbs"] * 1e9
     per_lane = launches_per_step // max(lanes, 1)
     passes = lanes * ((per_lane - 3) // 3 + 1 if per_lane > 3 else per_lane)      # launches of the transport kernel
-    t_issue, t_issue_nominal = ops / measured, ops / nominal
-    t_gather = {"l1_resident_64k": gbytes / mp["gather_l1_bytes_per_s"], "l2_resident_64m": gbytes / mp["gather_64m_bytes_per_s"],
-                "hbm_1400m": gbytes / mp["gather_1400m_bytes_per_s"]}
-    # compulsory HBM traffic: 32 B in + 32 B out per muon, and the part of the field grid the batch touches, once
-    state_bytes = 64 * n_muons + grid_bytes
-    dram = NCU_DRAM_BYTES_PER_BATCH[mode]
-    return {
-        "bound": "alu", "unit": "T thread-ops/s",
-        "achieved": ops / t_call_s / 1e12, "peak": measured / 1e12, "frac": t_issue / t_call_s,
-        "peak_nominal": nominal / 1e12, "frac_nominal": t_issue_nominal / t_call_s,
-        "peak_source": "measured in this process: mt_measure_peaks, fma.rn.f32 stream, 8 warps per scheduler "
-                       "(nominal = 148 SM x 128 lanes x %s sm_max_mhz %.0f)" % (peaks["source"], peaks["sm_max_mhz"]),
+    state_bytes = 64 * n_muons + grid_bytes                                # compulsory HBM traffic
+    dominant = "wave_transport_kernel" if per_lane > 1 else "transport_kernel"
+    cap = (capture or {}).get(dominant)
+    if cap and cap["launches"] != passes:
+        cap = None                                                         # not the launch sequence that was captured
+
+    # ---- the terms (seconds per step), each with what was achieved and the peak it is held against
+    terms = {"alu": dict(t=ops / nominal, achieved=ops / t_call_s / 1e12, peak=nominal / 1e12, unit="T thread-ops/s",
+                         basis="algorithmic ops, nominal issue peak 148 SM x 128 lanes x sm_max_mhz"),
+             "hbm": dict(t=state_bytes / hbm_bps, achieved=state_bytes / t_call_s / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
+                         basis="compulsory bytes, %s copy bandwidth" % peaks["source"])}
+    if cap:
+        wf = cap.get("l1tex__data_pipe_lsu_wavefronts.sum")
+        if wf:
+            terms["l1"] = dict(t=wf / (SM_COUNT * clock_hz), achieved=wf / t_call_s / 1e9, peak=SM_COUNT * clock_hz / 1e9,
+                               unit="G wavefronts/s", basis="measured L1 data-stage wavefronts (ncu), one per SM per clock")
+        l2b = cap.get("lts__t_bytes.sum")
+        if l2b and mp:
+            terms["l2"] = dict(t=l2b / mp["gather_64m_bytes_per_s"], achieved=l2b / t_call_s / 1e9,
+                               peak=mp["gather_64m_bytes_per_s"] / 1e9, unit="GB/s",
+                               basis="measured L2 bytes (ncu), random-sector L2 rate measured in this process")
+        db = cap.get("dram__bytes_read.sum", 0.0) + cap.get("dram__bytes_write.sum", 0.0)
+        if db:
+            terms["dram"] = dict(t=db / hbm_bps, achieved=db / t_call_s / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
+                                 basis="measured DRAM bytes (ncu), %s copy bandwidth" % peaks["source"])
+    bound = max(terms, key=lambda k: terms[k]["t"])
+    top = terms[bound]
+    frac = top["t"] / t_call_s
+    ranked = sorted(terms, key=lambda k: -terms[k]["t"])
+    reading = "largest term: %s, %.1f of %.1f ms measured (%.2f); then %s" % (
+        bound, 1e3 * top["t"], 1e3 * t_call_s, frac,
+        ", ".join("%s %.1f ms" % (k, 1e3 * terms[k]["t"]) for k in ranked[1:]))
+    if frac < 0.5:
+        reading += ("; no throughput term reaches half of the measured time: with %d muons on %d SMs the call is bound by the "
+                    "latency of one history's dependent steps and by the tails of its launches, not by a unit" % (n_muons, SM_COUNT))
+    if not cap:
+        reading += "; no ncu capture of this configuration: the l1 / l2 / dram terms are not evaluated"
+    dram = terms["dram"]["t"] * hbm_bps if "dram" in terms else None
+    out = {
+        "bound": bound, "unit": top["unit"], "achieved": top["achieved"], "peak": top["peak"], "frac": frac,
+        "peak_source": top["basis"],
+        "frac_nominal": terms["alu"]["t"] / t_call_s, "peak_nominal": nominal / 1e12,
+        "frac_nominal_is": "algorithmic thread-ops (%d per muon-step) over the nominal issue peak; the same figure as "
+                           "BENCH_r01 / r02's frac_nominal" % ops_step,
+        "frac_without_precomputed": (ops_step - pre) / ops_step * terms["alu"]["t"] / t_call_s,
+        "ops_per_muon_step": ops_step, "ops_per_muon_step_without_precomputed": ops_step - pre,
+        "gather_bytes_per_muon_step": gb_step,
         "kernel": ("wave_transport_kernel: %d z-slab passes (%d lane(s)) among the %d launches of a step (the rest sort "
                    "the live list)" % (passes, lanes, launches_per_step)) if per_lane > 1 else
                   "transport_kernel (%d launch(es) per step)" % launches_per_step,
-        "ops_per_muon_step": ops_step, "gather_bytes_per_muon_step": gb_step,
-        "terms_ms": {
-            "measured": 1e3 * t_call_s,
-            "t_issue_at_measured_ffma_peak": 1e3 * t_issue, "t_issue_at_nominal_peak": 1e3 * t_issue_nominal,
-            "t_gather_if_every_record_came_from": {k: 1e3 * v for k, v in t_gather.items()},
-            "reading": "the issue term binds.  The gather terms price every lane's record as a separate 32-byte sector "
-                       "at the random-sector rate of that level; a term above the measured time means the schedule does "
-                       "not pay it: the sorted wavefront makes a warp's lanes share sectors, the alias tables are served "
-                       "from L1 and the field grid (which does not allocate in L1) from the L2-resident z-slab (ncu: L2 hit "
-                       "93-95 %, 778 GB of L2 traffic per batch = 5.6 TB/s, DRAM 3 % busy)"},
-        "gather_tb_per_s": gbytes / t_call_s / 1e12,
-        "measured_peaks": {"ffma_T_thread_ops_per_s": measured / 1e12, "lop3_T": mp["lop3_thread_ops_per_s"] / 1e12,
-                           "imad_T": mp["imad_thread_ops_per_s"] / 1e12, "mulhi_T": mp["mulhi_thread_ops_per_s"] / 1e12,
-                           "mufu_T": mp["mufu_thread_ops_per_s"] / 1e12,
-                           # mixed streams as a fraction of the fma rate: near 1 = that pipe runs beside the FP32 stream,
-                           # 0.75 / 0.625 = its instructions take 2 / 4 FP32 issue cycles each (DESIGN.md §7)
-                           "mix_over_ffma": {"8_fma_4_lop3": mp["mix_ffma8_lop3_4_thread_ops_per_s"] / measured,
-                                             "8_fma_4_imad": mp["mix_ffma8_imad4_thread_ops_per_s"] / measured,
-                                             "8_fma_2_mulwide": mp["mix_ffma8_mulwide2_thread_ops_per_s"] / measured},
-                           "gather_TB_per_s": {"l1_resident_64k": mp["gather_l1_bytes_per_s"] / 1e12,
-                                               "l2_resident_675k": mp["gather_675k_bytes_per_s"] / 1e12,
-                                               "l2_resident_64m": mp["gather_64m_bytes_per_s"] / 1e12,
-                                               "hbm_1400m": mp["gather_1400m_bytes_per_s"] / 1e12},
-                           "hbm_copy_gbs_%s" % peaks["source"]: peaks["hbm_gbs"]},
+        "terms_ms": dict({"measured": 1e3 * t_call_s}, **{k: 1e3 * v["t"] for k, v in terms.items()}),
+        "terms_basis": {k: v["basis"] for k, v in terms.items()},
+        "reading": reading,
+        "ncu_capture": NCU_LAUNCH_LIST if cap else None,
         "traffic": (dram / passes) if dram else None,
-        "traffic_unit": "DRAM bytes per launch of the kernel = per-batch total / passes (ncu, %s)" % NCU_DRAM_SOURCE,
+        "traffic_unit": "DRAM bytes per launch of the kernel = per-step total / passes (ncu launch list)",
         "traffic_per_batch": dram,
         "algorithmic_hbm_bytes_per_batch": state_bytes,
         "algorithmic_hbm_bytes_note": "64 B of state per muon + the library's 32-byte-per-cell field grid read once",
         "traffic_over_algorithmic": (dram / state_bytes) if dram else None,
     }
+    if cap:
+        steps32 = steps_per_call / 32.0
+        out["measured_per_warp_step"] = {
+            "basis": "ncu launch list / (muon-steps / 32); a warp-step here is 32 muon-steps, whatever the lanes' activity",
+            "l1_wavefronts": cap.get("l1tex__data_pipe_lsu_wavefronts.sum", 0.0) / steps32,
+            "l1_sectors": cap.get("l1tex__t_sectors.sum", 0.0) / steps32,
+            "l2_sectors": cap.get("lts__t_sectors.sum", 0.0) / steps32,
+            "warp_instructions": cap.get("smsp__inst_executed.sum", 0.0) / steps32,
+            "by_source": "profiles/r3_l1_sources.md"}
+    if mp:
+        measured = mp["ffma_thread_ops_per_s"]                             # a pure FFMA stream on this device, now
+        out["frac_measured"] = ops / measured / t_call_s
+        out["peak_measured"] = measured / 1e12
+        out["peak_measured_source"] = ("mt_measure_peaks in this process after the timed region: fma.rn.f32 stream, 8 warps "
+                                       "per scheduler; SM clock while it ran: %s"
+                                       % (probe_clocks if probe_clocks is not None else "not sampled"))
+        out["gather_one_sector_per_lane_upper_ms"] = {
+            "note": "every lane's record priced as a 32-byte sector of its own at that level's random-sector rate; an upper "
+                    "estimate that takes no part in `bound`",
+            "l1_resident_64k": 1e3 * gbytes / mp["gather_l1_bytes_per_s"],
+            "l2_resident_64m": 1e3 * gbytes / mp["gather_64m_bytes_per_s"],
+            "hbm_1400m": 1e3 * gbytes / mp["gather_1400m_bytes_per_s"]}
+        out["measured_peaks"] = {
+            "ffma_T_thread_ops_per_s": measured / 1e12, "lop3_T": mp["lop3_thread_ops_per_s"] / 1e12,
+            "imad_T": mp["imad_thread_ops_per_s"] / 1e12, "mulhi_T": mp["mulhi_thread_ops_per_s"] / 1e12,
+            "mufu_T": mp["mufu_thread_ops_per_s"] / 1e12,
+            # mixed streams as a fraction of the fma rate: near 1 = that pipe runs beside the FP32 stream,
+            # 0.75 / 0.625 = its instructions take 2 / 4 FP32 issue cycles each (DESIGN.md §7)
+            "mix_over_ffma": {"8_fma_4_lop3": mp["mix_ffma8_lop3_4_thread_ops_per_s"] / measured,
+                              "8_fma_4_imad": mp["mix_ffma8_imad4_thread_ops_per_s"] / measured,
+                              "8_fma_2_mulwide": mp["mix_ffma8_mulwide2_thread_ops_per_s"] / measured},
+            "gather_TB_per_s": {"l1_resident_64k": mp["gather_l1_bytes_per_s"] / 1e12,
+                                "l2_resident_675k": mp["gather_675k_bytes_per_s"] / 1e12,
+                                "l2_resident_64m": mp["gather_64m_bytes_per_s"] / 1e12,
+                                "hbm_1400m": mp["gather_1400m_bytes_per_s"] / 1e12},
+            "hbm_copy_gbs_%s" % peaks["source"]: peaks["hbm_gbs"]}
+    else:
+        out["measured_peaks"] = None
+        out["measured_peaks_note"] = "mt_measure_peaks failed in this process: nominal and driver-measured peaks only"
+    return out
 
 
 # ------------------------------------------------------------------------------------------ workload
@@ -372,8 +471,18 @@ def run_ours(args, rank, world, local_rank):
     peaks = load_peaks()
     value = steps_all * args.steps / t_dev_max
     e2e_value = steps_all * e2e_steps / t_e2e_max
+    # The probe runs after the timed region (1.4 GB of its own, ~50 ms): a failure there must not cost the line, and the
+    # clock it ran at is recorded beside the peak it gives
+    mp, probe_clocks = None, None
+    try:
+        probe_sampler = ClockSampler(local_rank).start()
+        for _ in range(3):                                    # (long enough for a few 100 ms clock samples)
+            mp = b.mt_measure_peaks(local_rank)
+        probe_clocks = probe_sampler.stop().get("sm_mhz")
+    except Exception as e:                                    # MtError, OSError from nvidia-smi, ...
+        log("[bench] peak probe failed (%s): nominal peaks only" % e)
     roofline = roofline_block(mode, steps_per_call, t_dev / args.steps, max(1, launches // args.steps), lanes_used, n,
-                              grid_bytes, peaks, b.mt_measure_peaks(local_rank), args.field_mode, args.joint)
+                              grid_bytes, peaks, mp, args.field_mode, args.joint, ncu_capture(args), probe_clocks)
     line = {
         "metric": "muon_steps_per_s", "value": value, "unit": "muon-steps/s",
         "muons_per_s": muons_all * args.steps / t_dev_max,

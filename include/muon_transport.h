@@ -133,7 +133,8 @@ typedef struct {
 int mt_load_histograms(mt_ctx* ctx, const mt_hist_desc* desc);
 
 /* Build the alias tables (Walker/Vose; construction order DESIGN.md §3.9), pack them
- * and upload them.  MT_ERR_EMPTY_HIST names the offending table in mt_last_error(). */
+ * and upload them.  MT_ERR_EMPTY_HIST names the offending table in mt_last_error().  A failed call leaves the context
+ * without tables (the previous ones are not kept): MT_ERR_STATE from mt_set_geometry / mt_transport until it succeeds. */
 int mt_build_alias(mt_ctx* ctx, int placement);
 
 /* Test export of the tables as built: HOST outputs shaped like counts_dp / counts_th.  JOINT mode: prob_dp / alias_dp
@@ -186,7 +187,9 @@ typedef struct {
  * returns.  The library's copy takes 32 bytes per cell of the grid padded by one cell on every side.
  * On failure: an argument error found before anything is touched leaves the previous geometry in place; a failure
  * after the library's grid has been overwritten (a material id above n_materials in d_material, a CUDA error) leaves
- * the context WITHOUT a geometry, and mt_transport then returns MT_ERR_STATE until mt_set_geometry succeeds.
+ * the context WITHOUT a geometry, and mt_transport then returns MT_ERR_STATE until mt_set_geometry succeeds.  If the
+ * failure is a CUDA error while the tables are re-uploaded in the new geometry's material order, the tables are gone as
+ * well (mt_build_alias, then mt_set_geometry).
  * mt_load_histograms invalidates the tables and the geometry; mt_build_alias keeps a geometry that is set. */
 int mt_set_geometry(mt_ctx* ctx, const mt_geometry* geom);
 

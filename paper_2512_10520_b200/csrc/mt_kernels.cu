@@ -2,8 +2,13 @@
 // transport kernel for a launch configuration, and all launchers (sm_100a).  The transport kernels themselves are the
 // templates of mt_kernels.cuh, instantiated in the mt_inst_*.cu files.
 #include <cuda_runtime.h>
-#include <algorithm>
+#include <limits.h>
 #include <stdint.h>
+#include <algorithm>
+#include <map>
+#include <mutex>
+#include <tuple>
+#include <utility>
 #include "mt_kernels.cuh"
 
 namespace {
@@ -197,45 +202,105 @@ bool mt_has_lean(int mode, const MtLaunchCfg& cfg) {
 // ------------------------------------------------------------------------------------------------
 // launchers (called from mt_lib.cu)
 // ------------------------------------------------------------------------------------------------
-cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream) {
-  mt_kernel_fn fn = pick_kernel(P.mode, cfg);
-  cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
+// Function attributes of the transport kernels.  Both the dynamic shared-memory limit and the preferred carveout are state
+// of (device, kernel), shared by every context and thread of the process, and an occupancy query answers for whatever is
+// set at that moment.  So what is set is tracked here per (device, kernel) under one lock, the plan of a launch
+// configuration — its occupancy with shared memory unrestricted and the carveout sized from it — is worked out once per
+// (device, kernel, block, shared bytes) and kept, and an attribute is written only when it has to change: after the first
+// call at a configuration neither mt_occupancy nor a launch touches the attributes again (a z-slab batch used to make
+// two cudaFuncSetAttribute calls per pass and five resetting probes per call).
+namespace {
+
+struct FnPlanKey {
+  int device; const void* fn; unsigned block; size_t smem;
+  bool operator<(const FnPlanKey& o) const {
+    return std::tie(device, fn, block, smem) < std::tie(o.device, o.fn, o.block, o.smem);
+  }
+};
+struct FnPlan { int occ, carve; };
+struct FnApplied { long long smem = -1; int carve = INT_MIN; };       // what the (device, kernel) attributes hold now
+
+std::mutex g_fn_lock;
+std::map<FnPlanKey, FnPlan> g_fn_plans;
+std::map<std::pair<int, const void*>, FnApplied> g_fn_applied;
+
+cudaError_t apply_attrs(int device, const void* fn, size_t smem, int carve) {
+  FnApplied& a = g_fn_applied[std::make_pair(device, fn)];
+  if (a.smem != (long long)smem) {
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    a.smem = (long long)smem;
+  }
+  if (a.carve != carve) {
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+    if (e != cudaSuccess) return e;
+    a.carve = carve;
+  }
+  return cudaSuccess;
+}
+
+// (caller holds g_fn_lock)
+cudaError_t fn_plan(const void* fn, unsigned block, size_t smem, int* device_out, FnPlan* out) {
+  int device = 0;
+  cudaError_t e = cudaGetDevice(&device);
+  if (e != cudaSuccess) return e;
+  *device_out = device;
+  const FnPlanKey key = {device, fn, block, smem};
+  auto it = g_fn_plans.find(key);
+  if (it != g_fn_plans.end()) { *out = it->second; return cudaSuccess; }
+  // the occupancy wanted is the one with shared memory unrestricted: the carveout is sized from it
+  e = apply_attrs(device, fn, smem, (int)cudaSharedmemCarveoutDefault);
+  if (e != cudaSuccess) return e;
+  FnPlan plan = {0, (int)cudaSharedmemCarveoutDefault};
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&plan.occ, fn, (int)block, smem);
   if (e != cudaSuccess) return e;
   // As much L1 as the resident CTAs' shared memory leaves: the alias tables live there (mt_step.cuh: MT_GRID_HINT).  The
   // carveout is a preference the driver may honour at the cost of occupancy, so it is sized for the number of CTAs that fit
   // an SM when shared memory is not restricted (1 KB per CTA is the system's own), never below that.
-  {
-    struct Key { const void* fn; unsigned block; size_t smem; int carve; };
-    static thread_local Key last = {nullptr, 0u, 0, 0};
-    if (last.fn != (const void*)fn || last.block != cfg.block || last.smem != cfg.smem_bytes) {
-      e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutDefault);
-      if (e != cudaSuccess) return e;
-      int occ = 0;
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)fn, (int)cfg.block, cfg.smem_bytes);
-      if (e != cudaSuccess) return e;
-      const size_t need = (size_t)std::max(occ, 1) * (cfg.smem_bytes + 1024);
-      // the SM's shared-memory configurations (KB); the preference is a percentage of 228 KB that the driver rounds UP to
-      // one of them, so the smallest configuration that holds `need` is asked for by its own size rounded DOWN to a percent
-      static const int kb[] = {8, 16, 32, 64, 100, 132, 164, 196, 228};
-      int pick = 228;
-      for (int c : kb) if ((size_t)c * 1024 >= need) { pick = c; break; }
-      last = {(const void*)fn, cfg.block, cfg.smem_bytes, std::max(1, pick * 100 / 228)};
-    }
-    e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout, last.carve);
-    if (e != cudaSuccess) return e;
+  int sm_bytes = 0;
+  e = cudaDeviceGetAttribute(&sm_bytes, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device);
+  if (e != cudaSuccess) return e;
+  const size_t need = (size_t)std::max(plan.occ, 1) * (smem + 1024);
+  if (sm_bytes == 228 * 1024) {
+    // sm_100's shared-memory configurations (KB); the preference is a percentage of the SM's 228 KB that the driver rounds
+    // UP to one of them, so the smallest configuration that holds `need` is asked for by its own size rounded DOWN to a percent
+    static const int kb[] = {8, 16, 32, 64, 100, 132, 164, 196, 228};
+    int pick = 228;
+    for (int c : kb) if ((size_t)c * 1024 >= need) { pick = c; break; }
+    plan.carve = std::max(1, pick * 100 / 228);
+  } else if (sm_bytes > 0) {
+    // another SM: its configurations are not known here; ask for the share that holds `need` (the driver rounds up)
+    plan.carve = (int)std::min<size_t>(100, std::max<size_t>(1, (need * 100 + (size_t)sm_bytes - 1) / (size_t)sm_bytes));
   }
+  g_fn_plans[key] = plan;
+  *out = plan;
+  return cudaSuccess;
+}
+
+}  // namespace
+
+cudaError_t mt_launch_transport(const MtParams& P, const MtLaunchCfg& cfg, cudaStream_t stream) {
+  mt_kernel_fn fn = pick_kernel(P.mode, cfg);
+  std::lock_guard<std::mutex> lock(g_fn_lock);              // attributes and launch as one step: another thread's launch of
+  int device = 0;                                           // the same kernel may want other values
+  FnPlan plan;
+  cudaError_t e = fn_plan((const void*)fn, cfg.block, cfg.smem_bytes, &device, &plan);
+  if (e != cudaSuccess) return e;
+  e = apply_attrs(device, (const void*)fn, cfg.smem_bytes, plan.carve);
+  if (e != cudaSuccess) return e;
   void* args[] = {(void*)&P};
   return cudaLaunchKernel((const void*)fn, dim3(cfg.grid), dim3(cfg.block), args, cfg.smem_bytes, stream);
 }
 
 cudaError_t mt_occupancy(const MtParams& P, const MtLaunchCfg& cfg, int* blocks_per_sm) {
   mt_kernel_fn fn = pick_kernel(P.mode, cfg);
-  cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem_bytes);
+  std::lock_guard<std::mutex> lock(g_fn_lock);
+  int device = 0;
+  FnPlan plan;
+  cudaError_t e = fn_plan((const void*)fn, cfg.block, cfg.smem_bytes, &device, &plan);
   if (e != cudaSuccess) return e;
-  // (the answer wanted is the one with shared memory unrestricted: mt_launch_transport sizes the carveout from it)
-  e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutDefault);
-  if (e != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, (const void*)fn, cfg.block, cfg.smem_bytes);
+  *blocks_per_sm = plan.occ;
+  return cudaSuccess;
 }
 
 cudaError_t mt_launch_wave_bin(const MtParams& P, unsigned grid, cudaStream_t stream) {

@@ -21,9 +21,6 @@ namespace {
 using namespace mt;
 
 enum { SCHED_STATIC = 1, SCHED_REFILL = 2, SCHED_WAVEFRONT = 3 };
-#ifndef MT_STEPS_PER_VOTE
-#define MT_STEPS_PER_VOTE 2
-#endif
 // Muon records stream: a pass reads each once and writes each survivor once, 480 MB at the first pass against 126 MB of
 // L2 that should keep the slab's field layers, so they go through cache-streaming (evict-first) loads and stores
 // (ld.global.cs / st.global.cs: 142.6 -> 142.1 ms per 10^7 muons; -DMT_NO_STREAM restores plain accesses).

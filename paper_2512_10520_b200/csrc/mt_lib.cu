@@ -602,6 +602,9 @@ static int build_alias_impl(mt_ctx* c, int placement) {
   const size_t nt = (size_t)c->n_materials * c->n_pbins;
   const bool joint = (c->hist_mode == MT_HIST_JOINT);
   const int n_dp = joint ? c->n_dp * c->n_th : c->n_dp, n_th = joint ? 0 : c->n_th;   // JOINT: one table of n_dp * n_th cells
+  // From here on the host copies, the packed device tables and the blob are rewritten one after the other: until all three
+  // are done the context has NO tables (a failure on the way must not leave mt_transport running new sizes over old data)
+  c->have_tables = false;
   c->prob_dp.assign(nt * n_dp, 0.0f); c->alias_dp.assign(nt * n_dp, 0u);
   c->prob_th.assign(nt * n_th, 0.0f); c->alias_th.assign(nt * n_th, 0u);
   for (size_t t = 0; t < nt; ++t) {
@@ -617,8 +620,9 @@ static int build_alias_impl(mt_ctx* c, int placement) {
   int rc = upload_tables(c);
   if (rc != MT_OK) return rc;
   c->placement = placement;
-  c->have_tables = true;
-  return rebuild_blob(c);
+  rc = rebuild_blob(c);
+  c->have_tables = (rc == MT_OK);
+  return rc;
 }
 
 int mt_get_alias(const mt_ctx* c, float* prob_dp, uint32_t* alias_dp, float* prob_th, uint32_t* alias_th) {
@@ -728,12 +732,15 @@ static int set_geometry_impl(mt_ctx* c, const mt_geometry* gm) {
   c->blocks.swap(blks);
   c->geom.n_regions = (int32_t)c->regions.size();
   c->geom.n_blocks = (int32_t)c->blocks.size();
-  c->have_geom = true;
+  c->have_geom = true;                     // (rebuild_blob stages the regions / blocks of a geometry that is set)
   // the most-used materials come first in the packed tables, so that a shared-memory prefix holds them
   order_materials(c, weight);
-  const int rc = upload_tables(c);
-  if (rc != MT_OK) return rc;
-  return rebuild_blob(c);
+  int rc = upload_tables(c);
+  if (rc == MT_OK) rc = rebuild_blob(c);
+  // the header's promise: a failure after the swap leaves the context without a geometry (and, the tables having been
+  // reordered for it, without tables), never with the new region / block counts over the old device blob
+  if (rc != MT_OK) c->have_geom = c->have_tables = false;
+  return rc;
 }
 
 int mt_load_histograms(mt_ctx* c, const mt_hist_desc* d) { return guarded(c, [&] { return load_histograms_impl(c, d); }); }
@@ -1004,7 +1011,10 @@ int choose_lanes(const mt_ctx* c, uint64_t n, int sched, bool host_call) {
   // further lane costs ~1.3 ms of pass start-up and tails.  Device calls: two lanes let one lane's
   // passes fill the tails of the other's between 2^18 and 2^21 muons (+1 to +6 % with item-mode passes); above that a single lane's passes
   // are long enough that their tails do not matter (one lane is 1 % faster), below it there is nothing to overlap.
-  // REFILL and STATIC kernels run a muon's whole history in one launch: lanes only serialise them.
+  // REFILL and STATIC kernels run a muon's whole history in one launch: on a device call lanes only serialise them.  On
+  // a host-buffer call that is what is wanted under every schedule: the lanes' kernels run one after the other in stream-
+  // priority order (each sized for the whole machine), lane k + 1's inputs land while lane k computes and lane k's results
+  // leave while lane k + 1 computes.
   if (host_call && n >= ((uint64_t)1 << 21)) return 4;
   if (sched == MT_SCHED_WAVEFRONT && n >= ((uint64_t)1 << 18) && n < ((uint64_t)1 << 21)) return 2;
   return 1;
@@ -1103,6 +1113,10 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
     }
   }
 
+  // From the fork on, library streams hold work that the caller's stream has not been told to wait for: the fork, the
+  // launches and the join run inside `enqueue`, and if any of it fails the lanes are drained on the host before the error
+  // goes back (so a failed call never leaves kernels or copies running behind the caller's back on buffers it owns).
+  auto enqueue = [&]() -> int {
   // ---- fork: every lane (and the copy-in stream) starts where the caller's stream stands
   MT_CUDA(c, cudaEventRecord(c->ev_fork, stream));
   if (host) MT_CUDA(c, cudaStreamWaitEvent(c->copy_in, c->ev_fork, 0));
@@ -1192,6 +1206,14 @@ int run_transport(mt_ctx* c, const mt_muons_in* in, uint64_t n, uint64_t id_base
     MT_CUDA(c, cudaStreamWaitEvent(stream, L.done, 0));
   }
   return MT_OK;
+  };
+  rc = enqueue();
+  if (rc != MT_OK) {
+    if (host) cudaStreamSynchronize(c->copy_in);
+    for (int k = 0; k < K; ++k) cudaStreamSynchronize(lane_stream(k));
+    cudaGetLastError();                          // (the failure is already in last_error; leave no sticky-less error behind)
+  }
+  return rc;
 }
 
 }  // namespace
