@@ -9,8 +9,8 @@ roofline target is quoted on.  Rank r transports its own 10^7 muons (ids r*M ..)
 path (weak scaling).  One JSON line on stdout (rank 0); everything else goes to stderr.
 
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
-`--sweep` runs BASELINE.json configs[4] on one GPU instead (10^8 muons in batches of 10^7 at each table shape and
-placement, then muons-per-launch 2^14 .. 2^24) and prints one JSON line per point.
+`--sweep` runs BASELINE.json configs[4] instead (10^8 muons in batches of 10^7 at each table shape and placement — with
+`--gpus N` batch k on rank k % N — then, on one GPU, muons-per-launch 2^14 .. 2^24) and prints one JSON line per point.
 """
 import argparse
 import json
@@ -515,23 +515,36 @@ def run_ours(args, rank, world, local_rank):
 
 
 # ------------------------------------------------------------------------------------ configs[4] sweep
-def run_sweep(args):
-    """BASELINE.json configs[4] on one GPU: (A) 10^8 muons in 10 batches of 10^7 (id_base = batch * 10^7) for every
-    table shape x placement; (B) muons per launch 2^14 .. 2^24 on the middle shape.  One JSON line per point."""
+def run_sweep(args, rank, world, local_rank):
+    """BASELINE.json configs[4]: (A) 10^8 muons in 10 batches of 10^7 (id_base = batch * 10^7) for every table shape x
+    placement — with N ranks, batch k runs on rank k % N (sharding.batch_shard; replicated tables and grids, no collective
+    on the data path), a point's time is the MAX over ranks of each rank's summed device time and its muon-steps the SUM;
+    (B) muons per launch 2^14 .. 2^24 on the middle shape, one GPU by nature (rank 0 of a 1-rank job only).  One JSON line
+    per point, printed by rank 0."""
     import torch
+    import torch.distributed as dist
     from paper_2512_10520_b200 import binding as b, build as lib_build, workloads as w
+    from paper_2512_10520_b200.sharding import batch_shard, reduce_job
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the transport path has no CPU fallback")
-    lib_build.build()
-    dev = torch.device("cuda", 0)
-    torch.cuda.set_device(0)
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if rank == 0:
+        lib_build.build()
+    _, joined = join_ranks(args, rank, world, local_rank, "nccl")
+    if world > 1:
+        dist.barrier()
+    job = dist if world > 1 else None
     peaks = load_peaks()
-    alu_peak = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6
+    alu_peak = joined * SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6
     n_batch, n_batches = args.muons, args.sweep_batches
+    mine = batch_shard(n_batches, rank, world)
     stream = torch.cuda.Stream(device=dev)
     base = w.config3(n=8, device=dev)                        # grids once; histograms are regenerated per shape
-    out = {"pos_flag": torch.empty((n_batch, 4), dtype=torch.float32, device=dev),
-           "mom_steps": torch.empty((n_batch, 4), dtype=torch.float32, device=dev)}
+    n_launch_max = 1 << 24                                   # part (B)'s largest launch
+    n_out = max(n_batch, n_launch_max) if world == 1 else n_batch
+    out = {"pos_flag": torch.empty((n_out, 4), dtype=torch.float32, device=dev),
+           "mom_steps": torch.empty((n_out, 4), dtype=torch.float32, device=dev)}
 
     def timed(h, d_pos, d_mom, id_base, o):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -543,42 +556,52 @@ def run_sweep(args):
         return e0.elapsed_time(e1) * 1e-3, int(r["counters"][0].item())
 
     def emit(**kw):
+        if rank != 0:
+            return
+        kw["n_gpus"] = joined
         kw["roofline_frac_nominal"] = kw["muon_steps_per_s"] * ALG_OPS_PER_STEP["voxel"] / alu_peak
         print(json.dumps(kw), flush=True)
 
-    batches = [w.spectrum_muons(3, n_batch, "square", batch=k) for k in range(n_batches)]
+    batches = {k: w.spectrum_muons(3, n_batch, "square", batch=k) for k in mine}
+    o_batch = {k: v[:n_batch] for k, v in out.items()}
     for shape in w.CONFIG4_TABLE_SHAPES:
         t0 = time.time()
         hist = w.shield_histograms(3, [1.0, 1.0, 10.0], shape[0], shape[1], shape[2], args.sweep_draws)
-        log("[sweep] tables %dx%dx%d generated in %.1f s" % (shape + (time.time() - t0,)))
+        log("[sweep] rank %d: tables %dx%dx%d generated in %.1f s" % ((rank,) + shape + (time.time() - t0,)))
         for placement, pname in ((b.MT_PLACE_AUTO, "auto"), (b.MT_PLACE_L2, "l2"), (b.MT_PLACE_SMEM, "smem")):
-            h = b.MuonTransport(0)
+            h = b.MuonTransport(local_rank)
             try:
                 h.setup(hist, base.geom, placement)
                 h.set_option(b.MT_OPT_SCHEDULE, args.sched)
-                d0, m0 = torch.from_numpy(batches[0].pos_q).to(dev), torch.from_numpy(batches[0].mom).to(dev)
-                for _ in range(2):
-                    timed(h, d0, m0, 0, out)                 # warm-up
+                if mine:
+                    k0 = mine[0]
+                    d0, m0 = torch.from_numpy(batches[k0].pos_q).to(dev), torch.from_numpy(batches[k0].mom).to(dev)
+                    for _ in range(2):
+                        timed(h, d0, m0, k0 * n_batch, o_batch)      # warm-up
+                if world > 1:
+                    torch.cuda.synchronize()
+                    dist.barrier()
                 t_tot, s_tot = 0.0, 0
-                for k, mu in enumerate(batches):
-                    d_pos, d_mom = torch.from_numpy(mu.pos_q).to(dev), torch.from_numpy(mu.mom).to(dev)
-                    dt, st = timed(h, d_pos, d_mom, k * n_batch, out)
+                for k in mine:                                   # batch k of the job: generator batch k, ids from k * n_batch
+                    d_pos, d_mom = torch.from_numpy(batches[k].pos_q).to(dev), torch.from_numpy(batches[k].mom).to(dev)
+                    dt, st = timed(h, d_pos, d_mom, k * n_batch, o_batch)
                     t_tot += dt; s_tot += st
+                (t_max,), (s_all, m_all, b_all) = reduce_job([t_tot], [s_tot, n_batch * len(mine), len(mine)], job, dev)
                 emit(sweep="table_shape", pbins_x_dp_x_theta="%dx%dx%d" % shape, placement=pname,
-                     muons=n_batch * n_batches, batches=n_batches, muon_steps=s_tot, seconds=t_tot,
-                     muon_steps_per_s=s_tot / t_tot, muons_per_s=n_batch * n_batches / t_tot)
-            except b.MtError as e:
+                     muons=int(m_all), batches=int(b_all), batches_by_rank="batch k on rank k %% %d" % world,
+                     muon_steps=int(s_all), seconds=t_max, muon_steps_per_s=s_all / t_max, muons_per_s=m_all / t_max)
+            except b.MtError as e:                               # (the same refusal on every rank: no reduction to match)
                 emit(sweep="table_shape", pbins_x_dp_x_theta="%dx%dx%d" % shape, placement=pname,
                      muon_steps_per_s=0.0, unsupported=str(e))
             finally:
                 h.close()
-        if shape == w.CONFIG4_TABLE_SHAPES[1]:
-            h = b.MuonTransport(0).setup(hist, base.geom, b.MT_PLACE_AUTO)
+        if shape == w.CONFIG4_TABLE_SHAPES[1] and world == 1:
+            h = b.MuonTransport(local_rank).setup(hist, base.geom, b.MT_PLACE_AUTO)
             h.set_option(b.MT_OPT_SCHEDULE, args.sched)
-            d_pos, d_mom = torch.from_numpy(batches[0].pos_q).to(dev), torch.from_numpy(batches[0].mom).to(dev)
-            n_all = min(n_batch, 1 << 24)
+            mu = w.spectrum_muons(3, n_launch_max, "square", batch=0)     # 2^24 muons of their own: the last point is a real
+            d_pos, d_mom = torch.from_numpy(mu.pos_q).to(dev), torch.from_numpy(mu.mom).to(dev)      # 16 777 216-muon call
             for log2n in range(14, 25, 2):
-                n = min(1 << log2n, n_all)
+                n = 1 << log2n
                 o = {"pos_flag": out["pos_flag"][:n], "mom_steps": out["mom_steps"][:n]}
                 best, st = None, 0
                 for rep in range(4):
@@ -587,95 +610,11 @@ def run_sweep(args):
                 emit(sweep="muons_per_launch", pbins_x_dp_x_theta="%dx%dx%d" % shape, placement="auto", muons=n,
                      muon_steps=st, seconds=best, muon_steps_per_s=st / best, muons_per_s=n / best)
             h.close()
-
-
-def run_sweep_lanes(args):
-    """How a call is cut up (DESIGN.md §7 "lanes"): muons per call x slab thickness x concurrent lanes on config 3
-    (device-resident and host-buffer calls) and schedule x slab x lanes on configs 2, 2p and 1.  One JSON line per point;
-    best of `--steps` timed calls after one warm-up call."""
-    import torch
-    from paper_2512_10520_b200 import binding as b, build as lib_build, workloads as w
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the transport path has no CPU fallback")
-    lib_build.build()
-    dev = torch.device("cuda", 0)
-    torch.cuda.set_device(0)
-    stream = torch.cuda.Stream(device=dev)
-    nominal = SM_COUNT * LANES_PER_SM * load_peaks()["sm_max_mhz"] * 1e6
-
-    def timed(h, dq, dm, out):
-        best, steps = None, 0
-        for r in range(args.steps + 1):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            with torch.cuda.stream(stream):
-                e0.record(stream)
-                res = h.transport(dq, dm, 1, out=out, stream=stream)
-                e1.record(stream)
-                stream.synchronize()
-            steps = int(res["counters"][0].item())
-            if r > 0:
-                best = e0.elapsed_time(e1) if best is None else min(best, e0.elapsed_time(e1))
-        return best, steps
-
-    def timed_host(h, hq, hm, hout):
-        best = None
-        for r in range(args.steps + 1):
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            h.transport_host(hq, hm, 1, out=hout, stream=stream)
-            torch.cuda.synchronize()
-            if r > 0:
-                dt = (time.perf_counter() - t0) * 1e3
-                best = dt if best is None else min(best, dt)
-        return best
-
-    def emit(ops, ms, steps, **kw):
-        kw.update(ms=round(ms, 3), G_muon_steps_per_s=round(steps / ms / 1e6, 2), frac_nominal=round(steps / ms * 1e3 * ops / nominal, 3))
-        print(json.dumps(kw), flush=True)
-
-    wl = w.config3(n=8, device=dev, n_draws=args.draws)
-    mu = w.spectrum_muons(3, args.muons, "square")
-    h = b.MuonTransport(0).setup(wl.hist, wl.geom)
-    wl.geom.material = wl.geom.field = None
-    torch.cuda.empty_cache()
-    dq, dm = torch.from_numpy(mu.pos_q).to(dev), torch.from_numpy(mu.mom).to(dev)
-    out = {"pos_flag": torch.empty((len(dq), 4), device=dev), "mom_steps": torch.empty((len(dq), 4), device=dev)}
-    for n in sorted({min(1 << 18, args.muons), min(1 << 20, args.muons), min(1 << 22, args.muons), args.muons}):
-        o = {k: v[:n] for k, v in out.items()}
-        for slab in (0, 64, 128, 256):
-            for lanes, mode in ((0, 0), (1, 1), (1, 2), (2, 1), (2, 2), (4, 1), (4, 2)):
-                h.set_option(b.MT_OPT_LANES, lanes).set_option(b.MT_OPT_SLAB_CELLS, slab).set_option(b.MT_OPT_PASS_MODE, mode)
-                ms, st = timed(h, dq[:n], dm[:n], o)
-                emit(ALG_OPS_PER_STEP["voxel"], ms, st, workload="config3", call="device", muons=n, slab_cells=slab,
-                     lanes=lanes or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES),
-                     passes={0: "auto", 1: "persistent", 2: "item"}[mode])
-        h.set_option(b.MT_OPT_PASS_MODE, 0)
-    hq, hm = torch.from_numpy(mu.pos_q).pin_memory(), torch.from_numpy(mu.mom).pin_memory()
-    hout = {"pos_flag": torch.empty((len(hq), 4)).pin_memory(), "mom_steps": torch.empty((len(hq), 4)).pin_memory()}
-    h.set_option(b.MT_OPT_SLAB_CELLS, 0)
-    for lanes in (0, 1, 2, 4, 6, 8):
-        h.set_option(b.MT_OPT_LANES, lanes)
-        ms = timed_host(h, hq, hm, hout)
-        emit(ALG_OPS_PER_STEP["voxel"], ms, st, workload="config3", call="host (e2e)", muons=len(hq),
-             lanes=lanes or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES))
-    h.close()
-    del dq, dm, out, hq, hm, hout
-    torch.cuda.empty_cache()
-    for name, wl, mode in (("config2", w.config2(n=1_000_000, n_draws=args.draws), "regions"),
-                           ("config2p", w.config2p(n=1_000_000, n_draws=args.draws), "poly"),
-                           ("config1", w.config1(n=65536, n_draws=args.draws), "regions")):
-        h = b.MuonTransport(0).setup(wl.hist, wl.geom)
-        dq, dm = torch.from_numpy(wl.muons.pos_q).to(dev), torch.from_numpy(wl.muons.mom).to(dev)
-        out = {"pos_flag": torch.empty((len(dq), 4), device=dev), "mom_steps": torch.empty((len(dq), 4), device=dev)}
-        for sched in (0, 2, 3):
-            for slab in ((0,) if sched != 3 else (64, 128, 256)):
-                for lanes in ((0,) if sched == 0 else (1, 2, 4)):
-                    h.set_option(b.MT_OPT_SCHEDULE, sched).set_option(b.MT_OPT_LANES, lanes).set_option(b.MT_OPT_SLAB_CELLS, slab)
-                    ms, st = timed(h, dq, dm, out)
-                    emit(ALG_OPS_PER_STEP[mode], ms, st, workload=name, call="device", muons=len(dq),
-                         schedule=sched or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_SCHEDULE), slab_cells=slab,
-                         lanes=lanes or "auto=%d" % b.mt_get_info(h.ctx, b.MT_INFO_LAST_LANES))
-        h.close()
+            del d_pos, d_mom, mu
+    if world > 1:
+        torch.cuda.synchronize()
+        dist.barrier()
+        dist.destroy_process_group()
 
 
 def self_launch(n_gpus):
@@ -743,7 +682,6 @@ def main():
     ap.add_argument("--no-lean", action="store_true", help="MT_OPT_NO_LEAN: general kernels even where the lean variant applies")
     ap.add_argument("--poly", action="store_true", help="with --config 2: the convex-polyhedra shield (DESIGN.md 3.12)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
-    ap.add_argument("--sweep-lanes", action="store_true", help="lanes x slab x muons-per-call sweep (profiles/r2b_lanes.md)")
     ap.add_argument("--probes", action="store_true", help="only the in-process peak and field-path probes (one JSON line)")
     ap.add_argument("--draws", type=int, default=1_000_000, help="draws per generated histogram (BASELINE.json: 10^6)")
     ap.add_argument("--sweep-batches", type=int, default=10)
@@ -759,24 +697,21 @@ def main():
                           "field_paths_TB_per_s": {k[:3]: v * 32 / 1e12 for k, v in fp.items() if k.endswith("_per_s")},
                           "field_paths_records_per_launch": fp["records_per_launch"]}), flush=True)
         return
-    if args.sweep_lanes:
-        return run_sweep_lanes(args)
     if args.gpus < 1:
         raise SystemExit("bench.py: --gpus must be at least 1")
-    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not args.sweep:
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         self_launch(args.gpus)                                   # does not return
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if world != args.gpus and not args.sweep:
+    if world != args.gpus:
         # one rank per GPU or nothing: a line that says n_gpus = N must come from N ranks
         raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d (launch with --nproc-per-node %d, or drop the torchrun "
                          "environment and let bench.py start the ranks)" % (args.gpus, world, args.gpus))
     # every rank generates its own inputs: share the host cores instead of fighting for them
     os.environ.setdefault("MT_GEN_WORKERS", str(max(1, (os.cpu_count() or 1) // max(world, 1))))
     if args.sweep:
-        if rank == 0:
-            run_sweep(args)
+        run_sweep(args, rank, world, local_rank)
     elif args.impl == "reference":
         run_reference(args, rank, world)
     else:

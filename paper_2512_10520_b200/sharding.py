@@ -31,6 +31,15 @@ def strong_shard(n_total: int, rank: int, world: int) -> Shard:
     return Shard(rank, world, rank * q + min(rank, r), n)
 
 
+def batch_shard(n_batches: int, rank: int, world: int):
+    """A job made of whole batches (BASELINE.json configs[4]: 10^8 muons as ten batches of 10^7, batch k holding the ids
+    k * batch_size ..): batch k goes to rank k % world, so the ranks' batch counts differ by at most one and every batch
+    is run exactly once.  Returns this rank's batch indices, ascending; its id_base for batch k is k * batch_size."""
+    if not (0 <= rank < world) or n_batches < 0:
+        raise ValueError("bad shard request")
+    return list(range(rank, n_batches, world))
+
+
 def reduce_job(times_s, totals, dist=None, device=None):
     """Whole-job figures from per-rank ones: element-wise MAX of `times_s` (device-timed seconds) and SUM of
     `totals` (muon-steps, muons, ...) over the ranks of the default process group.  Returns two lists."""

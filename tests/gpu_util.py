@@ -2,6 +2,21 @@
 import numpy as np
 
 
+def need_device_memory(gib):
+    """The full-size parity tests need `gib` GiB free.  On a small development GPU they skip; on a B200-class device
+    (>= 150 GiB in all) too little free memory is a FAILURE: there the headline configurations must be checked, and a
+    silent skip would turn their parity into "untested"."""
+    import pytest
+    import torch
+    free, total = torch.cuda.mem_get_info()
+    if free >= gib * 2 ** 30:
+        return
+    msg = "needs %d GiB of device memory, %.1f GiB free of %.1f" % (gib, free / 2 ** 30, total / 2 ** 30)
+    if total >= 150 * 2 ** 30:
+        pytest.fail(msg + ": on this device the full-size parity tests must run")
+    pytest.skip(msg)
+
+
 def gpu_transport(mt, wl, sched=0, block=0, placement=0, id_base=0, exit_capacity=0, min_idle=0, slab=0,
                   sel=None, handle=None, lanes=0, pass_mode=0, lane_prio=0, sort_every=0):
     """Run workload `wl` on cuda:0 through the binding; returns numpy dict (pos, mom, flag, steps, ...)."""

@@ -9,7 +9,7 @@ import functools
 import numpy as np
 import pytest
 
-from gpu_util import compare, gpu_transport, ks_populations, oracle_transport
+from gpu_util import compare, gpu_transport, ks_populations, need_device_memory, oracle_transport
 
 pytestmark = pytest.mark.gpu
 
@@ -167,9 +167,7 @@ def test_config3_full_size_sampled(mt, oracle):
     import torch
     from paper_2512_10520_b200 import workloads as w
     b = mt.binding
-    free, _ = torch.cuda.mem_get_info()
-    if free < 12 * 2 ** 30:
-        pytest.skip("needs 12 GiB of device memory")
+    need_device_memory(12)
     wl = w.config3(device="cuda")
     n = len(wl.muons.pos_q)
     h = b.MuonTransport(0).setup(wl.hist, wl.geom)
@@ -228,9 +226,7 @@ def test_config4_full_size_sampled(mt, oracle, shape, batch):
     import torch
     from paper_2512_10520_b200 import workloads as w
     b = mt.binding
-    free, _ = torch.cuda.mem_get_info()
-    if free < 12 * 2 ** 30:
-        pytest.skip("needs 12 GiB of device memory")
+    need_device_memory(12)
     n = 10_000_000
     wl = w.config3(n=8, device="cuda", table_shape=shape, n_draws=200_000)
     wl.muons = w.spectrum_muons(3, n, "square", batch=batch)

@@ -53,6 +53,18 @@ def test_config3_small_contract_matches_libm_witness(oracle, workloads):
     check_against_witness(a, b, "config3 small (20000 muons, 80x80x750 grid)")
 
 
+def test_joint_mode_contract_matches_libm_witness(oracle, workloads):
+    """The same bar for the paper's joint 2D tables: there exp2c decodes BOTH sampled
+    values (the longitudinal loss fz and the transverse kick ft, which replaces the polar angle and its sine / cosine) and
+    the new |p| comes from one more square root — none of which the marginal-mode witness runs exercise."""
+    wl = workloads.config1(n=32768, n_draws=100_000, joint=True)
+    a, b = _both(oracle, wl)
+    check_against_witness(a, b, "config1 joint (32768 muons)")
+    wl = workloads.config3(n=20_000, n_draws=40_000, n_cells=2, half_width_cells=40, joint=True, table_shape=(100, 64, 32))
+    a, b = _both(oracle, wl)
+    check_against_witness(a, b, "config3 small joint (20000 muons, 80x80x750 grid)")
+
+
 def test_witness_in_double_is_the_physics_mode(oracle, workloads):
     """In float64 the polynomials (float32-accurate, ~1e-7) and libm differ at the 1e-7 level per sampled value, so the
     two double-precision runs agree on flag and step count for nearly every muon and on |p| to ~1e-6 relative:
