@@ -29,7 +29,10 @@ MT_STATIC_SCRATCH_MAX_MUONS, MT_STATIC_SCRATCH_BYTES = 65536, 9 * 1024 * 1024
 # every symbol include/muon_transport.h declares (tests check that the library exports each one)
 SYMBOLS = ["mt_strerror", "mt_last_error", "mt_create", "mt_destroy", "mt_set_option", "mt_load_histograms",
            "mt_build_alias", "mt_get_alias", "mt_set_geometry", "mt_transport", "mt_transport_host",
-           "mt_transport_static_scratch", "mt_launch_count", "mt_get_info", "mt_measure_peaks", "mt_probe_field_paths", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
+           "mt_transport_static_scratch", "mt_launch_count", "mt_get_info", "mt_debug_sample", "mt_debug_philox", "mt_debug_lookup"]
+# include/muon_probes.h: the measurement probes, in a library of their own (libmuon_probes.so) that the product never loads
+PROBES_LIB_PATH = os.path.join(HERE, "libmuon_probes.so")
+PROBE_SYMBOLS = ["mt_measure_peaks", "mt_probe_field_paths"]
 
 
 class mt_hist_desc(C.Structure):
@@ -115,13 +118,27 @@ def lib():
         L.mt_launch_count.restype = C.c_int64
         L.mt_launch_count.argtypes = [C.c_void_p]
         L.mt_get_info.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64)]
-        L.mt_measure_peaks.argtypes = [C.c_int, C.POINTER(mt_peaks)]
-        L.mt_probe_field_paths.argtypes = [C.c_int, C.POINTER(mt_field_paths)]
         L.mt_debug_sample.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_philox.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p]
         L.mt_debug_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
+
+
+_probes = None
+
+
+def probes_lib():
+    """Load libmuon_probes.so (include/muon_probes.h): measurement harness for bench.py and the tests, not the product."""
+    global _probes
+    if _probes is None:
+        if not os.path.exists(PROBES_LIB_PATH):
+            raise RuntimeError("libmuon_probes.so is missing: run `python -m paper_2512_10520_b200.build`")
+        L = C.CDLL(PROBES_LIB_PATH)
+        L.mt_measure_peaks.argtypes = [C.c_int, C.POINTER(mt_peaks)]
+        L.mt_probe_field_paths.argtypes = [C.c_int, C.POINTER(mt_field_paths)]
+        _probes = L
+    return _probes
 
 
 class MtError(RuntimeError):
@@ -350,9 +367,9 @@ def mt_get_info(ctx, what):
 
 
 def mt_measure_peaks(device=0):
-    """dict of the measured issue and gather peaks of the device (include/muon_transport.h: mt_peaks)"""
+    """dict of the measured issue and gather peaks of the device (include/muon_probes.h: mt_peaks)"""
     p = mt_peaks()
-    rc = lib().mt_measure_peaks(int(device), C.byref(p))
+    rc = probes_lib().mt_measure_peaks(int(device), C.byref(p))
     if rc != MT_OK:
         raise MtError(rc, "mt_measure_peaks(device=%d)" % device)
     return {name: getattr(p, name) for name, _ in mt_peaks._fields_}
@@ -361,7 +378,7 @@ def mt_measure_peaks(device=0):
 def mt_probe_field_paths(device=0):
     """corner records per second through global loads / texture fetches / a TMA-staged shared-memory window"""
     p = mt_field_paths()
-    rc = lib().mt_probe_field_paths(int(device), C.byref(p))
+    rc = probes_lib().mt_probe_field_paths(int(device), C.byref(p))
     if rc != MT_OK:
         raise MtError(rc, "mt_probe_field_paths(device=%d)" % device)
     return {name: getattr(p, name) for name, _ in mt_field_paths._fields_}

@@ -1,4 +1,5 @@
-"""Build libmuon_transport.so (the C-ABI library) in-tree with nvcc for sm_100a.
+"""Build libmuon_transport.so (the C-ABI library) and libmuon_probes.so (the measurement probes of include/muon_probes.h,
+which only bench.py and the tests load) in-tree with nvcc for sm_100a.
 
     python -m paper_2512_10520_b200.build [--force]
 
@@ -15,8 +16,11 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmuon_transport.so")
 SOURCES = ["mt_lib.cu", "mt_kernels.cu", "mt_inst_regions.cu", "mt_inst_poly.cu", "mt_inst_voxel_a.cu",
-           "mt_inst_voxel_b.cu", "mt_inst_lean.cu", "mt_probe.cu", "mt_probe_field.cu"]
-DEPS = SOURCES + ["mt_kernels.cuh", "mt_step.cuh", "mt_params.h", "mt_launch.h"]
+           "mt_inst_voxel_b.cu", "mt_inst_lean.cu"]
+# the measurement probes (include/muon_probes.h) are a library of their own: bench.py and tests load it, the product does not
+PROBES_LIB = os.path.join(HERE, "libmuon_probes.so")
+PROBE_SOURCES = ["mt_probe.cu", "mt_probe_field.cu"]
+DEPS = SOURCES + PROBE_SOURCES + ["mt_kernels.cuh", "mt_step.cuh", "mt_params.h", "mt_launch.h"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
               "-Xcompiler", "-fPIC,-Wall", "-Xptxas", "-v"]
@@ -39,9 +43,12 @@ def build(force: bool = False, verbose: bool = False, defines=(), checked: bool 
     bounds-checked (csrc/mt_params.h: MT_CHECK); load it through MUON_TRANSPORT_LIB (tests/test_gpu_checked.py)."""
     LIB = CHECKED_LIB if checked else globals()["LIB"]
     defines = tuple(defines) + (("MT_CHECKED",) if checked else ())
-    deps = [os.path.join(CSRC, d) for d in DEPS] + [os.path.join(INCLUDE, "muon_transport.h"), __file__]
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
+    deps = [os.path.join(CSRC, d) for d in DEPS] + [os.path.join(INCLUDE, "muon_transport.h"),
+                                                     os.path.join(INCLUDE, "muon_probes.h"), __file__]
+    targets = [LIB] if checked else [LIB, PROBES_LIB]
+    if not force and all(os.path.exists(t) and all(os.path.getmtime(t) >= os.path.getmtime(d) for d in deps) for t in targets):
         return LIB
+    sources = SOURCES if checked else SOURCES + PROBE_SOURCES
     bdir = os.path.join(HERE, "build")
     os.makedirs(bdir, exist_ok=True)
     tag = ".%d%s" % (os.getpid(), ".chk" if checked else "")
@@ -53,14 +60,15 @@ def build(force: bool = False, verbose: bool = False, defines=(), checked: bool 
         res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
         return obj, cmd, res
 
-    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as pool:
-        done = list(pool.map(compile_one, SOURCES))
+    with ThreadPoolExecutor(max_workers=min(len(sources), os.cpu_count() or 1)) as pool:
+        done = list(pool.map(compile_one, sources))
     log = []
     objs = []
+    probe_objs = []
     try:
         for obj, cmd, res in done:
             log.append(" ".join(cmd) + "\n" + res.stdout)
-            objs.append(obj)
+            (probe_objs if os.path.basename(cmd[-3]) in PROBE_SOURCES else objs).append(obj)
             if res.returncode != 0:
                 sys.stderr.write(res.stdout)
                 raise RuntimeError("nvcc failed compiling " + cmd[-3])
@@ -72,6 +80,15 @@ def build(force: bool = False, verbose: bool = False, defines=(), checked: bool 
             sys.stderr.write(res.stdout)
             raise RuntimeError("nvcc failed linking libmuon_transport.so")
         os.replace(tmp, LIB)
+        if probe_objs:
+            tmp = PROBES_LIB + ".tmp" + tag
+            link = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + probe_objs
+            res = subprocess.run(link, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+            log.append(" ".join(link) + "\n" + res.stdout)
+            if res.returncode != 0:
+                sys.stderr.write(res.stdout)
+                raise RuntimeError("nvcc failed linking libmuon_probes.so")
+            os.replace(tmp, PROBES_LIB)
     finally:
         for obj, _, _ in done:                    # every object this build wrote, also after a failed compile
             if os.path.exists(obj):

@@ -5,7 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "../../include/muon_transport.h"
+#include "../../include/muon_probes.h"
+#include "../../include/muon_transport.h"      // (the MT_ERR_* codes)
 #include "mt_launch.h"
 
 namespace {

@@ -8,10 +8,11 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "muon_transport.h")
+PROBES_HEADER = os.path.join(ROOT, "include", "muon_probes.h")
 
 
-def declared_functions():
-    src = open(HEADER).read()
+def declared_functions(header=HEADER):
+    src = open(header).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(mt_[a-z_]+)\s*\(", src)))
 
@@ -23,6 +24,21 @@ def test_library_exports_every_declared_symbol(mt):
     for n in names:
         assert hasattr(L, n), n
     assert sorted(mt.binding.SYMBOLS) == names
+
+
+def test_probes_live_in_their_own_library(mt):
+    """include/ holds two headers and each has its library: the measurement probes (include/muon_probes.h) are exported by
+    libmuon_probes.so and by it alone — the product boundary carries the transport calls and their documented hooks only."""
+    assert sorted(f for f in os.listdir(os.path.join(ROOT, "include")) if f.endswith(".h")) == ["muon_probes.h", "muon_transport.h"]
+    names = declared_functions(PROBES_HEADER)
+    assert names == sorted(mt.binding.PROBE_SYMBOLS) == ["mt_measure_peaks", "mt_probe_field_paths"]
+    P = ctypes.CDLL(mt.binding.PROBES_LIB_PATH)
+    L = ctypes.CDLL(mt.binding.LIB_PATH)
+    for n in names:
+        assert hasattr(P, n), n
+        assert not hasattr(L, n), n
+    for n in declared_functions():                       # and nothing of the transport ABI leaks into the probes' library
+        assert not hasattr(P, n), n
 
 
 def test_struct_layouts_match_the_header(mt):

@@ -1,4 +1,5 @@
-"""-m gpu: the in-process probes behind bench.py's roofline.measured_peaks (csrc/mt_probe.cu, mt_probe_field.cu) return
+"""-m gpu: the in-process probes behind bench.py's roofline.measured_peaks (include/muon_probes.h, libmuon_probes.so:
+csrc/mt_probe.cu, mt_probe_field.cu — a library of their own, not part of the transport boundary) return
 numbers that are physically ordered and inside the hardware's envelope — a probe whose loop the compiler deleted, or one
 that timed an empty launch, shows up here as a rate above what 148 SMs can issue."""
 import pytest
