@@ -60,7 +60,7 @@ PRECOMPUTED_OPS = {"philox_round_keys": 18, "trilinear_x_differences": 12}
 NCU_LAUNCH_LIST = "profiles/r3_launches.csv"
 NCU_CAPTURE_CONFIG = dict(config=3, muons=10_000_000, field_mode=0, joint=False, poly=False, sched=0, placement=0, block=0,
                           slab=0, lanes=0, sort_every=0, pass_mode=0, no_lean=False, blocks_per_sm=0, min_idle=0,
-                          draws=1_000_000)
+                          draws=1_000_000, n_cells=8, half_width_cells=100)
 
 
 def ncu_capture(args):
@@ -281,13 +281,19 @@ def roofline_block(mode, steps_per_call, t_call_s, launches_per_step, lanes, n_m
 
 
 # ------------------------------------------------------------------------------------------ workload
-def make_workload(config, n_muons, device, rank, joint=False, field_mode=0, poly=False, n_draws=1_000_000):
-    """BASELINE.json configs[config] with this rank's batch of muons (generator batch = rank)."""
+def make_workload(config, n_muons, device, rank, joint=False, field_mode=0, poly=False, n_draws=1_000_000, n_cells=8,
+                  half_width_cells=100):
+    """BASELINE.json configs[config] with this rank's batch of muons (generator batch = rank).  n_cells / half_width_cells:
+    config 3 on another voxel grid (3.75 m of z per shield cell at 1 cm, 2 x half_width_cells cells across; the defaults
+    are configs[3]'s 200x200x3000) — profiles/r3_slab_grids.md."""
     from paper_2512_10520_b200 import workloads as w
     t0 = time.time()
     if config == 3:
-        wl = w.config3(n=8, device=device, joint=joint, field_mode=field_mode, n_draws=n_draws)   # histograms + voxel grids (made on the GPU)
+        wl = w.config3(n=8, device=device, joint=joint, field_mode=field_mode, n_draws=n_draws, n_cells=n_cells,
+                       half_width_cells=half_width_cells)                # histograms + voxel grids (made on the GPU)
         wl.muons = w.spectrum_muons(3, n_muons, "square", batch=rank)
+        if half_width_cells < 100:                                        # a grid narrower than the 2 m start square
+            wl.muons.pos_q[:, :2] *= np.float32(half_width_cells * 0.01)
     elif config == 2:
         # --poly: config 2's muons and tables in the tapered-magnet polyhedra geometry (DESIGN.md §3.12)
         wl = w.config2p(n=8, joint=joint, n_draws=n_draws) if poly else w.config2(n=8, joint=joint, n_draws=n_draws)
@@ -340,7 +346,8 @@ def run_reference(args, rank, world):
         return
     import torch
     dev = "cuda" if torch.cuda.is_available() else "cpu"          # the grid generator may use the GPU; the timed code never does
-    wl = make_workload(args.config, args.muons, dev, 0, args.joint, args.field_mode, args.poly, args.draws)
+    wl = make_workload(args.config, args.muons, dev, 0, args.joint, args.field_mode, args.poly, args.draws, args.n_cells,
+                       args.half_width_cells)
     cores, desc, runner = oracle_sample(wl, args.muons, 0, args.ref_seconds, threads=args.ref_threads or None)
     for _ in range(args.warmup):
         runner()
@@ -385,7 +392,8 @@ def run_ours(args, rank, world, local_rank):
     from paper_2512_10520_b200.sharding import gather_ranges, reduce_job, weak_shard
     shard = weak_shard(args.muons, rank, world)               # own batch, own id range, no collective
     n, id_base = shard.n, shard.id_base
-    wl = make_workload(args.config, n, dev, rank, args.joint, args.field_mode, args.poly, args.draws)
+    wl = make_workload(args.config, n, dev, rank, args.joint, args.field_mode, args.poly, args.draws, args.n_cells,
+                       args.half_width_cells)
     mode = {0: "regions", 1: "voxel", 2: "poly"}[wl.geom.mode]
     grid_bytes = 32 * (wl.geom.nx + 2) * (wl.geom.ny + 2) * (wl.geom.nz + 2) if mode == "voxel" else 0
     h = b.MuonTransport(local_rank).setup(wl.hist, wl.geom, args.placement)
@@ -494,7 +502,8 @@ def run_ours(args, rank, world, local_rank):
                    "lanes": lanes_used,
                    "parallelism": "id-range sharding x%d, replicated tables and grids, no collective" % world,
                    "id_ranges": id_ranges,
-                   "l2": "inputs larger than L2 (320 MB muon state, 1.9 GB field grid per step)",
+                   "l2": "inputs larger than L2 (%d MB muon state in + out, %d MB field grid per step)" % (64 * n // 10 ** 6, grid_bytes // 10 ** 6),
+                   "grid": [wl.geom.nx, wl.geom.ny, wl.geom.nz] if mode == "voxel" else None,
                    "flags_rank0": {"stopped": int(flags[0]), "exited": int(flags[1]), "escaped": int(flags[2]),
                                    "maxsteps": int(flags[3])}},
         "e2e": {"value": e2e_value, "unit": "muon-steps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -681,6 +690,8 @@ def main():
     ap.add_argument("--field-mode", type=int, default=0, help="MT_FIELD_*: 1 nearest, 2 per-stage, 3 both (DESIGN.md 3.11)")
     ap.add_argument("--no-lean", action="store_true", help="MT_OPT_NO_LEAN: general kernels even where the lean variant applies")
     ap.add_argument("--poly", action="store_true", help="with --config 2: the convex-polyhedra shield (DESIGN.md 3.12)")
+    ap.add_argument("--n-cells", type=int, default=8, help="config 3: shield cells along z, 375 grid layers each (8 = configs[3])")
+    ap.add_argument("--half-width-cells", type=int, default=100, help="config 3: half the grid's width in cells (100 = configs[3])")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] (table shapes, muons per launch)")
     ap.add_argument("--probes", action="store_true", help="only the in-process peak and field-path probes (one JSON line)")
     ap.add_argument("--draws", type=int, default=1_000_000, help="draws per generated histogram (BASELINE.json: 10^6)")

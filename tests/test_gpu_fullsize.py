@@ -91,3 +91,25 @@ def test_polyhedral_shield_at_bench_size(mt, oracle, workloads):
         assert took["schedule"] == b.MT_SCHED_WAVEFRONT and took["lanes"] == 2
     finally:
         h.close()
+
+
+@pytest.mark.parametrize("half_width_cells,n_cells", [(50, 8), (200, 4)])
+def test_other_voxel_grids_under_the_default_slab(mt, oracle, workloads, half_width_cells, n_cells):
+    """The AUTO slab and CTA shape were tuned on configs[3]'s 200x200x3000 grid (1.3 MB per padded layer).  Grids with a
+    quarter and four times that layer — 100x100x3000 and 400x400x1500, where 96 layers are 32 MB and 500 MB against 126 MB
+    of L2 — go through the same full-batch launch path (2.5e6 muons: one lane, 96-cell slabs); every 50th muon against the
+    oracle.  (profiles/r3_slab_grids.md has the slab sweep on the three grids: AUTO is within 0.8 % of the best fixed slab.)"""
+    import torch
+    b = mt.binding
+    need_device_memory(24)
+    n = 2_500_000
+    wl = workloads.config3(n=n, n_draws=200_000, n_cells=n_cells, half_width_cells=half_width_cells, device="cuda")
+    h = b.MuonTransport(0).setup(wl.hist, wl.geom)
+    try:
+        took = _sampled(mt, oracle, wl, h, 50, 3 * n, "voxel grid %dx%dx%d" % (wl.geom.nx, wl.geom.ny, wl.geom.nz))
+        assert took["schedule"] == b.MT_SCHED_WAVEFRONT and took["lanes"] == 1
+    finally:
+        h.close()
+        wl.geom.material = wl.geom.field = None
+        del wl
+        torch.cuda.empty_cache()
